@@ -1,0 +1,315 @@
+#!/usr/bin/env python
+"""bench.py -- one JSON line for the deposit + fold + apply + return step (BASELINE.json metric).
+
+A "step" is one pass of the whole hot path (pm_deposit, pm_fold_ghosts, pm_apply_limited,
+pm_return_to_particles) over the synthetic config-5 workload (512^3 cells, 10^6 particles), all inputs
+resident in HBM.  `value` = cell-updates per second (whole job), timed with CUDA events on the stream the
+kernels are launched on, barrier + synchronize on both sides, max over ranks.  `e2e` = the same metric through
+pm_step_host with pinned HOST buffers (H2D + D2H inside the timed region).  Multi-GPU: the path does not
+shard (north_star: one GPU, no collectives), so `--gpus N` runs N independent replicas ("replicas only").
+
+`--impl reference` times the CPU oracle (oracle/pm_oracle.c) as it stands on a bounded sample.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "deposit+fold+apply+return step throughput at 512^3, 1e6 particles"
+UNIT = "Mcell-updates/s"
+ORACLE_SAMPLE_N = 256            # config-5-shaped block the oracle is timed on (same particles per cell)
+
+
+def env_int(name, default):
+    try:
+        return int(os.environ.get(name, default))
+    except ValueError:
+        return default
+
+
+# ---------------------------------------------------------------------------------------------
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.proc = None
+        self.lines = []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for ln in self.lines:
+            p = [x.strip() for x in ln.split(",")]
+            if len(p) < 7:
+                continue
+            try:
+                sm.append(float(p[0])); mx.append(float(p[1]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, p[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def measured_peak():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
+
+
+def ncu_traffic(kernel: str):
+    """DRAM bytes per launch from the committed ncu --set full capture, if recorded (profiles/ncu_traffic.json)."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "ncu_traffic.json")) as f:
+            return json.load(f).get(kernel)
+    except Exception:
+        return None
+
+
+# ---------------------------------------------------------------------------------------------
+def time_oracle(n: int, steps: int):
+    """The oracle, as it stands, single-threaded, on a config-5-shaped n^3 block with the same particles per cell."""
+    from oracle import pm_oracle as po
+    from paper_2509_18261_b200 import inputs
+    npart = int(round(1_000_000 * (n / 512.0) ** 3))
+    w = inputs.scaled_mixed(n, npart, seed_index=5)
+    o = po.Oracle(w.params, w.state, w.sinks, w.sne, keep_abs=False)
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        o.step(w.dt)
+    dt = (time.perf_counter() - t0) / steps
+    return {"value": n ** 3 / dt / 1e6, "unit": UNIT, "cores": 1, "kind": "oracle",
+            "sample": f"config-5-shaped {n}^3 block, {npart} particles (same particles per cell), {steps} step(s), "
+                      f"{dt:.2f} s per step, particles/s = {npart / dt:.3e}",
+            "seconds_per_step": dt, "particles_per_s": npart / dt}
+
+
+def run_reference(args, rank, world):
+    if rank != 0:
+        return
+    steps = max(1, min(args.steps, 2))
+    r = time_oracle(ORACLE_SAMPLE_N, steps)
+    line = {"impl": "reference", "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": r["seconds_per_step"] * 1e3,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "config5_large_512 (oracle timed on a bounded sample)", "sample": r["sample"]},
+            "cpu_baseline": {k: r[k] for k in ("value", "unit", "cores", "kind", "sample")},
+            "e2e": {"value": r["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# ---------------------------------------------------------------------------------------------
+def run_ours(args, rank, world, local_rank):
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    from paper_2509_18261_b200 import inputs, pm
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the CUDA path has no CPU fallback")
+    dev = torch.device(f"cuda:{local_rank}")
+    torch.cuda.set_device(dev)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    n = args.n
+    if n == 512 and args.particles == 1_000_000:
+        w = inputs.make(5)
+    else:
+        w = inputs.scaled_mixed(n, args.particles, seed_index=5)
+    N = n ** 3
+    npart = w.sinks.n + w.sne.n
+    ctx = pm.Context(w.params, device=str(dev))
+    st = pm.DeviceState.from_host(w.state, dev)
+    sk = pm.DeviceSinks.from_host(w.sinks, dev)
+    sn = pm.DeviceSNe.from_host(w.sne, dev)
+    stage_names = ("deposit", "fold", "apply", "return")
+
+    def one_step(ev=None):
+        if ev: ev[0].record()
+        ctx.pm_deposit(st, sk, sn, w.dt)
+        if ev: ev[1].record()
+        ctx.pm_fold_ghosts()
+        if ev: ev[2].record()
+        ctx.pm_apply_limited(st)
+        if ev: ev[3].record()
+        ctx.pm_return_to_particles(sk)
+        if ev: ev[4].record()
+
+    for _ in range(max(args.warmup, 3)):
+        one_step()
+    ctx.pm_check()
+    # activity fractions of the buffer the timed steps will see (for the algorithmic-bytes figure)
+    ctx.pm_deposit(st, sk, sn, w.dt)
+    ctx.pm_fold_ghosts()
+    own = [ctx.debug_buffer(ch)[1] for ch in range(6)]
+    sink_touched = own[0] != 0
+    touched = sink_touched.clone()
+    for ch in range(1, 6):
+        touched |= own[ch] != 0
+    t_frac, ts_frac = float(touched.double().mean()), float(sink_touched.double().mean())
+    del touched, sink_touched, own
+    ctx.pm_apply_limited(st)
+    ctx.pm_return_to_particles(sk)
+
+    sampler = ClockSampler(local_rank)
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(5)] for _ in range(args.steps)]
+    launches0 = ctx.pm_launch_count()
+    barrier()
+    sampler.start()
+    for it in range(args.steps):
+        one_step(evs[it])
+    barrier()
+    clocks = sampler.stop()
+    launches = ctx.pm_launch_count() - launches0
+    ctx.pm_check()
+    total_ms = evs[0][0].elapsed_time(evs[-1][4])
+    stage_ms = {nm: sum(e[i].elapsed_time(e[i + 1]) for e in evs) / args.steps for i, nm in enumerate(stage_names)}
+    t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    total_ms = float(t[0])
+    ms_per_step = total_ms / args.steps
+    value = world * N * args.steps / (total_ms * 1e-3) / 1e6
+
+    # ---- e2e through pm_step_host with pinned host buffers --------------------------------------
+    e2e_steps = max(1, min(args.steps, args.e2e_steps))
+    hst = inputs.State(*(torch.from_numpy(f).pin_memory() for f in w.state.fields()))
+    hk = w.sinks.copy()
+    for f in ("dm", "dpx", "dpy", "dpz"):
+        setattr(hk, f, np.zeros(hk.n))
+    ctx2 = ctx                                  # same ctx: staging is allocated on first use
+    del st
+    torch.cuda.empty_cache()
+    ctx2.pm_step_host(hst, hk, w.sne, w.dt)     # warm-up (allocates staging)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        ctx2.pm_step_host(hst, hk, w.sne, w.dt)
+    torch.cuda.synchronize(dev)
+    e2e_s = (time.perf_counter() - t0) / e2e_steps
+    te = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(te, op=dist.ReduceOp.MAX)
+    e2e_s = float(te[0])
+    h2d = 6 * N * 8 + 7 * w.sinks.n * 8 + 8 * w.sne.n * 8
+    d2h = 6 * N * 8 + 8 * w.sinks.n * 8
+
+    if rank == 0:
+        peak, peak_src = measured_peak()
+        # algorithmic bytes of the dominant kernel (k_apply_limited), DESIGN.md "Algorithmic bytes":
+        # every cell reads its 6 buffer words; a touched cell reads + writes 6 state words; a cell a sink
+        # removed mass from also writes the 4 return words.
+        apply_bytes = N * (48.0 + 96.0 * t_frac + 32.0 * ts_frac)
+        dense_bytes = N * 176.0
+        apply_s = stage_ms["apply"] * 1e-3
+        step_bytes = None
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": w.name, "cells": N, "particles": npart, "sinks": w.sinks.n, "sne": w.sne.n,
+                       "multi_gpu": "replicas only" if world > 1 else "single GPU",
+                       "l2_policy": "inputs larger than L2 (state 6 fields + 6-channel buffer, GBs >> 126 MB)",
+                       "touched_cell_fraction": t_frac, "sink_touched_fraction": ts_frac},
+            "particles_per_s": world * npart * args.steps / (total_ms * 1e-3),
+            "stage_ms": stage_ms,
+            "clocks": clocks,
+            "e2e": {"value": world * N / e2e_s / 1e6, "unit": UNIT, "h2d_bytes_per_step": h2d,
+                    "d2h_bytes_per_step": d2h, "ms_per_step": e2e_s * 1e3, "steps": e2e_steps,
+                    "api": "pm_step_host (pinned host buffers)"},
+            "gpu_launches": launches,
+            "roofline": {"bound": "hbm", "kernel": "k_apply_limited", "achieved": apply_bytes / apply_s / 1e9,
+                         "peak": peak, "unit": "GB/s", "frac": apply_bytes / apply_s / 1e9 / peak,
+                         "peak_source": peak_src, "traffic": ncu_traffic("k_apply_limited"),
+                         "algorithmic_bytes_per_launch": apply_bytes,
+                         "dense_equivalent_gbs": dense_bytes / apply_s / 1e9,
+                         "frac_of_8tbs_nominal": apply_bytes / apply_s / 1e9 / 8000.0},
+        }
+        # whole-step roofline (SURVEY 8(d) algorithmic bytes of the step, with the same activity fractions)
+        Nb = (n + 8) ** 3
+        step_bytes = (8.0 * 6 * Nb                       # buffer written once
+                      + 8.0 * 5 * min(1.0, t_frac) * N   # gather reads, each touched state cell once (upper bound)
+                      + 8.0 * 15 * npart                 # particle records
+                      + 3 * 8.0 * 6 * (Nb - N)           # fold
+                      + apply_bytes
+                      + 8.0 * 4 * ts_frac * N)           # return reads
+        line["step_roofline"] = {"algorithmic_bytes_per_step": step_bytes,
+                                 "achieved_gbs": step_bytes / (ms_per_step * 1e-3) / 1e9,
+                                 "frac_of_measured_peak": step_bytes / (ms_per_step * 1e-3) / 1e9 / peak,
+                                 "frac_of_8tbs_nominal": step_bytes / (ms_per_step * 1e-3) / 1e9 / 8000.0}
+        if world == 1 and not args.no_cpu_baseline:
+            r = time_oracle(ORACLE_SAMPLE_N, 1)
+            line["cpu_baseline"] = {k: r[k] for k in ("value", "unit", "cores", "kind", "sample")}
+        line["context"] = "paper: ~50% weak-scaling efficiency to 8192 MI250X GPUs on Frontier (PAPER.md L9, L437); no throughput published"
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--n", type=int, default=512, help="cells per side (default: config 5)")
+    ap.add_argument("--particles", type=int, default=1_000_000)
+    ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    rank, world, local_rank = env_int("RANK", 0), env_int("WORLD_SIZE", 1), env_int("LOCAL_RANK", 0)
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+    else:
+        run_ours(args, rank, world, local_rank)
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,163 @@
+/*
+ * pm.h -- C ABI of libpm_b200: one particle-mesh-particle exchange step on one B200 (sm_100a).
+ *
+ * Method: arxiv 2509.18261 (He et al.), /root/reference/PAPER.md.  "L" numbers are PAPER.md lines,
+ * "R" numbers are the readings listed in DESIGN.md.
+ *
+ *   pm_deposit             Step 1, Eq. 2 (L59-65) with the sink recipe of Sec. 3.1.1 (Eqs. 7-11, 13; L117-159)
+ *                          and the supernova recipe of Sec. 3.2.1 (Eqs. 17-20; L203-230): every particle adds its
+ *                          deposition function dU^s_ijk into a ghost-zoned buffer mesh with fp64 atomic additions.
+ *   pm_fold_ghosts         Step 2, Eq. 3 (L67-71): ghost-zone contents are added to the owning real zones.  On one
+ *                          GPU the "other rank" is the periodic image, so this is an in-device periodic fold.
+ *   pm_apply_limited       Steps 3 + 5, Eqs. 4 and 6 (L73-77, L89-93) fused: the cell-wise limiters (Eqs. 15-16,
+ *                          L161-171, with BASELINE's max-removable-fraction and density floor; Eq. 21) and
+ *                          U := U + eta dU^sum, in place on the caller's conserved state.
+ *   pm_return_to_particles Step 4, Eq. 5 (L79-87): u_s := u_s - sum_ijk eta_ijk dU^s_ijk V_ijk for every sink
+ *                          (supernova particles skip this step, L201).
+ *
+ * All pointers inside pm_state / pm_sinks / pm_sne are DEVICE pointers (cudaMalloc'ed by the caller, e.g. torch
+ * allocations) unless a function says "host".  Every array is fp64, contiguous.  Mesh fields hold nx*ny*nz values,
+ * x fastest ((k*ny + j)*nx + i), no ghost zones, periodic in all three directions.  The library never frees or
+ * reallocates caller memory.  The ctx owns: the ghost-zoned buffer mesh (6 channels), the return mesh (eta and the
+ * pre-step cell velocity, 4 words per cell, written where a sink removed mass), per-particle scratch.
+ *
+ * Execution: every call enqueues kernels on the ctx's CUDA stream and returns without synchronising the host
+ * (except pm_step_host, pm_check and pm_destroy).  Within a step the calls must come in the order
+ * deposit -> fold -> apply -> return (return may be skipped when there are no sinks); otherwise PM_EORDER.
+ * The buffer mesh stays valid (as dU^sum, L108) until the next pm_deposit, which resets it.
+ *
+ * Errors: every function returns 0 on success or a negative pm_status; no exceptions, no aborts, no output.
+ * pm_last_error(ctx) gives a human-readable message for the last failure on that ctx.
+ */
+#ifndef PM_B200_H
+#define PM_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    PM_OK = 0,
+    PM_EINVAL = -1,   /* null / misaligned pointer, bad parameter, grid smaller than 2g+1 cells, particle count changed */
+    PM_ENOMEM = -2,   /* device allocation failed */
+    PM_ECUDA = -3,    /* a CUDA call or kernel failed (sticky); text in pm_last_error */
+    PM_EORDER = -4,   /* call sequence violated */
+    PM_EDOMAIN = -5   /* a particle lies outside [x0, x0 + n dx); detected on device, reported by pm_check / pm_step_host */
+} pm_status;
+
+/* supernova regime selector, Eq. 19 (L223) */
+enum { PM_SN_AUTO = 0, PM_SN_FORCE_EJ = 1, PM_SN_FORCE_ST = 2, PM_SN_FORCE_MC = 3 };
+
+/* Plain data, copied at pm_create.  Units are the caller's; nothing is assumed about them. */
+typedef struct {
+    int32_t nx, ny, nz;          /* owned cells per axis (periodic); each must be >= 2g+1, g = ghost width */
+    int32_t sn_nsub;             /* omega sub-samples per axis, 1..8 (R17); 1 = binary centre test */
+    int32_t sn_regime;           /* PM_SN_* */
+    int32_t flags;               /* PM_FLAG_* */
+    double dx;                   /* cell size; V_ijk = dx^3 (uniform mesh, R33) */
+    double x0[3];                /* lower corner of cell (0,0,0) */
+    double G, gamma;             /* gravitational constant; adiabatic index for c_s^2 = gamma (gamma-1) e_int/rho */
+    double cs_iso;               /* > 0: use this constant sound speed instead (R6) */
+    double rk_sink, rk_sn;       /* kernel radii r_K in length units (L117, L201); 0 = that particle kind is unused */
+    double bondi_lambda;         /* lambda of Eq. 8; e^{3/2}/4 in the paper (L130) */
+    double f_max_remove;         /* largest fraction of a cell's mass sinks may remove per step (L161: 0.25) */
+    double rho_floor;            /* accretion never takes a cell below this density */
+    double sn_eps_k, sn_rm_ej, sn_rm_mc;     /* 0.28, 0.027, 1 (L223-225) */
+    double sn_msf_coeff, sn_msf_exp;         /* M_sf = coeff (n_H / nh_unit)^exp (L203) */
+    double sn_psnr_coeff, sn_psnr_exp;       /* P_snr = coeff (n_H / nh_unit)^exp, Eq. 20 (L229) */
+    double sn_mu_h, sn_nh_unit;              /* mass per H nucleus; unit of n_H */
+    double sn_eint_theta;        /* Eq. 21 floor: e_min = theta rho_2 (e_int,1/rho_1); 1 = as printed, 0 = e_int >= 0 only (R25) */
+} pm_params;
+
+enum {
+    PM_FLAG_DEBUG_SCALARS = 1,   /* keep per-particle scalars (pm_debug_sink_scalars / pm_debug_sn_scalars) */
+    PM_FLAG_DEBUG_LAMBDA = 2     /* keep the Eq. 21 lambda of every cell (pm_debug_lambda) */
+};
+
+typedef struct { double *rho, *mx, *my, *mz, *etot, *eint; } pm_state;
+
+/* Sink particles, u_s = (m, m v) (L49).  x,y,z are never modified.  dm, dpx, dpy, dpz are optional outputs
+ * (may be NULL): the mass and momentum actually returned to each sink in this step (Eq. 5). */
+typedef struct {
+    int64_t n;
+    const double *x, *y, *z;
+    double *vx, *vy, *vz, *m;
+    double *dm, *dpx, *dpy, *dpz;
+} pm_sinks;
+
+/* Supernova particles exploding in this step (never modified, L201). */
+typedef struct {
+    int64_t n;
+    const double *x, *y, *z, *vx, *vy, *vz, *e_sn, *m_ej;
+} pm_sne;
+
+typedef struct pm_ctx pm_ctx;
+
+/* Create a context on CUDA device `device`, launching on `cuda_stream` (a cudaStream_t; NULL = default stream).
+ * Allocates the buffer mesh ((n+2g)^3 x 6 channels) and, if rk_sink > 0, the return mesh (4 n^3 words). */
+int pm_create(const pm_params *params, int device, void *cuda_stream, pm_ctx **out);
+
+/* Step 1.  Resets the buffer mesh, then deposits every sink and SN (reading the PRE-step state).  sinks / sne may be
+ * NULL or have n == 0.  dt is the time step of Eq. 13.  Caches per-sink scalars (mdot, r_acc, sum w) for Step 4. */
+int pm_deposit(pm_ctx *ctx, const pm_state *state, const pm_sinks *sinks, const pm_sne *sne, double dt);
+
+/* Step 2.  Adds every ghost cell's contents to the periodically wrapped owned cell, in a fixed image order (the sum
+ * order of a cell is the same in every run, cf. Appendix A).  Ghost cells keep their values. */
+int pm_fold_ghosts(pm_ctx *ctx);
+
+/* Steps 3 + 5.  In place on the caller's state.  Leaves eta and the pre-step velocity for Step 4. */
+int pm_apply_limited(pm_ctx *ctx, pm_state *state);
+
+/* Step 4.  Must be given the same sinks (same n, same positions) as the preceding pm_deposit. */
+int pm_return_to_particles(pm_ctx *ctx, pm_sinks *sinks);
+
+/* Synchronise the ctx's stream and report PM_ECUDA / PM_EDOMAIN raised by earlier asynchronous work. */
+int pm_check(pm_ctx *ctx);
+
+/* One whole step with HOST buffers (the end-to-end path): copies state and particles host -> device into
+ * ctx-owned staging (allocated on first use), runs deposit, fold, apply, return, copies the state and the sink
+ * fields (vx, vy, vz, m and the optional dm, dp*) back, and synchronises.  All pointers in the three structs are
+ * HOST pointers here (pinned memory recommended). */
+int pm_step_host(pm_ctx *ctx, pm_state *host_state, pm_sinks *host_sinks, const pm_sne *host_sne, double dt);
+
+int pm_destroy(pm_ctx *ctx);
+
+const char *pm_last_error(const pm_ctx *ctx);
+
+/* Number of kernels this ctx has launched so far (bench.py's gpu_launches). */
+int64_t pm_launch_count(const pm_ctx *ctx);
+
+/* ---- test-only views (not timed) ---------------------------------------------------------------------------- */
+
+/* Buffer channel 0 = accretion d rho^sum (signed, <= 0, R1); 1..5 = SN d rho, d px, d py, d pz, d E.
+ * The channel is a contiguous (dims[0], dims[1], dims[2]) = (nz+2g, ny+2g, row pitch) array, x fastest; the row pitch
+ * is nx + 2*gx with gx = g rounded up to even (keeps 128-bit accesses aligned).  *origin = element offset of owned
+ * cell (0,0,0); owned cell (i,j,k) sits at origin + (k*dims[1] + j)*dims[2] + i, ghost cells at i,j,k in [-g, n+g).
+ * *ghost = g. */
+int pm_debug_buffer(pm_ctx *ctx, int channel, const double **dev_ptr, int64_t dims[3], int64_t *origin, int32_t *ghost);
+
+/* Return mesh word 0 = eta (Eq. 4), 1..3 = pre-step cell velocity; nx*ny*nz each, valid where buffer channel 0 != 0. */
+int pm_debug_return_mesh(pm_ctx *ctx, int word, const double **dev_ptr);
+
+/* lambda of Eq. 21 per cell (needs PM_FLAG_DEBUG_LAMBDA). */
+int pm_debug_lambda(pm_ctx *ctx, const double **dev_ptr);
+
+/* Per-particle scalars (need PM_FLAG_DEBUG_SCALARS), SoA with stride n:
+ * sinks: 0 rho_inf, 1 v_inf, 2 c_inf, 3 r_BH, 4 mdot, 5 r_acc, 6 sum w, 7 member count
+ * SNe:   0 M_snr, 1 V_snr, 2..4 v_COM, 5 n_H, 6 R_M, 7 |p_radial|, 8 regime (1 EJ, 2 ST, 3 MC) */
+int pm_debug_sink_scalars(pm_ctx *ctx, const double **dev_ptr, int64_t *n);
+int pm_debug_sn_scalars(pm_ctx *ctx, const double **dev_ptr, int64_t *n);
+
+/* Stencil of ONE particle at (x,y,z), evaluated by the same device code the deposit uses.  kind 0 = sink: writes
+ * 1 (member) / 0 for every cell of the (2g+1)^3 box; kind 1 = SN: writes the omega sub-sample count.  Box cells in
+ * (k, j, i) order into dev_counts (DEVICE pointer, int32, >= (2g+1)^3 entries); host_ijk (HOST, 3 ints) receives
+ * the host cell, *side (HOST) the box side.  Synchronises. */
+int pm_debug_stencil(pm_ctx *ctx, int kind, double x, double y, double z, int32_t *dev_counts, int32_t *host_ijk,
+                     int32_t *side);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PM_B200_H */

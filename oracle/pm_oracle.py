@@ -146,14 +146,14 @@ SN_DIAG = ("m_snr", "v_snr", "vcx", "vcy", "vcz", "n_h", "r_m", "p_rad")
 class Oracle:
     """Holds one problem (params, state, particles; all numpy, modified in place by step())."""
 
-    def __init__(self, params: dict, state, sinks, sne, keep_abs: bool = True):
+    def __init__(self, params: dict, state, sinks, sne, keep_abs: bool = True, mesh: bool = True):
         self.L = lib()
         self.pd = dict(params)
         self.p = make_params(params)
         self.state, self.sinks, self.sne = state, sinks, sne
         self.N = int(params["nx"]) * int(params["ny"]) * int(params["nz"])
         self.shape = (int(params["nz"]), int(params["ny"]), int(params["nx"]))
-        N = self.N
+        N = self.N if mesh else 0          # mesh=False: only sample_cells / particle_scalars / sink_amounts are used
         self.A = [np.zeros(N) for _ in range(6)]
         self.S = [np.zeros(N) for _ in range(5)]
         self.Aabs = [np.zeros(N) for _ in range(6)] if keep_abs else [None] * 6

@@ -1,0 +1,716 @@
+// pm_b200.cu -- kernels and C ABI of libpm_b200 (see include/pm.h).  sm_100a only; built with -fmad=false.
+//
+// Kernels:
+//   k_zero_buffer      a0  buffer reset, 128-bit stores
+//   k_deposit_sinks    a1-a3  one warp per sink: kernel means -> Bondi-Hoyle rate -> Gaussian weights -> fp64 RED
+//   k_deposit_sne      a1,a4,a5  one warp per SN: omega counts -> stencil sums -> Eq. 17 -> fp64 RED (5 channels)
+//   k_fold_ghosts      a6  gather fold: every owned cell within g of a face sums its <= 7 ghost images, fixed order
+//   k_apply_limited    a7  fused limiter + apply, 128-bit loads/stores, untouched cells skip the state traffic
+//   k_return_sinks     a8  one warp per sink: sum eta a V (1, v_old) with a shuffle reduction
+#include "pm_device.cuh"
+#include "../../include/pm.h"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+using namespace pm;
+
+// ---------------------------------------------------------------------------------------------------------------
+// context
+// ---------------------------------------------------------------------------------------------------------------
+enum Stage { ST_IDLE = 0, ST_DEPOSITED = 1, ST_FOLDED = 2, ST_APPLIED = 3 };
+
+struct pm_ctx {
+    pm_params prm;
+    DevP P;
+    int device;
+    cudaStream_t stream;
+    double *buf;        // kBufChannels * Nb
+    double *ret;        // kRetWords * N (NULL when rk_sink == 0)
+    double *lam;        // N (debug only)
+    double *sink_scal;  // 3 * cap_sinks: mdot, r_acc, sum w
+    long long cap_sinks;
+    double *dbg_sink;   // 8 * cap
+    long long cap_dbg_sink;
+    double *dbg_sn;     // 9 * cap
+    long long cap_dbg_sn;
+    int *err_flag;      // device
+    int *err_host;      // pinned
+    Stage stage;
+    long long n_sinks_dep, n_sne_dep;
+    double dt;
+    long long launches;
+    // host-step staging
+    double *stg_state;  long long stg_state_cap;
+    double *stg_sinks;  long long stg_sinks_cap;
+    double *stg_sne;    long long stg_sne_cap;
+    char msg[256];
+};
+
+#define PM_FAIL(ctx, code, ...) do { snprintf((ctx)->msg, sizeof((ctx)->msg), __VA_ARGS__); return (code); } while (0)
+#define PM_CUDA(ctx, call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { \
+    snprintf((ctx)->msg, sizeof((ctx)->msg), "%s failed: %s", #call, cudaGetErrorString(e_)); return PM_ECUDA; } } while (0)
+
+static int check_launch(pm_ctx *c, const char *name) {
+    cudaError_t e = cudaGetLastError();
+    c->launches += 1;
+    if (e != cudaSuccess) { snprintf(c->msg, sizeof(c->msg), "launch of %s failed: %s", name, cudaGetErrorString(e)); return PM_ECUDA; }
+    return PM_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// a0: buffer reset
+// ---------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_zero_buffer(double2 *__restrict__ p, long long n2) {
+    long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    const double2 z = make_double2(0.0, 0.0);
+    for (; i < n2; i += stride) p[i] = z;
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// a1-a3: sinks.  One warp per sink; lanes stride over the (2g+1)^3 box in (k,j,i) order.
+// ---------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(128) k_deposit_sinks(const DevP P, const DevState U, const DevSinks S, const double dt,
+                                                       double *__restrict__ buf0, double *__restrict__ scal,
+                                                       double *__restrict__ dbg, int *__restrict__ err) {
+    const long long s = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int lane = threadIdx.x & 31;
+    if (s >= S.n) return;
+    const double xs = S.x[s], ys = S.y[s], zs = S.z[s];
+    const int ih = host_cell(xs, P.x0[0], P.inv_dx), jh = host_cell(ys, P.x0[1], P.inv_dx), kh = host_cell(zs, P.x0[2], P.inv_dx);
+    if (ih < 0 || ih >= P.nx || jh < 0 || jh >= P.ny || kh < 0 || kh >= P.nz) {
+        if (lane == 0) { atomicOr(err, 1); scal[s] = 0.0; scal[S.n + s] = 1.0; scal[2 * S.n + s] = 1.0; }
+        return;
+    }
+    const double vsx = S.vx[s], vsy = S.vy[s], vsz = S.vz[s], ms = S.m[s];
+    const int g = P.gs, B = 2 * g + 1, nc = B * B * B;
+    double sum_rho = 0.0, srx = 0.0, sry = 0.0, srz = 0.0, src = 0.0;
+    int cnt = 0;
+    for (int c = lane; c < nc; c += 32) {
+        const int a = c % B, t = c / B, b = t % B, cc = t / B;
+        const int i = ih - g + a, j = jh - g + b, k = kh - g + cc;
+        const double r2 = dist2(cell_centre(P.x0[0], i, P.dx) - xs, cell_centre(P.x0[1], j, P.dx) - ys,
+                                cell_centre(P.x0[2], k, P.dx) - zs);
+        if (r2 <= P.rk2_sink) {
+            const long long q = owned_index(P, i, j, k);
+            const double rho = U.rho[q];
+            const double vx = U.mx[q] / rho, vy = U.my[q] / rho, vz = U.mz[q] / rho;
+            const double cs = sound_speed(P, rho, U.eint[q]);
+            sum_rho += rho;
+            srx += rho * (vx - vsx);
+            sry += rho * (vy - vsy);
+            srz += rho * (vz - vsz);
+            src += rho * cs;
+            cnt += 1;
+        }
+    }
+    sum_rho = warp_sum(sum_rho); srx = warp_sum(srx); sry = warp_sum(sry); srz = warp_sum(srz); src = warp_sum(src);
+    cnt = warp_sum_int(cnt);
+    const SinkScalars sc = sink_scalars(P, sum_rho, srx, sry, srz, src, cnt, ms);
+    const double ra2 = sc.r_acc * sc.r_acc;
+    double wsum = 0.0;
+    for (int c = lane; c < nc; c += 32) {
+        const int a = c % B, t = c / B, b = t % B, cc = t / B;
+        const double r2 = dist2(cell_centre(P.x0[0], ih - g + a, P.dx) - xs, cell_centre(P.x0[1], jh - g + b, P.dx) - ys,
+                                cell_centre(P.x0[2], kh - g + cc, P.dx) - zs);
+        if (r2 <= P.rk2_sink) wsum += exp(-r2 / ra2);
+    }
+    wsum = warp_sum(wsum);
+    for (int c = lane; c < nc; c += 32) {
+        const int a = c % B, t = c / B, b = t % B, cc = t / B;
+        const int i = ih - g + a, j = jh - g + b, k = kh - g + cc;
+        const double r2 = dist2(cell_centre(P.x0[0], i, P.dx) - xs, cell_centre(P.x0[1], j, P.dx) - ys,
+                                cell_centre(P.x0[2], k, P.dx) - zs);
+        if (r2 <= P.rk2_sink) {
+            const double amt = sink_cell_amount(P, r2, sc.r_acc, wsum, sc.mdot, dt);
+            atomicAdd(buf0 + ghost_index(P, i, j, k), -amt);          // R1: signed change
+        }
+    }
+    if (lane == 0) {
+        scal[s] = sc.mdot; scal[S.n + s] = sc.r_acc; scal[2 * S.n + s] = wsum;
+        if (dbg) {
+            const long long n = S.n;
+            dbg[s] = sc.rho_inf; dbg[n + s] = sc.v_inf; dbg[2 * n + s] = sc.c_inf; dbg[3 * n + s] = sc.r_bh;
+            dbg[4 * n + s] = sc.mdot; dbg[5 * n + s] = sc.r_acc; dbg[6 * n + s] = wsum; dbg[7 * n + s] = (double)cnt;
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// a1, a4, a5: supernovae.  One warp per SN; per-warp shared tables for the omega sub-sampling.
+// ---------------------------------------------------------------------------------------------------------------
+constexpr int kSnWarps = 8;
+
+__global__ void __launch_bounds__(kSnWarps * 32) k_deposit_sne(const DevP P, const DevState U, const DevSNe S,
+                                                                double *__restrict__ buf, double *__restrict__ dbg,
+                                                                int *__restrict__ err) {
+    extern __shared__ __align__(16) unsigned char smem[];
+    const int wib = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const long long s = (long long)blockIdx.x * kSnWarps + wib;
+    if (s >= S.n) return;
+    const int g = P.gn, B = 2 * g + 1, nc = B * B * B;
+    const SnTables T = sn_tables_at(smem + (size_t)wib * sn_table_bytes(B, P.nsub), B, P.nsub);
+    const double xs = S.x[s], ys = S.y[s], zs = S.z[s];
+    const int ih = host_cell(xs, P.x0[0], P.inv_dx), jh = host_cell(ys, P.x0[1], P.inv_dx), kh = host_cell(zs, P.x0[2], P.inv_dx);
+    if (ih < 0 || ih >= P.nx || jh < 0 || jh >= P.ny || kh < 0 || kh >= P.nz) {
+        if (lane == 0) atomicOr(err, 1);
+        return;
+    }
+    sn_fill_tables(P, T, lane, xs, ys, zs, ih, jh, kh);
+    const double vsx = S.vx[s], vsy = S.vy[s], vsz = S.vz[s], e_sn = S.e_sn[s], m_ej = S.m_ej[s];
+    double m_gas = 0.0, px = 0.0, py = 0.0, pz = 0.0, v_snr = 0.0;
+    for (int c = lane; c < nc; c += 32) {
+        const int a = c % B, t = c / B, b = t % B, cc = t / B;
+        const int cnt = sn_omega_count(P, T, a, b, cc);
+        T.cnt[c] = (unsigned short)cnt;
+        if (cnt > 0) {
+            const double omega = (double)cnt / P.nsub3;
+            const long long q = owned_index(P, ih - g + a, jh - g + b, kh - g + cc);
+            const double rho = U.rho[q];
+            const double vx = U.mx[q] / rho, vy = U.my[q] / rho, vz = U.mz[q] / rho;
+            const double mcell = omega * rho * P.V;
+            m_gas += mcell;
+            px += mcell * vx;
+            py += mcell * vy;
+            pz += mcell * vz;
+            v_snr += omega * P.V;
+        }
+    }
+    m_gas = warp_sum(m_gas); px = warp_sum(px); py = warp_sum(py); pz = warp_sum(pz); v_snr = warp_sum(v_snr);
+    const SnScalars sc = sn_scalars(P, m_gas, px, py, pz, v_snr, vsx, vsy, vsz, e_sn, m_ej);
+    __syncwarp();
+    for (int c = lane; c < nc; c += 32) {
+        const int cnt = T.cnt[c];
+        if (cnt == 0) continue;
+        const int a = c % B, t = c / B, b = t % B, cc = t / B;
+        const int i = ih - g + a, j = jh - g + b, k = kh - g + cc;
+        const long long q = owned_index(P, i, j, k);
+        const double rho = U.rho[q];
+        double d[5];
+        sn_cell_deposit(P, sc, xs, ys, zs, e_sn, m_ej, i, j, k, cnt, rho, U.mx[q] / rho, U.my[q] / rho, U.mz[q] / rho, d);
+        double *dst = buf + P.Nb + ghost_index(P, i, j, k);
+#pragma unroll
+        for (int f = 0; f < 5; ++f) atomicAdd(dst + (long long)f * P.Nb, d[f]);
+    }
+    if (dbg && lane == 0) {
+        const long long n = S.n;
+        dbg[s] = sc.m_snr; dbg[n + s] = sc.v_snr; dbg[2 * n + s] = sc.vcx; dbg[3 * n + s] = sc.vcy; dbg[4 * n + s] = sc.vcz;
+        dbg[5 * n + s] = sc.n_h; dbg[6 * n + s] = sc.r_m; dbg[7 * n + s] = sc.p_rad; dbg[8 * n + s] = (double)sc.regime;
+    }
+}
+
+// test-only: stencil of one particle through the same device functions
+__global__ void k_debug_stencil(const DevP P, int kind, double xs, double ys, double zs, int *__restrict__ counts,
+                                int *__restrict__ host_ijk) {
+    extern __shared__ __align__(16) unsigned char smem[];
+    const int lane = threadIdx.x & 31;
+    const int ih = host_cell(xs, P.x0[0], P.inv_dx), jh = host_cell(ys, P.x0[1], P.inv_dx), kh = host_cell(zs, P.x0[2], P.inv_dx);
+    if (lane == 0) { host_ijk[0] = ih; host_ijk[1] = jh; host_ijk[2] = kh; }
+    if (kind == 0) {
+        const int g = P.gs, B = 2 * g + 1, nc = B * B * B;
+        for (int c = lane; c < nc; c += 32) {
+            const int a = c % B, t = c / B, b = t % B, cc = t / B;
+            const double r2 = dist2(cell_centre(P.x0[0], ih - g + a, P.dx) - xs, cell_centre(P.x0[1], jh - g + b, P.dx) - ys,
+                                    cell_centre(P.x0[2], kh - g + cc, P.dx) - zs);
+            counts[c] = (r2 <= P.rk2_sink) ? 1 : 0;
+        }
+    } else {
+        const int g = P.gn, B = 2 * g + 1, nc = B * B * B;
+        const SnTables T = sn_tables_at(smem, B, P.nsub);
+        sn_fill_tables(P, T, lane, xs, ys, zs, ih, jh, kh);
+        for (int c = lane; c < nc; c += 32) {
+            const int a = c % B, t = c / B, b = t % B, cc = t / B;
+            counts[c] = sn_omega_count(P, T, a, b, cc);
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// a6: ghost fold (gather form).  One thread per owned cell that lies within g of a face; it adds, in the fixed
+// order (z image, y image, x image), the ghost copies of itself to the owned value, for all six channels.
+// ---------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_fold_ghosts(const DevP P, double *__restrict__ buf, long long n_edge,
+                                                     long long n_zslab, long long n_yslab) {
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= n_edge) return;
+    const int g = P.g, nx = P.nx, ny = P.ny, nz = P.nz;
+    int i, j, k;
+    if (t < n_zslab) {                       // k in [0,g) U [nz-g,nz): full planes
+        const long long plane = (long long)nx * ny;
+        int kk = (int)(t / plane);
+        long long r = t - (long long)kk * plane;
+        j = (int)(r / nx); i = (int)(r - (long long)j * nx);
+        k = kk < g ? kk : nz - 2 * g + kk;
+    } else if (t < n_zslab + n_yslab) {      // interior k, j in [0,g) U [ny-g,ny)
+        long long r = t - n_zslab;
+        const long long slab = (long long)nx * 2 * g;
+        int kk = (int)(r / slab);
+        r -= (long long)kk * slab;
+        int jj = (int)(r / nx); i = (int)(r - (long long)jj * nx);
+        k = g + kk;
+        j = jj < g ? jj : ny - 2 * g + jj;
+    } else {                                 // interior k and j, i in [0,g) U [nx-g,nx)
+        long long r = t - n_zslab - n_yslab;
+        const int w = 2 * g;
+        const long long slab = (long long)(ny - 2 * g) * w;
+        int kk = (int)(r / slab);
+        r -= (long long)kk * slab;
+        int jj = (int)(r / w); int ii = (int)(r - (long long)jj * w);
+        k = g + kk; j = g + jj;
+        i = ii < g ? ii : nx - 2 * g + ii;
+    }
+    // image offsets per axis: 0 plus (+n if within g of the low face) or (-n if within g of the high face)
+    const int ox = i < g ? nx : (i >= nx - g ? -nx : 0);
+    const int oy = j < g ? ny : (j >= ny - g ? -ny : 0);
+    const int oz = k < g ? nz : (k >= nz - g ? -nz : 0);
+    const long long base = ghost_index(P, i, j, k);
+#pragma unroll
+    for (int ch = 0; ch < kBufChannels; ++ch) {
+        double *b = buf + (long long)ch * P.Nb;
+        double acc = b[base];
+        for (int cz = 0; cz < 2; ++cz) {
+            if (cz && !oz) break;
+            for (int cy = 0; cy < 2; ++cy) {
+                if (cy && !oy) break;
+                for (int cx = 0; cx < 2; ++cx) {
+                    if (cx && !ox) break;
+                    if (!(cz | cy | cx)) continue;
+                    acc += b[ghost_index(P, i + cx * ox, j + cy * oy, k + cz * oz)];
+                }
+            }
+        }
+        b[base] = acc;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// a7: fused limiter + apply.  Each thread owns VEC consecutive cells of one x-row.
+// ---------------------------------------------------------------------------------------------------------------
+template <int VEC> struct Vec;
+template <> struct Vec<1> { typedef double type; };
+template <> struct Vec<2> { typedef double2 type; };
+
+template <int VEC>
+__device__ __forceinline__ void ldv(const double *p, double v[VEC]) {
+    if constexpr (VEC == 2) { const double2 t = *reinterpret_cast<const double2 *>(p); v[0] = t.x; v[1] = t.y; }
+    else v[0] = *p;
+}
+template <int VEC>
+__device__ __forceinline__ void stv(double *p, const double v[VEC]) {
+    if constexpr (VEC == 2) *reinterpret_cast<double2 *>(p) = make_double2(v[0], v[1]);
+    else *p = v[0];
+}
+
+template <int VEC, bool LAM>
+__global__ void __launch_bounds__(256) k_apply_limited(const DevP P, const DevState U, const double *__restrict__ buf,
+                                                       double *__restrict__ ret, double *__restrict__ lam_out,
+                                                       unsigned int n_items, unsigned int items_per_row) {
+    const unsigned int item = blockIdx.x * blockDim.x + threadIdx.x;
+    if (item >= n_items) return;
+    const unsigned int row = item / items_per_row;
+    const unsigned int i0 = (item - row * items_per_row) * VEC;
+    const unsigned int k = row / (unsigned int)P.ny, j = row - k * (unsigned int)P.ny;
+    const long long q = (long long)row * P.nx + i0;
+    const long long gq = (long long)(k + P.g) * P.pk + (long long)(j + P.g) * P.pj + (i0 + P.gx);
+    double b[kBufChannels][VEC];
+#pragma unroll
+    for (int ch = 0; ch < kBufChannels; ++ch) ldv<VEC>(buf + (long long)ch * P.Nb + gq, b[ch]);
+    bool any = false;
+#pragma unroll
+    for (int ch = 0; ch < kBufChannels; ++ch)
+#pragma unroll
+        for (int v = 0; v < VEC; ++v) any |= (b[ch][v] != 0.0);
+    if (!any) {
+        if (LAM) { double one[VEC]; for (int v = 0; v < VEC; ++v) one[v] = 1.0; stv<VEC>(lam_out + q, one); }
+        return;                                 // dU^sum = 0: U unchanged, nothing to write
+    }
+    double *fld[6] = { U.rho, U.mx, U.my, U.mz, U.etot, U.eint };
+    double u[6][VEC];
+#pragma unroll
+    for (int f = 0; f < 6; ++f) ldv<VEC>(fld[f] + q, u[f]);
+    double lam[VEC];
+#pragma unroll
+    for (int v = 0; v < VEC; ++v) {
+        double uc[6], bc[6], vold[3] = { 0.0, 0.0, 0.0 };
+#pragma unroll
+        for (int f = 0; f < 6; ++f) { uc[f] = u[f][v]; bc[f] = b[f][v]; }
+        const double eta = apply_cell(P, uc, bc, &lam[v], vold);
+#pragma unroll
+        for (int f = 0; f < 6; ++f) u[f][v] = uc[f];
+        if (bc[0] != 0.0 && ret) {              // Step 4 needs eta and the pre-step velocity where a sink removed mass
+            ret[q + v] = eta;
+            ret[P.N + q + v] = vold[0];
+            ret[2 * P.N + q + v] = vold[1];
+            ret[3 * P.N + q + v] = vold[2];
+        }
+    }
+#pragma unroll
+    for (int f = 0; f < 6; ++f) stv<VEC>(fld[f] + q, u[f]);
+    if (LAM) stv<VEC>(lam_out + q, lam);
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// a8: return to particles (Eq. 5).  One warp per sink; shuffle reduction; no atomics.
+// ---------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(128) k_return_sinks(const DevP P, const DevSinks S, const double dt,
+                                                      const double *__restrict__ scal, const double *__restrict__ ret) {
+    const long long s = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int lane = threadIdx.x & 31;
+    if (s >= S.n) return;
+    const double xs = S.x[s], ys = S.y[s], zs = S.z[s];
+    const int ih = host_cell(xs, P.x0[0], P.inv_dx), jh = host_cell(ys, P.x0[1], P.inv_dx), kh = host_cell(zs, P.x0[2], P.inv_dx);
+    if (ih < 0 || ih >= P.nx || jh < 0 || jh >= P.ny || kh < 0 || kh >= P.nz) return;   // flagged at deposit
+    const double mdot = scal[s], r_acc = scal[S.n + s], wsum = scal[2 * S.n + s];
+    const int g = P.gs, B = 2 * g + 1, nc = B * B * B;
+    double dm = 0.0, dpx = 0.0, dpy = 0.0, dpz = 0.0;
+    for (int c = lane; c < nc; c += 32) {
+        const int a = c % B, t = c / B, b = t % B, cc = t / B;
+        const int i = ih - g + a, j = jh - g + b, k = kh - g + cc;
+        const double r2 = dist2(cell_centre(P.x0[0], i, P.dx) - xs, cell_centre(P.x0[1], j, P.dx) - ys,
+                                cell_centre(P.x0[2], k, P.dx) - zs);
+        if (r2 <= P.rk2_sink) {
+            const double amt = sink_cell_amount(P, r2, r_acc, wsum, mdot, dt);
+            if (amt > 0.0) {                     // amt == 0 deposits nothing, so the return mesh has no entry there
+                const long long q = owned_index(P, i, j, k);
+                const double gain = ret[q] * amt * P.V;
+                dm += gain;
+                dpx += gain * ret[P.N + q];
+                dpy += gain * ret[2 * P.N + q];
+                dpz += gain * ret[3 * P.N + q];
+            }
+        }
+    }
+    dm = warp_sum(dm); dpx = warp_sum(dpx); dpy = warp_sum(dpy); dpz = warp_sum(dpz);
+    if (lane == 0) {
+        const double m_old = S.m[s], m_new = m_old + dm;
+        S.vx[s] = (m_old * S.vx[s] + dpx) / m_new;
+        S.vy[s] = (m_old * S.vy[s] + dpy) / m_new;
+        S.vz[s] = (m_old * S.vz[s] + dpz) / m_new;
+        S.m[s] = m_new;
+        if (S.dm) S.dm[s] = dm;
+        if (S.dpx) S.dpx[s] = dpx;
+        if (S.dpy) S.dpy[s] = dpy;
+        if (S.dpz) S.dpz[s] = dpz;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// host side
+// ---------------------------------------------------------------------------------------------------------------
+static int ceil_div_pos(double a, double b) { return (int)std::ceil(a / b); }
+
+static bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+static int grow(pm_ctx *c, double **p, long long *cap, long long need) {
+    if (need <= *cap) return PM_OK;
+    if (*p) { PM_CUDA(c, cudaFree(*p)); *p = nullptr; *cap = 0; }
+    long long n = need + need / 4 + 64;
+    cudaError_t e = cudaMalloc(p, (size_t)n * sizeof(double));
+    if (e != cudaSuccess) { *p = nullptr; PM_FAIL(c, PM_ENOMEM, "cudaMalloc of %lld doubles failed: %s", n, cudaGetErrorString(e)); }
+    *cap = n;
+    return PM_OK;
+}
+
+extern "C" int pm_create(const pm_params *prm, int device, void *cuda_stream, pm_ctx **out) {
+    if (!prm || !out) return PM_EINVAL;
+    *out = nullptr;
+    if (prm->nx < 1 || prm->ny < 1 || prm->nz < 1 || !(prm->dx > 0.0)) return PM_EINVAL;
+    if (prm->rk_sink < 0.0 || prm->rk_sn < 0.0) return PM_EINVAL;
+    if (prm->rk_sn > 0.0 && (prm->sn_nsub < 1 || prm->sn_nsub > 8)) return PM_EINVAL;
+    if (prm->sn_regime < 0 || prm->sn_regime > 3) return PM_EINVAL;
+    if (!(prm->f_max_remove >= 0.0 && prm->f_max_remove <= 1.0) || prm->rho_floor < 0.0) return PM_EINVAL;
+    const int gs = prm->rk_sink > 0.0 ? ceil_div_pos(prm->rk_sink, prm->dx) : 0;
+    const int gn = prm->rk_sn > 0.0 ? ceil_div_pos(prm->rk_sn, prm->dx) : 0;
+    const int g = gs > gn ? gs : gn;
+    if (g < 1 || g > 8) return PM_EINVAL;
+    if (prm->nx < 2 * g + 1 || prm->ny < 2 * g + 1 || prm->nz < 2 * g + 1) return PM_EINVAL;     // R32
+    const long long N = (long long)prm->nx * prm->ny * prm->nz;
+    if (N >= (1ll << 31)) return PM_EINVAL;
+
+    pm_ctx *c = new (std::nothrow) pm_ctx();
+    if (!c) return PM_ENOMEM;
+    std::memset(c, 0, sizeof(*c));
+    c->prm = *prm;
+    c->device = device;
+    c->stream = (cudaStream_t)cuda_stream;
+    DevP &P = c->P;
+    P.nx = prm->nx; P.ny = prm->ny; P.nz = prm->nz;
+    P.g = g; P.gs = gs; P.gn = gn; P.nsub = prm->sn_nsub > 0 ? prm->sn_nsub : 1; P.regime = prm->sn_regime;
+    P.gx = (g + 1) & ~1;
+    P.pj = prm->nx + 2 * P.gx; P.pk = P.pj * (prm->ny + 2 * g);
+    P.N = N; P.Nb = P.pk * (prm->nz + 2 * g);
+    P.dx = prm->dx; P.inv_dx = 1.0 / prm->dx; P.V = prm->dx * prm->dx * prm->dx;
+    for (int a = 0; a < 3; ++a) P.x0[a] = prm->x0[a];
+    P.G = prm->G; P.gamma = prm->gamma; P.cs_iso = prm->cs_iso;
+    P.rk_sink = prm->rk_sink; P.rk2_sink = prm->rk_sink * prm->rk_sink;
+    P.rk_sn = prm->rk_sn; P.rk2_sn = prm->rk_sn * prm->rk_sn;
+    P.lambda = prm->bondi_lambda; P.fmax = prm->f_max_remove; P.rho_floor = prm->rho_floor;
+    P.eps_k = prm->sn_eps_k; P.rm_ej = prm->sn_rm_ej; P.rm_mc = prm->sn_rm_mc;
+    P.msf_c = prm->sn_msf_coeff; P.msf_e = prm->sn_msf_exp; P.psnr_c = prm->sn_psnr_coeff; P.psnr_e = prm->sn_psnr_exp;
+    P.mu_h = prm->sn_mu_h; P.nh_unit = prm->sn_nh_unit; P.theta = prm->sn_eint_theta;
+    P.nsub3 = (double)P.nsub * (double)P.nsub * (double)P.nsub;
+
+    cudaError_t e = cudaSetDevice(device);
+    if (e == cudaSuccess) e = cudaMalloc(&c->buf, (size_t)kBufChannels * P.Nb * sizeof(double));
+    if (e == cudaSuccess && gs > 0) e = cudaMalloc(&c->ret, (size_t)kRetWords * N * sizeof(double));
+    if (e == cudaSuccess && (prm->flags & PM_FLAG_DEBUG_LAMBDA)) e = cudaMalloc(&c->lam, (size_t)N * sizeof(double));
+    if (e == cudaSuccess) e = cudaMalloc(&c->err_flag, sizeof(int));
+    if (e == cudaSuccess) e = cudaMallocHost(&c->err_host, sizeof(int));
+    if (e == cudaSuccess) e = cudaMemsetAsync(c->err_flag, 0, sizeof(int), c->stream);
+    if (e == cudaSuccess && c->ret) e = cudaMemsetAsync(c->ret, 0, (size_t)kRetWords * N * sizeof(double), c->stream);
+    if (e == cudaSuccess) {
+        // opt in to the dynamic shared memory the SN kernel may need (<= 8 warps x tables)
+        const size_t smem = kSnWarps * sn_table_bytes(2 * (gn > 0 ? gn : 1) + 1, P.nsub);
+        if (smem > 48 * 1024) e = cudaFuncSetAttribute(k_deposit_sne, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    }
+    if (e != cudaSuccess) {
+        int rc = (e == cudaErrorMemoryAllocation) ? PM_ENOMEM : PM_ECUDA;
+        cudaGetLastError();
+        if (c->buf) cudaFree(c->buf);
+        if (c->ret) cudaFree(c->ret);
+        if (c->lam) cudaFree(c->lam);
+        if (c->err_flag) cudaFree(c->err_flag);
+        if (c->err_host) cudaFreeHost(c->err_host);
+        delete c;
+        return rc;
+    }
+    c->stage = ST_IDLE;
+    *out = c;
+    return PM_OK;
+}
+
+extern "C" int pm_destroy(pm_ctx *c) {
+    if (!c) return PM_EINVAL;
+    cudaSetDevice(c->device);
+    cudaStreamSynchronize(c->stream);
+    double *ptrs[] = { c->buf, c->ret, c->lam, c->sink_scal, c->dbg_sink, c->dbg_sn, c->stg_state, c->stg_sinks, c->stg_sne };
+    for (double *p : ptrs) if (p) cudaFree(p);
+    if (c->err_flag) cudaFree(c->err_flag);
+    if (c->err_host) cudaFreeHost(c->err_host);
+    delete c;
+    return PM_OK;
+}
+
+extern "C" const char *pm_last_error(const pm_ctx *c) { return c ? c->msg : "null ctx"; }
+extern "C" int64_t pm_launch_count(const pm_ctx *c) { return c ? c->launches : 0; }
+
+static bool state_ok(const pm_state *s) { return s && s->rho && s->mx && s->my && s->mz && s->etot && s->eint; }
+
+extern "C" int pm_deposit(pm_ctx *c, const pm_state *st, const pm_sinks *sk, const pm_sne *sn, double dt) {
+    if (!c) return PM_EINVAL;
+    if (!state_ok(st)) PM_FAIL(c, PM_EINVAL, "pm_deposit: null state pointer");
+    const long long nk = sk ? sk->n : 0, nn = sn ? sn->n : 0;
+    if (nk < 0 || nn < 0) PM_FAIL(c, PM_EINVAL, "pm_deposit: negative particle count");
+    if (nk > 0 && c->P.gs == 0) PM_FAIL(c, PM_EINVAL, "pm_deposit: sinks given but rk_sink == 0");
+    if (nn > 0 && c->P.gn == 0) PM_FAIL(c, PM_EINVAL, "pm_deposit: SNe given but rk_sn == 0");
+    if (nk > 0 && !(sk->x && sk->y && sk->z && sk->vx && sk->vy && sk->vz && sk->m)) PM_FAIL(c, PM_EINVAL, "pm_deposit: null sink array");
+    if (nn > 0 && !(sn->x && sn->y && sn->z && sn->vx && sn->vy && sn->vz && sn->e_sn && sn->m_ej)) PM_FAIL(c, PM_EINVAL, "pm_deposit: null SN array");
+    PM_CUDA(c, cudaSetDevice(c->device));
+    const DevP &P = c->P;
+    const bool dbg = (c->prm.flags & PM_FLAG_DEBUG_SCALARS) != 0;
+    int rc;
+    if ((rc = grow(c, &c->sink_scal, &c->cap_sinks, 3 * nk)) != PM_OK) return rc;
+    if (dbg && (rc = grow(c, &c->dbg_sink, &c->cap_dbg_sink, 8 * nk)) != PM_OK) return rc;
+    if (dbg && (rc = grow(c, &c->dbg_sn, &c->cap_dbg_sn, 9 * nn)) != PM_OK) return rc;
+
+    {   // a0: reset (L59 "all cells initialized to zero")
+        const long long n2 = (long long)kBufChannels * P.Nb / 2;
+        k_zero_buffer<<<148 * 8, 256, 0, c->stream>>>(reinterpret_cast<double2 *>(c->buf), n2);
+        if ((rc = check_launch(c, "k_zero_buffer")) != PM_OK) return rc;
+    }
+    const DevState U = { st->rho, st->mx, st->my, st->mz, st->etot, st->eint };
+    if (nk > 0) {
+        const DevSinks S = { nk, sk->x, sk->y, sk->z, sk->vx, sk->vy, sk->vz, sk->m, sk->dm, sk->dpx, sk->dpy, sk->dpz };
+        const unsigned blocks = (unsigned)((nk + 3) / 4);
+        k_deposit_sinks<<<blocks, 128, 0, c->stream>>>(P, U, S, dt, c->buf, c->sink_scal, dbg ? c->dbg_sink : nullptr, c->err_flag);
+        if ((rc = check_launch(c, "k_deposit_sinks")) != PM_OK) return rc;
+    }
+    if (nn > 0) {
+        const DevSNe S = { nn, sn->x, sn->y, sn->z, sn->vx, sn->vy, sn->vz, sn->e_sn, sn->m_ej };
+        const unsigned blocks = (unsigned)((nn + kSnWarps - 1) / kSnWarps);
+        const size_t smem = kSnWarps * sn_table_bytes(2 * P.gn + 1, P.nsub);
+        k_deposit_sne<<<blocks, kSnWarps * 32, smem, c->stream>>>(P, U, S, c->buf, dbg ? c->dbg_sn : nullptr, c->err_flag);
+        if ((rc = check_launch(c, "k_deposit_sne")) != PM_OK) return rc;
+    }
+    c->n_sinks_dep = nk; c->n_sne_dep = nn; c->dt = dt;
+    c->stage = ST_DEPOSITED;
+    return PM_OK;
+}
+
+extern "C" int pm_fold_ghosts(pm_ctx *c) {
+    if (!c) return PM_EINVAL;
+    if (c->stage != ST_DEPOSITED) PM_FAIL(c, PM_EORDER, "pm_fold_ghosts must follow pm_deposit");
+    PM_CUDA(c, cudaSetDevice(c->device));
+    const DevP &P = c->P;
+    const long long g2 = 2 * P.g;
+    const long long n_z = g2 * P.ny * P.nx;
+    const long long n_y = (long long)(P.nz - g2) * g2 * P.nx;
+    const long long n_x = (long long)(P.nz - g2) * (P.ny - g2) * g2;
+    const long long n_edge = n_z + n_y + n_x;
+    const unsigned blocks = (unsigned)((n_edge + 255) / 256);
+    k_fold_ghosts<<<blocks, 256, 0, c->stream>>>(P, c->buf, n_edge, n_z, n_y);
+    int rc = check_launch(c, "k_fold_ghosts");
+    if (rc != PM_OK) return rc;
+    c->stage = ST_FOLDED;
+    return PM_OK;
+}
+
+template <int VEC>
+static void launch_apply(pm_ctx *c, const DevState &U) {
+    const DevP &P = c->P;
+    const unsigned ipr = (unsigned)(P.nx / VEC);
+    const unsigned n_items = (unsigned)(P.N / VEC);
+    const unsigned blocks = (n_items + 255) / 256;
+    if (c->lam) k_apply_limited<VEC, true><<<blocks, 256, 0, c->stream>>>(P, U, c->buf, c->ret, c->lam, n_items, ipr);
+    else k_apply_limited<VEC, false><<<blocks, 256, 0, c->stream>>>(P, U, c->buf, c->ret, nullptr, n_items, ipr);
+}
+
+extern "C" int pm_apply_limited(pm_ctx *c, pm_state *st) {
+    if (!c) return PM_EINVAL;
+    if (c->stage != ST_FOLDED) PM_FAIL(c, PM_EORDER, "pm_apply_limited must follow pm_fold_ghosts");
+    if (!state_ok(st)) PM_FAIL(c, PM_EINVAL, "pm_apply_limited: null state pointer");
+    PM_CUDA(c, cudaSetDevice(c->device));
+    const DevState U = { st->rho, st->mx, st->my, st->mz, st->etot, st->eint };
+    const bool vec2 = (c->P.nx % 2 == 0) && aligned16(st->rho) && aligned16(st->mx) && aligned16(st->my) &&
+                      aligned16(st->mz) && aligned16(st->etot) && aligned16(st->eint);
+    if (vec2) launch_apply<2>(c, U); else launch_apply<1>(c, U);
+    int rc = check_launch(c, "k_apply_limited");
+    if (rc != PM_OK) return rc;
+    c->stage = ST_APPLIED;
+    return PM_OK;
+}
+
+extern "C" int pm_return_to_particles(pm_ctx *c, pm_sinks *sk) {
+    if (!c) return PM_EINVAL;
+    if (c->stage != ST_APPLIED) PM_FAIL(c, PM_EORDER, "pm_return_to_particles must follow pm_apply_limited");
+    const long long nk = sk ? sk->n : 0;
+    if (nk != c->n_sinks_dep) PM_FAIL(c, PM_EINVAL, "pm_return_to_particles: %lld sinks, but %lld were deposited", nk, c->n_sinks_dep);
+    PM_CUDA(c, cudaSetDevice(c->device));
+    if (nk > 0) {
+        if (!(sk->x && sk->y && sk->z && sk->vx && sk->vy && sk->vz && sk->m)) PM_FAIL(c, PM_EINVAL, "pm_return_to_particles: null sink array");
+        const DevSinks S = { nk, sk->x, sk->y, sk->z, sk->vx, sk->vy, sk->vz, sk->m, sk->dm, sk->dpx, sk->dpy, sk->dpz };
+        const unsigned blocks = (unsigned)((nk + 3) / 4);
+        k_return_sinks<<<blocks, 128, 0, c->stream>>>(c->P, S, c->dt, c->sink_scal, c->ret);
+        int rc = check_launch(c, "k_return_sinks");
+        if (rc != PM_OK) return rc;
+    }
+    c->stage = ST_IDLE;
+    return PM_OK;
+}
+
+extern "C" int pm_check(pm_ctx *c) {
+    if (!c) return PM_EINVAL;
+    PM_CUDA(c, cudaSetDevice(c->device));
+    PM_CUDA(c, cudaMemcpyAsync(c->err_host, c->err_flag, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+    PM_CUDA(c, cudaStreamSynchronize(c->stream));
+    if (*c->err_host & 1) {
+        PM_CUDA(c, cudaMemsetAsync(c->err_flag, 0, sizeof(int), c->stream));
+        PM_FAIL(c, PM_EDOMAIN, "a particle lies outside the domain [x0, x0 + n dx)");
+    }
+    return PM_OK;
+}
+
+extern "C" int pm_step_host(pm_ctx *c, pm_state *hs, pm_sinks *hk, const pm_sne *hn, double dt) {
+    if (!c) return PM_EINVAL;
+    if (!state_ok(hs)) PM_FAIL(c, PM_EINVAL, "pm_step_host: null state pointer");
+    PM_CUDA(c, cudaSetDevice(c->device));
+    const long long N = c->P.N, nk = hk ? hk->n : 0, nn = hn ? hn->n : 0;
+    int rc;
+    if ((rc = grow(c, &c->stg_state, &c->stg_state_cap, 6 * N)) != PM_OK) return rc;
+    if ((rc = grow(c, &c->stg_sinks, &c->stg_sinks_cap, 11 * nk)) != PM_OK) return rc;
+    if ((rc = grow(c, &c->stg_sne, &c->stg_sne_cap, 8 * nn)) != PM_OK) return rc;
+    cudaStream_t s = c->stream;
+    double *hst[6] = { hs->rho, hs->mx, hs->my, hs->mz, hs->etot, hs->eint };
+    for (int f = 0; f < 6; ++f) PM_CUDA(c, cudaMemcpyAsync(c->stg_state + f * N, hst[f], N * 8, cudaMemcpyHostToDevice, s));
+    pm_state ds = { c->stg_state, c->stg_state + N, c->stg_state + 2 * N, c->stg_state + 3 * N, c->stg_state + 4 * N, c->stg_state + 5 * N };
+    pm_sinks dk; std::memset(&dk, 0, sizeof(dk));
+    pm_sne dn; std::memset(&dn, 0, sizeof(dn));
+    if (nk > 0) {
+        const double *src[7] = { hk->x, hk->y, hk->z, hk->vx, hk->vy, hk->vz, hk->m };
+        for (int f = 0; f < 7; ++f) {
+            if (!src[f]) PM_FAIL(c, PM_EINVAL, "pm_step_host: null sink array");
+            PM_CUDA(c, cudaMemcpyAsync(c->stg_sinks + f * nk, src[f], nk * 8, cudaMemcpyHostToDevice, s));
+        }
+        double *b = c->stg_sinks;
+        dk.n = nk; dk.x = b; dk.y = b + nk; dk.z = b + 2 * nk; dk.vx = b + 3 * nk; dk.vy = b + 4 * nk; dk.vz = b + 5 * nk; dk.m = b + 6 * nk;
+        dk.dm = b + 7 * nk; dk.dpx = b + 8 * nk; dk.dpy = b + 9 * nk; dk.dpz = b + 10 * nk;
+    }
+    if (nn > 0) {
+        const double *src[8] = { hn->x, hn->y, hn->z, hn->vx, hn->vy, hn->vz, hn->e_sn, hn->m_ej };
+        for (int f = 0; f < 8; ++f) {
+            if (!src[f]) PM_FAIL(c, PM_EINVAL, "pm_step_host: null SN array");
+            PM_CUDA(c, cudaMemcpyAsync(c->stg_sne + f * nn, src[f], nn * 8, cudaMemcpyHostToDevice, s));
+        }
+        double *b = c->stg_sne;
+        dn.n = nn; dn.x = b; dn.y = b + nn; dn.z = b + 2 * nn; dn.vx = b + 3 * nn; dn.vy = b + 4 * nn; dn.vz = b + 5 * nn;
+        dn.e_sn = b + 6 * nn; dn.m_ej = b + 7 * nn;
+    }
+    if ((rc = pm_deposit(c, &ds, nk > 0 ? &dk : nullptr, nn > 0 ? &dn : nullptr, dt)) != PM_OK) return rc;
+    if ((rc = pm_fold_ghosts(c)) != PM_OK) return rc;
+    if ((rc = pm_apply_limited(c, &ds)) != PM_OK) return rc;
+    if ((rc = pm_return_to_particles(c, nk > 0 ? &dk : nullptr)) != PM_OK) return rc;
+    for (int f = 0; f < 6; ++f) PM_CUDA(c, cudaMemcpyAsync(hst[f], c->stg_state + f * N, N * 8, cudaMemcpyDeviceToHost, s));
+    if (nk > 0) {
+        double *dst[8] = { hk->vx, hk->vy, hk->vz, hk->m, hk->dm, hk->dpx, hk->dpy, hk->dpz };
+        for (int f = 0; f < 8; ++f)
+            if (dst[f]) PM_CUDA(c, cudaMemcpyAsync(dst[f], c->stg_sinks + (3 + f) * nk, nk * 8, cudaMemcpyDeviceToHost, s));
+    }
+    return pm_check(c);
+}
+
+// ---- test-only views ---------------------------------------------------------------------------------------------
+extern "C" int pm_debug_buffer(pm_ctx *c, int channel, const double **dev_ptr, int64_t dims[3], int64_t *origin, int32_t *ghost) {
+    if (!c || !dev_ptr || channel < 0 || channel >= kBufChannels) return PM_EINVAL;
+    *dev_ptr = c->buf + (long long)channel * c->P.Nb;
+    if (dims) { dims[0] = c->P.nz + 2 * c->P.g; dims[1] = c->P.ny + 2 * c->P.g; dims[2] = c->P.pj; }
+    if (origin) *origin = (long long)c->P.g * c->P.pk + (long long)c->P.g * c->P.pj + c->P.gx;
+    if (ghost) *ghost = c->P.g;
+    return PM_OK;
+}
+
+extern "C" int pm_debug_return_mesh(pm_ctx *c, int word, const double **dev_ptr) {
+    if (!c || !dev_ptr || word < 0 || word >= kRetWords || !c->ret) return PM_EINVAL;
+    *dev_ptr = c->ret + (long long)word * c->P.N;
+    return PM_OK;
+}
+
+extern "C" int pm_debug_lambda(pm_ctx *c, const double **dev_ptr) {
+    if (!c || !dev_ptr || !c->lam) return PM_EINVAL;
+    *dev_ptr = c->lam;
+    return PM_OK;
+}
+
+extern "C" int pm_debug_sink_scalars(pm_ctx *c, const double **dev_ptr, int64_t *n) {
+    if (!c || !dev_ptr || !n || !(c->prm.flags & PM_FLAG_DEBUG_SCALARS)) return PM_EINVAL;
+    *dev_ptr = c->dbg_sink; *n = c->n_sinks_dep;
+    return PM_OK;
+}
+
+extern "C" int pm_debug_sn_scalars(pm_ctx *c, const double **dev_ptr, int64_t *n) {
+    if (!c || !dev_ptr || !n || !(c->prm.flags & PM_FLAG_DEBUG_SCALARS)) return PM_EINVAL;
+    *dev_ptr = c->dbg_sn; *n = c->n_sne_dep;
+    return PM_OK;
+}
+
+extern "C" int pm_debug_stencil(pm_ctx *c, int kind, double x, double y, double z, int32_t *dev_counts, int32_t *host_ijk, int32_t *side) {
+    if (!c || !dev_counts || !host_ijk || !side || kind < 0 || kind > 1) return PM_EINVAL;
+    const int g = kind == 0 ? c->P.gs : c->P.gn;
+    if (g == 0) PM_FAIL(c, PM_EINVAL, "pm_debug_stencil: that particle kind is unused");
+    PM_CUDA(c, cudaSetDevice(c->device));
+    int *d_ijk = nullptr;
+    PM_CUDA(c, cudaMalloc(&d_ijk, 3 * sizeof(int)));
+    const size_t smem = kind == 1 ? sn_table_bytes(2 * g + 1, c->P.nsub) : 0;
+    k_debug_stencil<<<1, 32, smem, c->stream>>>(c->P, kind, x, y, z, dev_counts, d_ijk);
+    int rc = check_launch(c, "k_debug_stencil");
+    if (rc == PM_OK) {
+        cudaError_t e = cudaMemcpyAsync(host_ijk, d_ijk, 3 * sizeof(int), cudaMemcpyDeviceToHost, c->stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+        if (e != cudaSuccess) { snprintf(c->msg, sizeof(c->msg), "pm_debug_stencil: %s", cudaGetErrorString(e)); rc = PM_ECUDA; }
+    }
+    cudaFree(d_ijk);
+    *side = 2 * g + 1;
+    return rc;
+}

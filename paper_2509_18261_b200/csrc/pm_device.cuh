@@ -1,0 +1,280 @@
+// pm_device.cuh -- device-side arithmetic of the particle-mesh-particle step (sm_100a).
+//
+// Everything that decides an integer (host cell, stencil membership, omega sub-sample counts) is written so that
+// no FMA contraction can change it: this translation unit is compiled with -fmad=false, and every expression
+// below keeps the operation order stated in DESIGN.md ("Arithmetic contract").
+// Citations: "L" = /root/reference/PAPER.md line, "R" = DESIGN.md reading.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace pm {
+
+constexpr int kBufChannels = 6;      // 0: accretion d rho (signed, R1/R29); 1..5: SN d rho, d p (3), d E
+constexpr int kRetWords = 4;         // eta, v_old (3)
+constexpr double kFourPi = 12.566370614359172953850573533118;
+
+struct DevP {
+    int nx, ny, nz;
+    int g;            // ghost width of the buffer mesh = max(gs, gn)
+    int gx;           // x offset of the owned origin inside a ghosted row: g rounded up to even (16-byte alignment)
+    int gs, gn;       // kernel half-widths in cells: ceil(r_K / dx) (L59: ghosts must contain r_K)
+    int nsub, regime;
+    long long pj, pk; // ghosted pitches (elements): j-stride = nx + 2gx, k-stride = (nx+2gx)(ny+2g)
+    long long N, Nb;  // owned / ghosted cell counts
+    double dx, inv_dx, V, x0[3];
+    double G, gamma, cs_iso;
+    double rk_sink, rk2_sink, rk_sn, rk2_sn;
+    double lambda, fmax, rho_floor;
+    double eps_k, rm_ej, rm_mc, msf_c, msf_e, psnr_c, psnr_e, mu_h, nh_unit, theta;
+    double nsub3;
+};
+
+struct DevState { double *rho, *mx, *my, *mz, *etot, *eint; };
+struct DevSinks { long long n; const double *x, *y, *z; double *vx, *vy, *vz, *m, *dm, *dpx, *dpy, *dpz; };
+struct DevSNe { long long n; const double *x, *y, *z, *vx, *vy, *vz, *e_sn, *m_ej; };
+
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+__device__ __forceinline__ int warp_sum_int(int v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+// Host cell {ijk}_s (L43): floor((x - x0) * inv_dx)
+__device__ __forceinline__ int host_cell(double x, double x0, double inv_dx) { return (int)floor((x - x0) * inv_dx); }
+
+// Centre of unwrapped cell i, and of sub-sample q of it (R17)
+__device__ __forceinline__ double cell_centre(double x0, int i, double dx) { return x0 + ((double)i + 0.5) * dx; }
+__device__ __forceinline__ double sub_centre(double x0, int i, int q, int nsub, double dx) {
+    return x0 + ((double)i + ((double)q + 0.5) / (double)nsub) * dx;
+}
+// r^2 summed in the order z, y, x
+__device__ __forceinline__ double dist2(double ddx, double ddy, double ddz) { return (ddz * ddz + ddy * ddy) + ddx * ddx; }
+
+// periodic wrap of an index known to lie in [-n, 2n)
+__device__ __forceinline__ int wrap1(int i, int n) { return i < 0 ? i + n : (i >= n ? i - n : i); }
+
+__device__ __forceinline__ long long owned_index(const DevP &P, int i, int j, int k) {
+    return ((long long)wrap1(k, P.nz) * P.ny + wrap1(j, P.ny)) * P.nx + wrap1(i, P.nx);
+}
+// ghosted index of UNWRAPPED cell (i,j,k), each in [-g, n+g)
+__device__ __forceinline__ long long ghost_index(const DevP &P, int i, int j, int k) {
+    return (long long)(k + P.g) * P.pk + (long long)(j + P.g) * P.pj + (i + P.gx);
+}
+
+__device__ __forceinline__ double sound_speed(const DevP &P, double rho, double eint) {
+    if (P.cs_iso > 0.0) return P.cs_iso;
+    return sqrt(P.gamma * (P.gamma - 1.0) * eint / rho);
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// Sink accretion (Sec. 3.1.1)
+// ---------------------------------------------------------------------------------------------------------------
+struct SinkScalars { double rho_inf, v_inf, c_inf, r_bh, mdot, r_acc; };
+
+// Eq. 7, Eq. 8 (second form), Eq. 10 from the kernel sums (R4-R7)
+__device__ __forceinline__ SinkScalars sink_scalars(const DevP &P, double sum_rho, double srx, double sry, double srz,
+                                                    double sum_rc, int cnt, double ms) {
+    SinkScalars s;
+    s.rho_inf = sum_rho / (double)cnt;
+    s.v_inf = sqrt((srx * srx + sry * sry) + srz * srz) / sum_rho;
+    s.c_inf = sum_rc / sum_rho;
+    s.r_bh = P.G * ms / (s.v_inf * s.v_inf + s.c_inf * s.c_inf);
+    s.mdot = kFourPi * s.rho_inf * (s.r_bh * s.r_bh) * sqrt(P.lambda * P.lambda * (s.c_inf * s.c_inf) + s.v_inf * s.v_inf);
+    if (s.r_bh < 0.25 * P.dx) s.r_acc = 0.25 * P.dx;
+    else if (s.r_bh > 0.5 * P.rk_sink) s.r_acc = 0.5 * P.rk_sink;
+    else s.r_acc = s.r_bh;
+    return s;
+}
+
+// Eq. 9, Eq. 11, Eq. 13 mass row (per unit volume), Truelove term off (R10)
+__device__ __forceinline__ double sink_cell_amount(const DevP &P, double r2, double r_acc, double wsum, double mdot, double dt) {
+    double w = exp(-r2 / (r_acc * r_acc));
+    double phi = w / wsum;
+    return mdot * phi * dt / P.V;
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// Supernova stencil weights (R17): per-warp shared tables of squared sub-sample offsets per axis
+// ---------------------------------------------------------------------------------------------------------------
+struct SnTables {
+    double *d2[3];     // [B * nsub] squared offset of each sub-sample centre from the particle, per axis
+    double *dmin[3];   // [B] min over the cell's sub-samples
+    double *dmax[3];   // [B] max over the cell's sub-samples
+    unsigned short *cnt;   // [B^3] omega counts
+};
+
+__host__ __device__ inline size_t sn_table_bytes(int B, int nsub) {
+    size_t doubles = (size_t)3 * B * nsub + (size_t)6 * B;
+    size_t bytes = doubles * 8 + (size_t)B * B * B * 2;
+    return (bytes + 15) & ~(size_t)15;
+}
+
+__device__ __forceinline__ SnTables sn_tables_at(unsigned char *base, int B, int nsub) {
+    SnTables t;
+    double *d = reinterpret_cast<double *>(base);
+    for (int a = 0; a < 3; ++a) { t.d2[a] = d; d += B * nsub; }
+    for (int a = 0; a < 3; ++a) { t.dmin[a] = d; d += B; }
+    for (int a = 0; a < 3; ++a) { t.dmax[a] = d; d += B; }
+    t.cnt = reinterpret_cast<unsigned short *>(d);
+    return t;
+}
+
+// Fill the per-axis tables (whole warp cooperates), then __syncwarp.
+__device__ __forceinline__ void sn_fill_tables(const DevP &P, const SnTables &t, int lane, double xs, double ys, double zs,
+                                               int ih, int jh, int kh) {
+    const int B = 2 * P.gn + 1, ns = P.nsub;
+    const double ps[3] = { xs, ys, zs };
+    const int h[3] = { ih, jh, kh };
+    for (int e = lane; e < 3 * B * ns; e += 32) {
+        int ax = e / (B * ns), r = e - ax * (B * ns);
+        int c = r / ns, q = r - c * ns;
+        double d = sub_centre(P.x0[ax], h[ax] - P.gn + c, q, ns, P.dx) - ps[ax];
+        t.d2[ax][r] = d * d;
+    }
+    __syncwarp();
+    for (int e = lane; e < 3 * B; e += 32) {
+        int ax = e / B, c = e - ax * B;
+        double lo = t.d2[ax][c * ns], hi = lo;
+        for (int q = 1; q < ns; ++q) { double v = t.d2[ax][c * ns + q]; lo = fmin(lo, v); hi = fmax(hi, v); }
+        t.dmin[ax][c] = lo;
+        t.dmax[ax][c] = hi;
+    }
+    __syncwarp();
+}
+
+// omega count of box cell (a,b,c) = (x,y,z offsets in [0,B)).  Exactly the number of sub-samples with
+// (dz^2 + dy^2) + dx^2 <= r_K^2: the two shortcuts are exact because fp addition is monotone in each argument.
+__device__ __forceinline__ int sn_omega_count(const DevP &P, const SnTables &t, int a, int b, int c) {
+    const int ns = P.nsub;
+    const double rk2 = P.rk2_sn;
+    if ((t.dmax[2][c] + t.dmax[1][b]) + t.dmax[0][a] <= rk2) return ns * ns * ns;
+    if ((t.dmin[2][c] + t.dmin[1][b]) + t.dmin[0][a] > rk2) return 0;
+    int cnt = 0;
+    for (int qz = 0; qz < ns; ++qz) {
+        const double z2 = t.d2[2][c * ns + qz];
+        for (int qy = 0; qy < ns; ++qy) {
+            const double s = z2 + t.d2[1][b * ns + qy];
+            for (int qx = 0; qx < ns; ++qx) cnt += ((s + t.d2[0][a * ns + qx]) <= rk2) ? 1 : 0;
+        }
+    }
+    return cnt;
+}
+
+struct SnScalars { double m_snr, v_snr, vcx, vcy, vcz, e_kin, n_h, r_m, p_rad; int regime; };
+
+// Eq. 18, n_H, R_M, Eqs. 19-20 from the stencil sums (R18-R20, R23-R24, R27)
+__device__ __forceinline__ SnScalars sn_scalars(const DevP &P, double m_gas, double px, double py, double pz, double v_snr,
+                                                double vsx, double vsy, double vsz, double e_sn, double m_ej) {
+    SnScalars s;
+    s.m_snr = m_gas + m_ej;
+    s.v_snr = v_snr;
+    s.vcx = (px + m_ej * vsx) / s.m_snr;
+    s.vcy = (py + m_ej * vsy) / s.m_snr;
+    s.vcz = (pz + m_ej * vsz) / s.m_snr;
+    s.e_kin = 0.5 * m_ej * ((vsx * vsx + vsy * vsy) + vsz * vsz);
+    s.n_h = s.m_snr / (P.mu_h * s.v_snr);
+    double m_sf = P.msf_c * pow(s.n_h / P.nh_unit, P.msf_e);
+    s.r_m = s.m_snr / m_sf;
+    int regime = P.regime;
+    if (regime == 0) regime = (s.r_m > P.rm_mc) ? 3 : ((s.r_m > P.rm_ej) ? 2 : 1);
+    s.regime = regime;
+    if (regime == 3) s.p_rad = P.psnr_c * pow(s.n_h / P.nh_unit, P.psnr_e);
+    else if (regime == 2) s.p_rad = sqrt(2.0 * s.m_snr * P.eps_k * e_sn);
+    else s.p_rad = 0.0;
+    return s;
+}
+
+// Eq. 17 for one cell with omega > 0 (R21, R22): out = (d rho, d p, d E)
+__device__ __forceinline__ void sn_cell_deposit(const DevP &P, const SnScalars &s, double xs, double ys, double zs,
+                                                double e_sn, double m_ej, int i, int j, int k, int cnt,
+                                                double rho, double vx, double vy, double vz, double out[5]) {
+    const double omega = (double)cnt / P.nsub3;
+    const double ddx = cell_centre(P.x0[0], i, P.dx) - xs;
+    const double ddy = cell_centre(P.x0[1], j, P.dx) - ys;
+    const double ddz = cell_centre(P.x0[2], k, P.dx) - zs;
+    const double r = sqrt(dist2(ddx, ddy, ddz));
+    double rhx = 0.0, rhy = 0.0, rhz = 0.0;
+    if (r > 0.0) { rhx = ddx / r; rhy = ddy / r; rhz = ddz / r; }
+    const double drho = omega * m_ej / s.v_snr;
+    const double pscale = (s.p_rad / s.v_snr) * omega;
+    const double prx = pscale * rhx, pry = pscale * rhy, prz = pscale * rhz;
+    out[0] = drho;
+    out[1] = omega * rho * (s.vcx - vx) + drho * s.vcx + prx;
+    out[2] = omega * rho * (s.vcy - vy) + drho * s.vcy + pry;
+    out[3] = omega * rho * (s.vcz - vz) + drho * s.vcz + prz;
+    out[4] = omega * (e_sn + s.e_kin) / s.v_snr + ((s.vcx * prx + s.vcy * pry) + s.vcz * prz);
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// Steps 3 + 5 for one cell.  u = (rho, mx, my, mz, etot, eint) in/out; b = the six buffer channels (dU^sum).
+// Returns eta; *lam receives the Eq. 21 factor; *vold the pre-step velocity (only meaningful when b[0] != 0).
+// ---------------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ double apply_cell(const DevP &P, double u[6], const double b[6], double *lam_out, double vold[3]) {
+    const double a = -b[0];
+    double eta = 1.0;                                   // R12
+    if (a > 0.0) {                                      // Eqs. 15-16 with rho_Tr = inf (R10), generalised (R11)
+        double alim = a;
+        const double cap = P.fmax * u[0];
+        if (cap < alim) alim = cap;
+        double room = u[0] - P.rho_floor;
+        if (room < 0.0) room = 0.0;
+        if (room < alim) alim = room;
+        eta = alim / a;
+        const double rho = u[0];
+        vold[0] = u[1] / rho; vold[1] = u[2] / rho; vold[2] = u[3] / rho;
+        // accretion group is rank one in the cell's own state (R29): dU_f = b0 * (U_f / rho)
+        const double A1 = b[0] * vold[0], A2 = b[0] * vold[1], A3 = b[0] * vold[2];
+        const double A4 = b[0] * (u[4] / rho), A5 = b[0] * (u[5] / rho);
+        u[0] = u[0] + eta * b[0];
+        u[1] = u[1] + eta * A1;
+        u[2] = u[2] + eta * A2;
+        u[3] = u[3] + eta * A3;
+        u[4] = u[4] + eta * A4;
+        u[5] = u[5] + eta * A5;
+    }
+    double lam = 1.0;
+    const bool touched = (b[1] != 0.0) || (b[5] != 0.0) || (b[2] != 0.0) || (b[3] != 0.0) || (b[4] != 0.0);
+    if (touched) {                                      // Eq. 21 (R25), then Eq. 6 for the SN group
+        const double rho1 = u[0], eint1 = u[5];
+        const double rho2 = rho1 + b[1];
+        const double e2 = u[4] + b[5];
+        const double emin = P.theta * rho2 * (eint1 / rho1);
+        const double K = 2.0 * rho2 * (e2 - emin);
+        const double p1x = u[1], p1y = u[2], p1z = u[3];
+        const double qx = p1x + b[2], qy = p1y + b[3], qz = p1z + b[4];
+        const double q2 = (qx * qx + qy * qy) + qz * qz;
+        if (!(q2 <= K)) {
+            const double aa = (b[2] * b[2] + b[3] * b[3]) + b[4] * b[4];
+            const double bb = (p1x * b[2] + p1y * b[3]) + p1z * b[4];
+            const double cc = ((p1x * p1x + p1y * p1y) + p1z * p1z) - K;
+            if (aa > 0.0) {
+                const double disc = bb * bb - aa * cc;
+                if (disc < 0.0) lam = 0.0;
+                else {
+                    lam = (-bb + sqrt(disc)) / aa;
+                    if (lam < 0.0) lam = 0.0;
+                    if (lam > 1.0) lam = 1.0;
+                }
+            }
+        }
+        u[0] = rho2;
+        u[1] = p1x + lam * b[2];
+        u[2] = p1y + lam * b[3];
+        u[3] = p1z + lam * b[4];
+        u[4] = e2;
+        const double ke = ((u[1] * u[1] + u[2] * u[2]) + u[3] * u[3]) / (2.0 * rho2);
+        double ei = e2 - ke;                            // L241
+        if (ei < 0.0) ei = 0.0;
+        u[5] = ei;
+    }
+    *lam_out = lam;
+    return eta;
+}
+
+}  // namespace pm

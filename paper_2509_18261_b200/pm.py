@@ -1,0 +1,345 @@
+"""Thin Python binding over the C ABI of libpm_b200.so (include/pm.h).
+
+Argument marshalling only: every step of the path runs in the CUDA kernels of csrc/pm_b200.cu.  torch is
+used for device memory and the stream handle.  There is no CPU fallback: if the library is missing or was
+not built, importing/using this module raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libpm_b200.so")
+SRC = [os.path.join(_HERE, "csrc", "pm_b200.cu")]
+HDRS = [os.path.join(_HERE, "csrc", "pm_device.cuh"), os.path.join(os.path.dirname(_HERE), "include", "pm.h")]
+
+PM_OK, PM_EINVAL, PM_ENOMEM, PM_ECUDA, PM_EORDER, PM_EDOMAIN = 0, -1, -2, -3, -4, -5
+PM_FLAG_DEBUG_SCALARS, PM_FLAG_DEBUG_LAMBDA = 1, 2
+STATUS_NAMES = {0: "PM_OK", -1: "PM_EINVAL", -2: "PM_ENOMEM", -3: "PM_ECUDA", -4: "PM_EORDER", -5: "PM_EDOMAIN"}
+
+EXPORTS = ["pm_create", "pm_deposit", "pm_fold_ghosts", "pm_apply_limited", "pm_return_to_particles", "pm_check",
+           "pm_step_host", "pm_destroy", "pm_last_error", "pm_launch_count", "pm_debug_buffer",
+           "pm_debug_return_mesh", "pm_debug_lambda", "pm_debug_sink_scalars", "pm_debug_sn_scalars",
+           "pm_debug_stencil"]
+
+c_dp = C.POINTER(C.c_double)
+
+
+class PmParams(C.Structure):
+    _fields_ = [
+        ("nx", C.c_int32), ("ny", C.c_int32), ("nz", C.c_int32),
+        ("sn_nsub", C.c_int32), ("sn_regime", C.c_int32), ("flags", C.c_int32),
+        ("dx", C.c_double), ("x0", C.c_double * 3),
+        ("G", C.c_double), ("gamma", C.c_double), ("cs_iso", C.c_double),
+        ("rk_sink", C.c_double), ("rk_sn", C.c_double),
+        ("bondi_lambda", C.c_double), ("f_max_remove", C.c_double), ("rho_floor", C.c_double),
+        ("sn_eps_k", C.c_double), ("sn_rm_ej", C.c_double), ("sn_rm_mc", C.c_double),
+        ("sn_msf_coeff", C.c_double), ("sn_msf_exp", C.c_double),
+        ("sn_psnr_coeff", C.c_double), ("sn_psnr_exp", C.c_double),
+        ("sn_mu_h", C.c_double), ("sn_nh_unit", C.c_double),
+        ("sn_eint_theta", C.c_double),
+    ]
+
+
+class PmState(C.Structure):
+    _fields_ = [(f, C.c_void_p) for f in ("rho", "mx", "my", "mz", "etot", "eint")]
+
+
+class PmSinks(C.Structure):
+    _fields_ = [("n", C.c_int64)] + [(f, C.c_void_p) for f in
+                                     ("x", "y", "z", "vx", "vy", "vz", "m", "dm", "dpx", "dpy", "dpz")]
+
+
+class PmSNe(C.Structure):
+    _fields_ = [("n", C.c_int64)] + [(f, C.c_void_p) for f in ("x", "y", "z", "vx", "vy", "vz", "e_sn", "m_ej")]
+
+
+class PmError(RuntimeError):
+    def __init__(self, status: int, where: str, msg: str = ""):
+        self.status = status
+        super().__init__(f"{where}: {STATUS_NAMES.get(status, status)} {msg}".strip())
+
+
+def build(force: bool = False, verbose: bool = False) -> str:
+    """Compile libpm_b200.so in-tree for sm_100a (nvcc cross-compiles without a GPU)."""
+    newest = max(os.path.getmtime(p) for p in SRC + HDRS)
+    if not force and os.path.exists(LIB_PATH) and os.path.getmtime(LIB_PATH) >= newest:
+        return LIB_PATH
+    cmd = ["nvcc", "-gencode", "arch=compute_100a,code=sm_100a", "-std=c++17", "-O3", "-lineinfo", "-fmad=false",
+           "-Xcompiler", "-fPIC", "-shared", "-o", LIB_PATH] + SRC
+    if verbose:
+        cmd.insert(1, "-Xptxas=-v")
+    subprocess.check_call(cmd)
+    return LIB_PATH
+
+
+_lib = None
+
+
+def lib():
+    """Load the CUDA library; fail loudly when it is missing (no fallback)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(f"{LIB_PATH} not built: run `python -c 'import __graft_entry__ as g; g.build()'`")
+        L = C.CDLL(LIB_PATH)
+        vp, i32p, i64p = C.c_void_p, C.POINTER(C.c_int32), C.POINTER(C.c_int64)
+        L.pm_create.argtypes = [C.POINTER(PmParams), C.c_int, vp, C.POINTER(vp)]
+        L.pm_deposit.argtypes = [vp, C.POINTER(PmState), C.POINTER(PmSinks), C.POINTER(PmSNe), C.c_double]
+        L.pm_fold_ghosts.argtypes = [vp]
+        L.pm_apply_limited.argtypes = [vp, C.POINTER(PmState)]
+        L.pm_return_to_particles.argtypes = [vp, C.POINTER(PmSinks)]
+        L.pm_check.argtypes = [vp]
+        L.pm_step_host.argtypes = [vp, C.POINTER(PmState), C.POINTER(PmSinks), C.POINTER(PmSNe), C.c_double]
+        L.pm_destroy.argtypes = [vp]
+        L.pm_last_error.argtypes = [vp]
+        L.pm_last_error.restype = C.c_char_p
+        L.pm_launch_count.argtypes = [vp]
+        L.pm_launch_count.restype = C.c_int64
+        L.pm_debug_buffer.argtypes = [vp, C.c_int, C.POINTER(vp), i64p, i64p, i32p]
+        L.pm_debug_return_mesh.argtypes = [vp, C.c_int, C.POINTER(vp)]
+        L.pm_debug_lambda.argtypes = [vp, C.POINTER(vp)]
+        L.pm_debug_sink_scalars.argtypes = [vp, C.POINTER(vp), i64p]
+        L.pm_debug_sn_scalars.argtypes = [vp, C.POINTER(vp), i64p]
+        L.pm_debug_stencil.argtypes = [vp, C.c_int, C.c_double, C.c_double, C.c_double, vp, i32p, i32p]
+        for name in EXPORTS:
+            if name not in ("pm_last_error", "pm_launch_count"):
+                getattr(L, name).restype = C.c_int
+        _lib = L
+    return _lib
+
+
+def make_params(p: dict, flags: int = 0) -> PmParams:
+    o = PmParams()
+    for k, _ in PmParams._fields_:
+        if k == "flags":
+            o.flags = flags
+        elif k == "x0":
+            o.x0[0], o.x0[1], o.x0[2] = (float(v) for v in p["x0"])
+        else:
+            setattr(o, k, p[k])
+    return o
+
+
+def _ptr(t):
+    if t is None:
+        return None
+    assert t.dtype == torch.float64 and t.is_contiguous(), "fp64 contiguous tensors only"
+    return t.data_ptr()
+
+
+def _from_ptr(ptr: int, n: int, device, dtype=torch.float64):
+    """Wrap library-owned device memory in a tensor (debug views only) via __cuda_array_interface__."""
+    typestr = {torch.float64: "<f8", torch.int32: "<i4"}[dtype]
+
+    class _Holder:
+        __cuda_array_interface__ = {"shape": (n,), "typestr": typestr, "data": (ptr, False), "version": 2}
+    return torch.as_tensor(_Holder(), device=device)
+
+
+class DeviceState:
+    FIELDS = ("rho", "mx", "my", "mz", "etot", "eint")
+
+    def __init__(self, *fields):
+        assert len(fields) == 6
+        self.rho, self.mx, self.my, self.mz, self.etot, self.eint = fields
+
+    @classmethod
+    def from_host(cls, st, device):
+        return cls(*(torch.from_numpy(getattr(st, f)).to(device) for f in cls.FIELDS))
+
+    def fields(self):
+        return [getattr(self, f) for f in self.FIELDS]
+
+    def c(self) -> PmState:
+        s = PmState()
+        for f in self.FIELDS:
+            setattr(s, f, _ptr(getattr(self, f)))
+        return s
+
+
+class DeviceSinks:
+    IN = ("x", "y", "z", "vx", "vy", "vz", "m")
+    OUT = ("dm", "dpx", "dpy", "dpz")
+
+    def __init__(self, n, **t):
+        self.n = n
+        for f in self.IN + self.OUT:
+            setattr(self, f, t.get(f))
+
+    @classmethod
+    def from_host(cls, sk, device, with_outputs=True):
+        t = {f: torch.from_numpy(getattr(sk, f)).to(device) for f in cls.IN}
+        if with_outputs:
+            for f in cls.OUT:
+                t[f] = torch.zeros(sk.n, dtype=torch.float64, device=device)
+        return cls(sk.n, **t)
+
+    def c(self) -> PmSinks:
+        s = PmSinks()
+        s.n = self.n
+        for f in self.IN + self.OUT:
+            setattr(s, f, _ptr(getattr(self, f)))
+        return s
+
+
+class DeviceSNe:
+    IN = ("x", "y", "z", "vx", "vy", "vz", "e_sn", "m_ej")
+
+    def __init__(self, n, **t):
+        self.n = n
+        for f in self.IN:
+            setattr(self, f, t.get(f))
+
+    @classmethod
+    def from_host(cls, sn, device):
+        return cls(sn.n, **{f: torch.from_numpy(getattr(sn, f)).to(device) for f in cls.IN})
+
+    def c(self) -> PmSNe:
+        s = PmSNe()
+        s.n = self.n
+        for f in self.IN:
+            setattr(s, f, _ptr(getattr(self, f)))
+        return s
+
+
+class Context:
+    """One pm_ctx.  Methods have the names of the C entry points and only marshal arguments."""
+
+    def __init__(self, params: dict, device="cuda:0", stream=None, flags: int = 0):
+        self.L = lib()
+        self.device = torch.device(device)
+        self.params = dict(params)
+        idx = self.device.index if self.device.index is not None else 0
+        if stream is None:
+            stream = torch.cuda.current_stream(self.device)
+        self.stream = stream
+        self._p = make_params(params, flags)
+        h = C.c_void_p()
+        rc = self.L.pm_create(C.byref(self._p), idx, C.c_void_p(stream.cuda_stream), C.byref(h))
+        if rc != PM_OK:
+            raise PmError(rc, "pm_create")
+        self.h = h
+
+    def _chk(self, rc, where):
+        if rc != PM_OK:
+            raise PmError(rc, where, self.L.pm_last_error(self.h).decode())
+
+    def pm_deposit(self, state: DeviceState, sinks, sne, dt: float):
+        cs = state.c()
+        ck = sinks.c() if sinks is not None else None
+        cn = sne.c() if sne is not None else None
+        self._chk(self.L.pm_deposit(self.h, C.byref(cs), C.byref(ck) if ck else None, C.byref(cn) if cn else None, dt),
+                  "pm_deposit")
+
+    def pm_fold_ghosts(self):
+        self._chk(self.L.pm_fold_ghosts(self.h), "pm_fold_ghosts")
+
+    def pm_apply_limited(self, state: DeviceState):
+        cs = state.c()
+        self._chk(self.L.pm_apply_limited(self.h, C.byref(cs)), "pm_apply_limited")
+
+    def pm_return_to_particles(self, sinks):
+        ck = sinks.c() if sinks is not None else None
+        self._chk(self.L.pm_return_to_particles(self.h, C.byref(ck) if ck else None), "pm_return_to_particles")
+
+    def pm_check(self):
+        self._chk(self.L.pm_check(self.h), "pm_check")
+
+    def step(self, state, sinks, sne, dt):
+        """deposit -> fold -> apply -> return (four C calls, all asynchronous on the ctx stream)."""
+        self.pm_deposit(state, sinks, sne, dt)
+        self.pm_fold_ghosts()
+        self.pm_apply_limited(state)
+        self.pm_return_to_particles(sinks)
+
+    def pm_step_host(self, st, sk, sn, dt: float):
+        """Host-buffer step: st / sk / sn hold numpy arrays or CPU (pinned) tensors; updated in place."""
+        def hp(a):
+            if a is None:
+                return None
+            if isinstance(a, torch.Tensor):
+                assert a.device.type == "cpu" and a.dtype == torch.float64 and a.is_contiguous()
+                return a.data_ptr()
+            assert a.dtype.name == "float64" and a.flags["C_CONTIGUOUS"]
+            return a.ctypes.data
+        cs = PmState()
+        for f in DeviceState.FIELDS:
+            setattr(cs, f, hp(getattr(st, f)))
+        ck = PmSinks()
+        ck.n = sk.n if sk is not None else 0
+        if sk is not None:
+            for f in DeviceSinks.IN + DeviceSinks.OUT:
+                setattr(ck, f, hp(getattr(sk, f, None)))
+        cn = PmSNe()
+        cn.n = sn.n if sn is not None else 0
+        if sn is not None:
+            for f in DeviceSNe.IN:
+                setattr(cn, f, hp(getattr(sn, f)))
+        self._chk(self.L.pm_step_host(self.h, C.byref(cs), C.byref(ck), C.byref(cn), dt), "pm_step_host")
+
+    def pm_launch_count(self) -> int:
+        return int(self.L.pm_launch_count(self.h))
+
+    # ---- test-only views ------------------------------------------------------------------------
+    def debug_buffer(self, channel: int):
+        """Returns (ghosted tensor (nz+2g, ny+2g, pitch), owned view (nz, ny, nx), g)."""
+        ptr = C.c_void_p()
+        dims = (C.c_int64 * 3)()
+        origin = C.c_int64()
+        g = C.c_int32()
+        self._chk(self.L.pm_debug_buffer(self.h, channel, C.byref(ptr), dims, C.byref(origin), C.byref(g)), "pm_debug_buffer")
+        d = [int(v) for v in dims]
+        t = _from_ptr(ptr.value, d[0] * d[1] * d[2], self.device).view(d[0], d[1], d[2])
+        nx, ny, nz = self.params["nx"], self.params["ny"], self.params["nz"]
+        gz = g.value
+        ox = origin.value - (gz * d[1] + gz) * d[2]
+        owned = t[gz:gz + nz, gz:gz + ny, ox:ox + nx]
+        return t, owned, gz, ox
+
+    def debug_return_mesh(self, word: int):
+        ptr = C.c_void_p()
+        self._chk(self.L.pm_debug_return_mesh(self.h, word, C.byref(ptr)), "pm_debug_return_mesh")
+        nx, ny, nz = self.params["nx"], self.params["ny"], self.params["nz"]
+        return _from_ptr(ptr.value, nx * ny * nz, self.device).view(nz, ny, nx)
+
+    def debug_lambda(self):
+        ptr = C.c_void_p()
+        self._chk(self.L.pm_debug_lambda(self.h, C.byref(ptr)), "pm_debug_lambda")
+        nx, ny, nz = self.params["nx"], self.params["ny"], self.params["nz"]
+        return _from_ptr(ptr.value, nx * ny * nz, self.device).view(nz, ny, nx)
+
+    def debug_sink_scalars(self):
+        ptr, n = C.c_void_p(), C.c_int64()
+        self._chk(self.L.pm_debug_sink_scalars(self.h, C.byref(ptr), C.byref(n)), "pm_debug_sink_scalars")
+        return _from_ptr(ptr.value, 8 * n.value, self.device).view(8, n.value)
+
+    def debug_sn_scalars(self):
+        ptr, n = C.c_void_p(), C.c_int64()
+        self._chk(self.L.pm_debug_sn_scalars(self.h, C.byref(ptr), C.byref(n)), "pm_debug_sn_scalars")
+        return _from_ptr(ptr.value, 9 * n.value, self.device).view(9, n.value)
+
+    def debug_stencil(self, kind: int, x: float, y: float, z: float):
+        """(counts reshaped (side, side, side) in (k, j, i) order as a CPU int32 tensor, host cell (i, j, k))."""
+        counts = torch.zeros(17 ** 3, dtype=torch.int32, device=self.device)
+        host = (C.c_int32 * 3)()
+        side = C.c_int32()
+        self._chk(self.L.pm_debug_stencil(self.h, kind, x, y, z, C.c_void_p(counts.data_ptr()), host, C.byref(side)),
+                  "pm_debug_stencil")
+        s = side.value
+        return counts[:s ** 3].view(s, s, s).cpu(), tuple(int(v) for v in host)
+
+    def close(self):
+        if getattr(self, "h", None) is not None and self.h.value:
+            self.L.pm_destroy(self.h)
+            self.h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
