@@ -70,7 +70,7 @@ typedef struct {
 typedef struct {
     double *A[6];        /* signed accretion changes dU^sum (rho, mx, my, mz, etot, eint), <= 0 for rho (R1) */
     double *S[5];        /* SN changes dU^sum (rho, mx, my, mz, etot) */
-    double *Aabs[6];     /* sum_s |dU^s| per channel (Appendix A error scale, L610; R36) */
+    double *Aabs[6];     /* sum over particles of |terms added| per channel (Appendix A error scale, L610; R36) */
     double *Sabs[5];
     double *eta;         /* Eq. 4 ratio for the accretion group */
     double *lam;         /* Eq. 21 lambda for the SN momentum (1 where no SN touches) */
@@ -278,7 +278,7 @@ static void sn_compute_scalars(const orc_params *p, const orc_state *U, double x
 /* O5: Eq. 17 for one cell with omega > 0 (R21, R22). out = (d rho, d px, d py, d pz, d E). */
 static void sn_cell_deposit(const orc_params *p, const sn_scalars *sc, double xs, double ys, double zs,
                             double e_sn, double m_ej, int64_t i, int64_t j, int64_t k, int cnt,
-                            double rho, double vx, double vy, double vz, double out[5]) {
+                            double rho, double vx, double vy, double vz, double out[5], double out_abs[5]) {
     const double nsub3 = (double)p->sn_nsub * (double)p->sn_nsub * (double)p->sn_nsub;
     double omega = (double)cnt / nsub3;
     double ddx = cell_centre(p->x0[0], i, p->dx) - xs;
@@ -295,6 +295,13 @@ static void sn_cell_deposit(const orc_params *p, const sn_scalars *sc, double xs
     out[2] = omega * rho * (sc->vcy - vy) + drho * sc->vcy + pry;
     out[3] = omega * rho * (sc->vcz - vz) + drho * sc->vcz + prz;
     out[4] = omega * (e_sn + sc->e_kin) / sc->v_snr + ((sc->vcx * prx + sc->vcy * pry) + sc->vcz * prz);
+    /* error scale only (Appendix A; R36): the sum of the absolute values of the TERMS added above, since the
+     * velocity-smoothing terms of one particle already cancel against each other */
+    out_abs[0] = drho;
+    out_abs[1] = omega * rho * (fabs(sc->vcx) + fabs(vx)) + drho * fabs(sc->vcx) + fabs(prx);
+    out_abs[2] = omega * rho * (fabs(sc->vcy) + fabs(vy)) + drho * fabs(sc->vcy) + fabs(pry);
+    out_abs[3] = omega * rho * (fabs(sc->vcz) + fabs(vz)) + drho * fabs(sc->vcz) + fabs(prz);
+    out_abs[4] = omega * (e_sn + sc->e_kin) / sc->v_snr + ((fabs(sc->vcx * prx) + fabs(sc->vcy * pry)) + fabs(sc->vcz * prz));
 }
 
 static void store_sn_diag(orc_sne *sn, int64_t s, const sn_scalars *sc) {
@@ -436,9 +443,12 @@ int orc_deposit(const orc_params *p, const orc_state *U, orc_sinks *sk, orc_sne 
                     d[3] = -a * (U->mz[c] / rho);
                     d[4] = -a * (U->etot[c] / rho);
                     d[5] = -a * (U->eint[c] / rho);
+                    /* error scale only (R36): |term| times its condition number with respect to r_acc^2, because
+                     * a ~ exp(-r^2/r_acc^2) amplifies a relative change of r_acc^2 by r^2/r_acc^2 (up to 16 r_K^2/dx^2) */
+                    double cond = 1.0 + r2 / (sc.r_acc * sc.r_acc);
                     for (int f = 0; f < 6; ++f) {
                         mo->A[f][c] += d[f];
-                        if (mo->Aabs[f]) mo->Aabs[f][c] += fabs(d[f]);
+                        if (mo->Aabs[f]) mo->Aabs[f][c] += fabs(d[f]) * cond;
                     }
                     if (mo->sink_count) mo->sink_count[c] += 1;
                 }
@@ -455,12 +465,12 @@ int orc_deposit(const orc_params *p, const orc_state *U, orc_sinks *sk, orc_sne 
                     if (cnt == 0) continue;
                     int64_t c = cell_index(p, i, j, k);
                     double rho = U->rho[c];
-                    double d[5];
+                    double d[5], da[5];
                     sn_cell_deposit(p, &sc, xs, ys, zs, sn->e_sn[s], sn->m_ej[s], i, j, k, cnt,
-                                    rho, U->mx[c] / rho, U->my[c] / rho, U->mz[c] / rho, d);
+                                    rho, U->mx[c] / rho, U->my[c] / rho, U->mz[c] / rho, d, da);
                     for (int f = 0; f < 5; ++f) {
                         mo->S[f][c] += d[f];
-                        if (mo->Sabs[f]) mo->Sabs[f][c] += fabs(d[f]);
+                        if (mo->Sabs[f]) mo->Sabs[f][c] += da[f];
                     }
                     if (mo->sn_count) mo->sn_count[c] += 1;
                 }
@@ -581,7 +591,8 @@ int orc_sample_cells(const orc_params *p, const orc_state *U, const orc_sinks *s
             double a = sink_cell_amount(p, &sc, r2, dt);
             double d[6] = { -a, -a * (U->mx[c] / rho), -a * (U->my[c] / rho), -a * (U->mz[c] / rho),
                             -a * (U->etot[c] / rho), -a * (U->eint[c] / rho) };
-            for (int f = 0; f < 6; ++f) { A[f] += d[f]; Aa[f] += fabs(d[f]); }
+            double cond = 1.0 + r2 / (sc.r_acc * sc.r_acc);
+            for (int f = 0; f < 6; ++f) { A[f] += d[f]; Aa[f] += fabs(d[f]) * cond; }
         }
         for (int64_t s = 0; sn && s < sn->n; ++s) {
             int64_t ih = host_cell(sn->x[s], p->x0[0], inv_dx), jh = host_cell(sn->y[s], p->x0[1], inv_dx), kh = host_cell(sn->z[s], p->x0[2], inv_dx);
@@ -591,10 +602,10 @@ int orc_sample_cells(const orc_params *p, const orc_state *U, const orc_sinks *s
             if (cnt == 0) continue;
             sn_scalars sc;
             sn_compute_scalars(p, U, sn->x[s], sn->y[s], sn->z[s], sn->vx[s], sn->vy[s], sn->vz[s], sn->e_sn[s], sn->m_ej[s], &sc);
-            double d[5];
+            double d[5], da[5];
             sn_cell_deposit(p, &sc, sn->x[s], sn->y[s], sn->z[s], sn->e_sn[s], sn->m_ej[s], ih + di, jh + dj, kh + dk, cnt,
-                            rho, U->mx[c] / rho, U->my[c] / rho, U->mz[c] / rho, d);
-            for (int f = 0; f < 5; ++f) { S[f] += d[f]; Sa[f] += fabs(d[f]); }
+                            rho, U->mx[c] / rho, U->my[c] / rho, U->mz[c] / rho, d, da);
+            for (int f = 0; f < 5; ++f) { S[f] += d[f]; Sa[f] += da[f]; }
             nsn += 1;
         }
         double u[6] = { U->rho[c], U->mx[c], U->my[c], U->mz[c], U->etot[c], U->eint[c] };

@@ -141,8 +141,6 @@ def test_sn_only_params_ghost3():
     w = inputs.scaled_mixed(7, 12, seed_index=5, n_clusters=1)
     w.params["rk_sink"] = 0.0
     w = inputs.Workload("sn7", w.params, w.state, inputs.empty_sinks(), w.sne, w.dt, 1)
-    o = parity.make_oracle(w)
-    o.pd["rk_sink"] = 0.0
     parity.run_and_compare(w, steps=1)
 
 
@@ -232,7 +230,7 @@ def test_config5_large_sampled():
 
     def owned_at(ch):
         return g.ctx.debug_buffer(ch)[1][kz_t, jy_t, ix_t].cpu().numpy()
-    parity.close_strict(owned_at(0), ref["A"][:, 0], "accretion d rho (sampled)")
+    parity.close_reorder(owned_at(0), ref["A"][:, 0], ref["Aabs"][:, 0], "accretion d rho (sampled)")
     parity.close_strict(owned_at(1), ref["S"][:, 0], "SN d rho (sampled)")
     for f in (1, 2, 3, 4):
         parity.close_reorder(owned_at(1 + f), ref["S"][:, f], ref["Sabs"][:, f], f"SN channel {f} (sampled)")
