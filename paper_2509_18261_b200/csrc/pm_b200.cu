@@ -46,6 +46,8 @@ struct pm_ctx {
     double *stg_state;  long long stg_state_cap;
     double *stg_sinks;  long long stg_sinks_cap;
     double *stg_sne;    long long stg_sne_cap;
+    // particle binning: keys[np] | perm[np] | counts[2*ntile + 1]
+    int *bin_mem;       long long bin_cap;
     char msg[256];
 };
 
@@ -71,14 +73,66 @@ __global__ void __launch_bounds__(256) k_zero_buffer(double2 *__restrict__ p, lo
 }
 
 // ---------------------------------------------------------------------------------------------------------------
+// a1: host cells -> bins.  Sinks use keys [0, ntile), SNe [ntile, 2 ntile); perm[0..nk) lists sink indices bin by
+// bin, perm[nk..nk+nn) SN indices.  Order inside a bin is whatever the atomic append gives (results depend on it
+// only through the order of the atomic additions, as they do anyway).
+// ---------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_bin_count(const DevP P, const double *__restrict__ kx, const double *__restrict__ ky,
+                                                   const double *__restrict__ kz, long long nk,
+                                                   const double *__restrict__ nx_, const double *__restrict__ ny_,
+                                                   const double *__restrict__ nz_, long long nn,
+                                                   int *__restrict__ keys, int *__restrict__ counts) {
+    const long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= nk + nn) return;
+    const bool sink = p < nk;
+    const long long q = sink ? p : p - nk;
+    const double x = sink ? kx[q] : nx_[q], y = sink ? ky[q] : ny_[q], z = sink ? kz[q] : nz_[q];
+    int ih = host_cell(x, P.x0[0], P.inv_dx), jh = host_cell(y, P.x0[1], P.inv_dx), kh = host_cell(z, P.x0[2], P.inv_dx);
+    ih = min(max(ih, 0), P.nx - 1); jh = min(max(jh, 0), P.ny - 1); kh = min(max(kh, 0), P.nz - 1);   // outsiders are flagged later
+    const int key = bin_key(P, ih, jh, kh) + (sink ? 0 : P.ntile);
+    keys[p] = key;
+    atomicAdd(counts + key, 1);
+}
+
+// exclusive prefix sum of counts[0..n) in place, one block
+__global__ void __launch_bounds__(1024) k_bin_scan(int *__restrict__ counts, int n) {
+    __shared__ int part[1024];
+    const int t = threadIdx.x;
+    const int chunk = (n + 1023) / 1024;
+    const int lo = min(t * chunk, n), hi = min(lo + chunk, n);
+    int sum = 0;
+    for (int i = lo; i < hi; ++i) sum += counts[i];
+    part[t] = sum;
+    __syncthreads();
+    for (int off = 1; off < 1024; off <<= 1) {
+        const int v = t >= off ? part[t - off] : 0;
+        __syncthreads();
+        part[t] += v;
+        __syncthreads();
+    }
+    int run = part[t] - sum;
+    for (int i = lo; i < hi; ++i) { const int c = counts[i]; counts[i] = run; run += c; }
+}
+
+__global__ void __launch_bounds__(256) k_bin_fill(const int *__restrict__ keys, int *__restrict__ cursor,
+                                                  int *__restrict__ perm, long long np, long long nk) {
+    const long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= np) return;
+    const int pos = atomicAdd(cursor + keys[p], 1);
+    perm[pos] = (int)(p < nk ? p : p - nk);
+}
+
+// ---------------------------------------------------------------------------------------------------------------
 // a1-a3: sinks.  One warp per sink; lanes stride over the (2g+1)^3 box in (k,j,i) order.
 // ---------------------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(128) k_deposit_sinks(const DevP P, const DevState U, const DevSinks S, const double dt,
                                                        double *__restrict__ buf0, double *__restrict__ scal,
-                                                       double *__restrict__ dbg, int *__restrict__ err) {
-    const long long s = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+                                                       double *__restrict__ dbg, int *__restrict__ err,
+                                                       const int *__restrict__ perm) {
+    const long long w = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
     const int lane = threadIdx.x & 31;
-    if (s >= S.n) return;
+    if (w >= S.n) return;
+    const long long s = perm[w];
     const double xs = S.x[s], ys = S.y[s], zs = S.z[s];
     const int ih = host_cell(xs, P.x0[0], P.inv_dx), jh = host_cell(ys, P.x0[1], P.inv_dx), kh = host_cell(zs, P.x0[2], P.inv_dx);
     if (ih < 0 || ih >= P.nx || jh < 0 || jh >= P.ny || kh < 0 || kh >= P.nz) {
@@ -146,11 +200,12 @@ constexpr int kSnWarps = 8;
 
 __global__ void __launch_bounds__(kSnWarps * 32) k_deposit_sne(const DevP P, const DevState U, const DevSNe S,
                                                                 double *__restrict__ buf, double *__restrict__ dbg,
-                                                                int *__restrict__ err) {
+                                                                int *__restrict__ err, const int *__restrict__ perm) {
     extern __shared__ __align__(16) unsigned char smem[];
     const int wib = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const long long s = (long long)blockIdx.x * kSnWarps + wib;
-    if (s >= S.n) return;
+    const long long w = (long long)blockIdx.x * kSnWarps + wib;
+    if (w >= S.n) return;
+    const long long s = perm[w];
     const int g = P.gn, B = 2 * g + 1, nc = B * B * B;
     const SnTables T = sn_tables_at(smem + (size_t)wib * sn_table_bytes(B, P.nsub), B, P.nsub);
     const double xs = S.x[s], ys = S.y[s], zs = S.z[s];
@@ -356,10 +411,12 @@ __global__ void __launch_bounds__(256) k_apply_limited(const DevP P, const DevSt
 // a8: return to particles (Eq. 5).  One warp per sink; shuffle reduction; no atomics.
 // ---------------------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(128) k_return_sinks(const DevP P, const DevSinks S, const double dt,
-                                                      const double *__restrict__ scal, const double *__restrict__ ret) {
-    const long long s = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+                                                      const double *__restrict__ scal, const double *__restrict__ ret,
+                                                      const int *__restrict__ perm) {
+    const long long w = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
     const int lane = threadIdx.x & 31;
-    if (s >= S.n) return;
+    if (w >= S.n) return;
+    const long long s = perm[w];
     const double xs = S.x[s], ys = S.y[s], zs = S.z[s];
     const int ih = host_cell(xs, P.x0[0], P.inv_dx), jh = host_cell(ys, P.x0[1], P.inv_dx), kh = host_cell(zs, P.x0[2], P.inv_dx);
     if (ih < 0 || ih >= P.nx || jh < 0 || jh >= P.ny || kh < 0 || kh >= P.nz) return;   // flagged at deposit
@@ -452,6 +509,8 @@ extern "C" int pm_create(const pm_params *prm, int device, void *cuda_stream, pm
     P.msf_c = prm->sn_msf_coeff; P.msf_e = prm->sn_msf_exp; P.psnr_c = prm->sn_psnr_coeff; P.psnr_e = prm->sn_psnr_exp;
     P.mu_h = prm->sn_mu_h; P.nh_unit = prm->sn_nh_unit; P.theta = prm->sn_eint_theta;
     P.nsub3 = (double)P.nsub * (double)P.nsub * (double)P.nsub;
+    P.nsbx = (((prm->nx + 7) >> 3) + 3) >> 2; P.nsby = (((prm->ny + 7) >> 3) + 3) >> 2; P.nsbz = (((prm->nz + 7) >> 3) + 3) >> 2;
+    P.ntile = P.nsbx * P.nsby * P.nsbz * 64;
 
     cudaError_t e = cudaSetDevice(device);
     if (e == cudaSuccess) e = cudaMalloc(&c->buf, (size_t)kBufChannels * P.Nb * sizeof(double));
@@ -488,6 +547,7 @@ extern "C" int pm_destroy(pm_ctx *c) {
     cudaStreamSynchronize(c->stream);
     double *ptrs[] = { c->buf, c->ret, c->lam, c->sink_scal, c->dbg_sink, c->dbg_sn, c->stg_state, c->stg_sinks, c->stg_sne };
     for (double *p : ptrs) if (p) cudaFree(p);
+    if (c->bin_mem) cudaFree(c->bin_mem);
     if (c->err_flag) cudaFree(c->err_flag);
     if (c->err_host) cudaFreeHost(c->err_host);
     delete c;
@@ -516,6 +576,30 @@ extern "C" int pm_deposit(pm_ctx *c, const pm_state *st, const pm_sinks *sk, con
     if (dbg && (rc = grow(c, &c->dbg_sink, &c->cap_dbg_sink, 8 * nk)) != PM_OK) return rc;
     if (dbg && (rc = grow(c, &c->dbg_sn, &c->cap_dbg_sn, 9 * nn)) != PM_OK) return rc;
 
+    const long long np = nk + nn;
+    int *keys = nullptr, *perm = nullptr, *counts = nullptr;
+    if (np > 0) {   // a1: bin particles by host tile
+        if (np >= (1ll << 31)) PM_FAIL(c, PM_EINVAL, "pm_deposit: too many particles");
+        const long long need = 2 * np + 2ll * P.ntile + 1;
+        if (need > c->bin_cap) {
+            if (c->bin_mem) { PM_CUDA(c, cudaFree(c->bin_mem)); c->bin_mem = nullptr; c->bin_cap = 0; }
+            const long long cap = need + need / 4;
+            cudaError_t e = cudaMalloc(&c->bin_mem, (size_t)cap * sizeof(int));
+            if (e != cudaSuccess) { c->bin_mem = nullptr; PM_FAIL(c, PM_ENOMEM, "cudaMalloc of bins failed: %s", cudaGetErrorString(e)); }
+            c->bin_cap = cap;
+        }
+        keys = c->bin_mem; perm = keys + np; counts = perm + np;
+        const int nkeys = 2 * P.ntile + 1;
+        PM_CUDA(c, cudaMemsetAsync(counts, 0, (size_t)nkeys * sizeof(int), c->stream));
+        const unsigned blocks = (unsigned)((np + 255) / 256);
+        k_bin_count<<<blocks, 256, 0, c->stream>>>(P, nk ? sk->x : nullptr, nk ? sk->y : nullptr, nk ? sk->z : nullptr, nk,
+                                                   nn ? sn->x : nullptr, nn ? sn->y : nullptr, nn ? sn->z : nullptr, nn, keys, counts);
+        if ((rc = check_launch(c, "k_bin_count")) != PM_OK) return rc;
+        k_bin_scan<<<1, 1024, 0, c->stream>>>(counts, nkeys);
+        if ((rc = check_launch(c, "k_bin_scan")) != PM_OK) return rc;
+        k_bin_fill<<<blocks, 256, 0, c->stream>>>(keys, counts, perm, np, nk);
+        if ((rc = check_launch(c, "k_bin_fill")) != PM_OK) return rc;
+    }
     {   // a0: reset (L59 "all cells initialized to zero")
         const long long n2 = (long long)kBufChannels * P.Nb / 2;
         k_zero_buffer<<<148 * 8, 256, 0, c->stream>>>(reinterpret_cast<double2 *>(c->buf), n2);
@@ -525,14 +609,14 @@ extern "C" int pm_deposit(pm_ctx *c, const pm_state *st, const pm_sinks *sk, con
     if (nk > 0) {
         const DevSinks S = { nk, sk->x, sk->y, sk->z, sk->vx, sk->vy, sk->vz, sk->m, sk->dm, sk->dpx, sk->dpy, sk->dpz };
         const unsigned blocks = (unsigned)((nk + 3) / 4);
-        k_deposit_sinks<<<blocks, 128, 0, c->stream>>>(P, U, S, dt, c->buf, c->sink_scal, dbg ? c->dbg_sink : nullptr, c->err_flag);
+        k_deposit_sinks<<<blocks, 128, 0, c->stream>>>(P, U, S, dt, c->buf, c->sink_scal, dbg ? c->dbg_sink : nullptr, c->err_flag, perm);
         if ((rc = check_launch(c, "k_deposit_sinks")) != PM_OK) return rc;
     }
     if (nn > 0) {
         const DevSNe S = { nn, sn->x, sn->y, sn->z, sn->vx, sn->vy, sn->vz, sn->e_sn, sn->m_ej };
         const unsigned blocks = (unsigned)((nn + kSnWarps - 1) / kSnWarps);
         const size_t smem = kSnWarps * sn_table_bytes(2 * P.gn + 1, P.nsub);
-        k_deposit_sne<<<blocks, kSnWarps * 32, smem, c->stream>>>(P, U, S, c->buf, dbg ? c->dbg_sn : nullptr, c->err_flag);
+        k_deposit_sne<<<blocks, kSnWarps * 32, smem, c->stream>>>(P, U, S, c->buf, dbg ? c->dbg_sn : nullptr, c->err_flag, perm + nk);
         if ((rc = check_launch(c, "k_deposit_sne")) != PM_OK) return rc;
     }
     c->n_sinks_dep = nk; c->n_sne_dep = nn; c->dt = dt;
@@ -593,7 +677,7 @@ extern "C" int pm_return_to_particles(pm_ctx *c, pm_sinks *sk) {
         if (!(sk->x && sk->y && sk->z && sk->vx && sk->vy && sk->vz && sk->m)) PM_FAIL(c, PM_EINVAL, "pm_return_to_particles: null sink array");
         const DevSinks S = { nk, sk->x, sk->y, sk->z, sk->vx, sk->vy, sk->vz, sk->m, sk->dm, sk->dpx, sk->dpy, sk->dpz };
         const unsigned blocks = (unsigned)((nk + 3) / 4);
-        k_return_sinks<<<blocks, 128, 0, c->stream>>>(c->P, S, c->dt, c->sink_scal, c->ret);
+        k_return_sinks<<<blocks, 128, 0, c->stream>>>(c->P, S, c->dt, c->sink_scal, c->ret, c->bin_mem + c->n_sinks_dep + c->n_sne_dep);
         int rc = check_launch(c, "k_return_sinks");
         if (rc != PM_OK) return rc;
     }

@@ -28,6 +28,8 @@ struct DevP {
     double lambda, fmax, rho_floor;
     double eps_k, rm_ej, rm_mc, msf_c, msf_e, psnr_c, psnr_e, mu_h, nh_unit, theta;
     double nsub3;
+    int nsbx, nsby, nsbz;   // super-blocks (4x4x4 tiles of 8^3 cells) per axis: the bins particles are ordered by
+    int ntile;              // nsbx*nsby*nsbz*64 bin keys per particle kind
 };
 
 struct DevState { double *rho, *mx, *my, *mz, *etot, *eint; };
@@ -65,6 +67,17 @@ __device__ __forceinline__ long long owned_index(const DevP &P, int i, int j, in
 // ghosted index of UNWRAPPED cell (i,j,k), each in [-g, n+g)
 __device__ __forceinline__ long long ghost_index(const DevP &P, int i, int j, int k) {
     return (long long)(k + P.g) * P.pk + (long long)(j + P.g) * P.pj + (i + P.gx);
+}
+
+// Bin key of a host cell: super-blocks in raster order, the 4x4x4 tiles inside one in Morton order.  Particles are
+// processed bin by bin (a counting sort by this key, filled by atomic append -- no global comparison sort), so that
+// the buffer and state sectors a particle touches are still in L2 from its neighbours.
+__device__ __forceinline__ int bin_key(const DevP &P, int ih, int jh, int kh) {
+    const int tx = ih >> 3, ty = jh >> 3, tz = kh >> 3;
+    const int sb = ((tz >> 2) * P.nsby + (ty >> 2)) * P.nsbx + (tx >> 2);
+    const int lx = tx & 3, ly = ty & 3, lz = tz & 3;
+    const int local = (lx & 1) | ((ly & 1) << 1) | ((lz & 1) << 2) | ((lx & 2) << 2) | ((ly & 2) << 3) | ((lz & 2) << 4);
+    return sb * 64 + local;
 }
 
 __device__ __forceinline__ double sound_speed(const DevP &P, double rho, double eint) {
