@@ -73,7 +73,8 @@ typedef struct {
 
 enum {
     PM_FLAG_DEBUG_SCALARS = 1,   /* keep per-particle scalars (pm_debug_sink_scalars / pm_debug_sn_scalars) */
-    PM_FLAG_DEBUG_LAMBDA = 2     /* keep the Eq. 21 lambda of every cell (pm_debug_lambda) */
+    PM_FLAG_DEBUG_LAMBDA = 2,    /* keep the Eq. 21 lambda of every cell (pm_debug_lambda) */
+    PM_FLAG_GENERIC_KERNELS = 4  /* always use the generic (any radius, any n_sub) deposit / return kernels */
 };
 
 typedef struct { double *rho, *mx, *my, *mz, *etot, *eint; } pm_state;

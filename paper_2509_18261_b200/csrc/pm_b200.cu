@@ -8,6 +8,7 @@
 //   k_apply_limited    a7  fused limiter + apply, 128-bit loads/stores, untouched cells skip the state traffic
 //   k_return_sinks     a8  one warp per sink: sum eta a V (1, v_old) with a shuffle reduction
 #include "pm_device.cuh"
+#include "pm_fast.cuh"
 #include "../../include/pm.h"
 
 #include <cmath>
@@ -48,6 +49,7 @@ struct pm_ctx {
     double *stg_sne;    long long stg_sne_cap;
     // particle binning: keys[np] | perm[np] | counts[2*ntile + 1]
     int *bin_mem;       long long bin_cap;
+    bool force_generic; // PM_FLAG_GENERIC_KERNELS: never take the specialised (g = 3 / n_sub = 4, g = 4) kernels
     char msg[256];
 };
 
@@ -536,6 +538,7 @@ extern "C" int pm_create(const pm_params *prm, int device, void *cuda_stream, pm
         delete c;
         return rc;
     }
+    c->force_generic = (prm->flags & PM_FLAG_GENERIC_KERNELS) != 0;
     c->stage = ST_IDLE;
     *out = c;
     return PM_OK;
@@ -609,14 +612,20 @@ extern "C" int pm_deposit(pm_ctx *c, const pm_state *st, const pm_sinks *sk, con
     if (nk > 0) {
         const DevSinks S = { nk, sk->x, sk->y, sk->z, sk->vx, sk->vy, sk->vz, sk->m, sk->dm, sk->dpx, sk->dpy, sk->dpz };
         const unsigned blocks = (unsigned)((nk + 3) / 4);
-        k_deposit_sinks<<<blocks, 128, 0, c->stream>>>(P, U, S, dt, c->buf, c->sink_scal, dbg ? c->dbg_sink : nullptr, c->err_flag, perm);
+        if (P.gs == 4 && !c->force_generic)
+            k_deposit_sinks_g4<<<blocks, kFastSinkWarps * 32, 0, c->stream>>>(P, U, S, dt, c->buf, c->sink_scal, dbg ? c->dbg_sink : nullptr, c->err_flag, perm);
+        else
+            k_deposit_sinks<<<blocks, 128, 0, c->stream>>>(P, U, S, dt, c->buf, c->sink_scal, dbg ? c->dbg_sink : nullptr, c->err_flag, perm);
         if ((rc = check_launch(c, "k_deposit_sinks")) != PM_OK) return rc;
     }
     if (nn > 0) {
         const DevSNe S = { nn, sn->x, sn->y, sn->z, sn->vx, sn->vy, sn->vz, sn->e_sn, sn->m_ej };
         const unsigned blocks = (unsigned)((nn + kSnWarps - 1) / kSnWarps);
         const size_t smem = kSnWarps * sn_table_bytes(2 * P.gn + 1, P.nsub);
-        k_deposit_sne<<<blocks, kSnWarps * 32, smem, c->stream>>>(P, U, S, c->buf, dbg ? c->dbg_sn : nullptr, c->err_flag, perm + nk);
+        if (P.gn == 3 && P.nsub == 4 && !c->force_generic)
+            k_deposit_sne_g3n4<<<blocks, kFastSnWarps * 32, 0, c->stream>>>(P, U, S, c->buf, dbg ? c->dbg_sn : nullptr, c->err_flag, perm + nk);
+        else
+            k_deposit_sne<<<blocks, kSnWarps * 32, smem, c->stream>>>(P, U, S, c->buf, dbg ? c->dbg_sn : nullptr, c->err_flag, perm + nk);
         if ((rc = check_launch(c, "k_deposit_sne")) != PM_OK) return rc;
     }
     c->n_sinks_dep = nk; c->n_sne_dep = nn; c->dt = dt;
@@ -677,7 +686,11 @@ extern "C" int pm_return_to_particles(pm_ctx *c, pm_sinks *sk) {
         if (!(sk->x && sk->y && sk->z && sk->vx && sk->vy && sk->vz && sk->m)) PM_FAIL(c, PM_EINVAL, "pm_return_to_particles: null sink array");
         const DevSinks S = { nk, sk->x, sk->y, sk->z, sk->vx, sk->vy, sk->vz, sk->m, sk->dm, sk->dpx, sk->dpy, sk->dpz };
         const unsigned blocks = (unsigned)((nk + 3) / 4);
-        k_return_sinks<<<blocks, 128, 0, c->stream>>>(c->P, S, c->dt, c->sink_scal, c->ret, c->bin_mem + c->n_sinks_dep + c->n_sne_dep);
+        const int *perm = c->bin_mem + c->n_sinks_dep + c->n_sne_dep;
+        if (c->P.gs == 4 && !c->force_generic)
+            k_return_sinks_g4<<<blocks, kFastSinkWarps * 32, 0, c->stream>>>(c->P, S, c->dt, c->sink_scal, c->ret, perm);
+        else
+            k_return_sinks<<<blocks, 128, 0, c->stream>>>(c->P, S, c->dt, c->sink_scal, c->ret, perm);
         int rc = check_launch(c, "k_return_sinks");
         if (rc != PM_OK) return rc;
     }

@@ -15,10 +15,10 @@ import torch
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libpm_b200.so")
 SRC = [os.path.join(_HERE, "csrc", "pm_b200.cu")]
-HDRS = [os.path.join(_HERE, "csrc", "pm_device.cuh"), os.path.join(os.path.dirname(_HERE), "include", "pm.h")]
+HDRS = [os.path.join(_HERE, "csrc", "pm_device.cuh"), os.path.join(_HERE, "csrc", "pm_fast.cuh"), os.path.join(os.path.dirname(_HERE), "include", "pm.h")]
 
 PM_OK, PM_EINVAL, PM_ENOMEM, PM_ECUDA, PM_EORDER, PM_EDOMAIN = 0, -1, -2, -3, -4, -5
-PM_FLAG_DEBUG_SCALARS, PM_FLAG_DEBUG_LAMBDA = 1, 2
+PM_FLAG_DEBUG_SCALARS, PM_FLAG_DEBUG_LAMBDA, PM_FLAG_GENERIC_KERNELS = 1, 2, 4
 STATUS_NAMES = {0: "PM_OK", -1: "PM_EINVAL", -2: "PM_ENOMEM", -3: "PM_ECUDA", -4: "PM_EORDER", -5: "PM_EDOMAIN"}
 
 EXPORTS = ["pm_create", "pm_deposit", "pm_fold_ghosts", "pm_apply_limited", "pm_return_to_particles", "pm_check",

@@ -92,6 +92,15 @@ def test_mixed_small_grids(n, npart):
     print(f"cells needing the R36 reorder term: {n2}")
 
 
+def test_generic_kernels_same_contract(monkeypatch):
+    """PM_FLAG_GENERIC_KERNELS: the any-radius / any-n_sub kernels on the shapes the specialised ones normally take."""
+    w = inputs.scaled_mixed(40, 500, seed_index=5)
+    flags = pm.PM_FLAG_DEBUG_SCALARS | pm.PM_FLAG_DEBUG_LAMBDA | pm.PM_FLAG_GENERIC_KERNELS
+    orig = parity.GpuRun.__init__
+    monkeypatch.setattr(parity.GpuRun, "__init__", lambda self, w_, device="cuda:0", flags=flags: orig(self, w_, device, flags))
+    parity.run_and_compare(w, steps=2)
+
+
 def test_seam_particles():
     """Particles whose stencils straddle the periodic seam in every direction exercise ghosts + fold (L284 analogue)."""
     w = inputs.scaled_mixed(32, 64, seed_index=5)
