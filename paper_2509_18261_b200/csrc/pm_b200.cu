@@ -96,14 +96,38 @@ __global__ void __launch_bounds__(256) k_bin_count(const DevP P, const double *_
     atomicAdd(counts + key, 1);
 }
 
-// exclusive prefix sum of counts[0..n) in place, one block
-__global__ void __launch_bounds__(1024) k_bin_scan(int *__restrict__ counts, int n) {
+// Exclusive prefix sum of counts[0..n), two levels: every block scans its own 2048 keys in place and publishes its
+// total; one block then scans the totals; k_bin_fill adds the block offset back.
+constexpr int kScanChunk = 2048;
+
+__global__ void __launch_bounds__(256) k_bin_scan_local(int *__restrict__ counts, int n, int *__restrict__ sums) {
+    __shared__ int part[256];
+    const int t = threadIdx.x;
+    const int base = blockIdx.x * kScanChunk + t * 8;
+    int v[8], sum = 0;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) { v[i] = (base + i < n) ? counts[base + i] : 0; sum += v[i]; }
+    part[t] = sum;
+    __syncthreads();
+    for (int off = 1; off < 256; off <<= 1) {
+        const int add = t >= off ? part[t - off] : 0;
+        __syncthreads();
+        part[t] += add;
+        __syncthreads();
+    }
+    int run = part[t] - sum;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) { if (base + i < n) counts[base + i] = run; run += v[i]; }
+    if (t == 255) sums[blockIdx.x] = part[255];
+}
+
+__global__ void __launch_bounds__(1024) k_bin_scan_sums(int *__restrict__ sums, int n) {
     __shared__ int part[1024];
     const int t = threadIdx.x;
     const int chunk = (n + 1023) / 1024;
     const int lo = min(t * chunk, n), hi = min(lo + chunk, n);
     int sum = 0;
-    for (int i = lo; i < hi; ++i) sum += counts[i];
+    for (int i = lo; i < hi; ++i) sum += sums[i];
     part[t] = sum;
     __syncthreads();
     for (int off = 1; off < 1024; off <<= 1) {
@@ -113,14 +137,16 @@ __global__ void __launch_bounds__(1024) k_bin_scan(int *__restrict__ counts, int
         __syncthreads();
     }
     int run = part[t] - sum;
-    for (int i = lo; i < hi; ++i) { const int c = counts[i]; counts[i] = run; run += c; }
+    for (int i = lo; i < hi; ++i) { const int c = sums[i]; sums[i] = run; run += c; }
 }
 
 __global__ void __launch_bounds__(256) k_bin_fill(const int *__restrict__ keys, int *__restrict__ cursor,
-                                                  int *__restrict__ perm, long long np, long long nk) {
+                                                  const int *__restrict__ sums, int *__restrict__ perm, long long np,
+                                                  long long nk) {
     const long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= np) return;
-    const int pos = atomicAdd(cursor + keys[p], 1);
+    const int key = keys[p];
+    const int pos = atomicAdd(cursor + key, 1) + sums[key / kScanChunk];
     perm[pos] = (int)(p < nk ? p : p - nk);
 }
 
@@ -488,6 +514,7 @@ extern "C" int pm_create(const pm_params *prm, int device, void *cuda_stream, pm
     if (prm->nx < 2 * g + 1 || prm->ny < 2 * g + 1 || prm->nz < 2 * g + 1) return PM_EINVAL;     // R32
     const long long N = (long long)prm->nx * prm->ny * prm->nz;
     if (N >= (1ll << 31)) return PM_EINVAL;
+    if ((long long)(prm->nx + 2 * g + 2) * (prm->ny + 2 * g) * (prm->nz + 2 * g) >= (1ll << 31)) return PM_EINVAL;
 
     pm_ctx *c = new (std::nothrow) pm_ctx();
     if (!c) return PM_ENOMEM;
@@ -583,7 +610,9 @@ extern "C" int pm_deposit(pm_ctx *c, const pm_state *st, const pm_sinks *sk, con
     int *keys = nullptr, *perm = nullptr, *counts = nullptr;
     if (np > 0) {   // a1: bin particles by host tile
         if (np >= (1ll << 31)) PM_FAIL(c, PM_EINVAL, "pm_deposit: too many particles");
-        const long long need = 2 * np + 2ll * P.ntile + 1;
+        const int nkeys = 2 * P.ntile + 1;
+        const int nscan = (nkeys + kScanChunk - 1) / kScanChunk;
+        const long long need = 2 * np + nkeys + nscan;
         if (need > c->bin_cap) {
             if (c->bin_mem) { PM_CUDA(c, cudaFree(c->bin_mem)); c->bin_mem = nullptr; c->bin_cap = 0; }
             const long long cap = need + need / 4;
@@ -592,15 +621,17 @@ extern "C" int pm_deposit(pm_ctx *c, const pm_state *st, const pm_sinks *sk, con
             c->bin_cap = cap;
         }
         keys = c->bin_mem; perm = keys + np; counts = perm + np;
-        const int nkeys = 2 * P.ntile + 1;
+        int *sums = counts + nkeys;
         PM_CUDA(c, cudaMemsetAsync(counts, 0, (size_t)nkeys * sizeof(int), c->stream));
         const unsigned blocks = (unsigned)((np + 255) / 256);
         k_bin_count<<<blocks, 256, 0, c->stream>>>(P, nk ? sk->x : nullptr, nk ? sk->y : nullptr, nk ? sk->z : nullptr, nk,
                                                    nn ? sn->x : nullptr, nn ? sn->y : nullptr, nn ? sn->z : nullptr, nn, keys, counts);
         if ((rc = check_launch(c, "k_bin_count")) != PM_OK) return rc;
-        k_bin_scan<<<1, 1024, 0, c->stream>>>(counts, nkeys);
-        if ((rc = check_launch(c, "k_bin_scan")) != PM_OK) return rc;
-        k_bin_fill<<<blocks, 256, 0, c->stream>>>(keys, counts, perm, np, nk);
+        k_bin_scan_local<<<nscan, 256, 0, c->stream>>>(counts, nkeys, sums);
+        if ((rc = check_launch(c, "k_bin_scan_local")) != PM_OK) return rc;
+        k_bin_scan_sums<<<1, 1024, 0, c->stream>>>(sums, nscan);
+        if ((rc = check_launch(c, "k_bin_scan_sums")) != PM_OK) return rc;
+        k_bin_fill<<<blocks, 256, 0, c->stream>>>(keys, counts, sums, perm, np, nk);
         if ((rc = check_launch(c, "k_bin_fill")) != PM_OK) return rc;
     }
     {   // a0: reset (L59 "all cells initialized to zero")

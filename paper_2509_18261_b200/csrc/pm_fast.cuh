@@ -14,11 +14,15 @@ namespace pm {
 constexpr int kFastSnWarps = 8;
 constexpr int kSnB = 7, kSnCells = 343, kSnNs = 4;
 
+// Box cell (a, b, c) = (x, y, z offsets in 0..6) packed as a | b << 3 | c << 6 (< 448).
 struct __align__(16) SnWarpSmem {
     double d2[3][kSnB * kSnNs];     // squared sub-sample offsets per axis
     double dmin[3][8], dmax[3][8];  // per-cell min / max of them
-    unsigned short list[352];       // boundary-cell list, then active-cell list
-    unsigned char cnt[352];         // omega counts (0..64)
+    double dc[3][8];                // cell-centre offsets from the particle per axis
+    int off[3][8];                  // wrapped owned-index contribution per axis (x: i, y: j*nx, z: k*nx*ny)
+    int goff[2][8];                 // ghosted-index contribution of y and z
+    unsigned short list[352];       // boundary-cell list, then active-cell list (packed codes)
+    unsigned char cnt[448];         // omega counts (0..64) by packed code
 };
 
 __device__ __forceinline__ unsigned lanemask_lt() {
@@ -30,10 +34,16 @@ __device__ __forceinline__ unsigned lanemask_lt() {
 __device__ __forceinline__ double pick3(int ax, double a, double b, double c) { return ax == 0 ? a : (ax == 1 ? b : c); }
 
 // One warp per SN particle, particles taken in bin order (perm).
-__global__ void __launch_bounds__(kFastSnWarps * 32, 2) k_deposit_sne_g3n4(const DevP P, const DevState U, const DevSNe S,
+__global__ void __launch_bounds__(kFastSnWarps * 32, 3) k_deposit_sne_g3n4(const DevP P, const DevState U, const DevSNe S,
                                                                             double *__restrict__ buf, double *__restrict__ dbg,
                                                                             int *__restrict__ err, const int *__restrict__ perm) {
     __shared__ SnWarpSmem sm_all[kFastSnWarps];
+    __shared__ unsigned short dec[352];          // linear box index -> packed code, shared by the CTA
+    for (int c = threadIdx.x; c < kSnCells; c += blockDim.x) {
+        const int a = c % 7, t = c / 7;
+        dec[c] = (unsigned short)(a | ((t % 7) << 3) | ((t / 7) << 6));
+    }
+    __syncthreads();
     const int wib = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const long long w = (long long)blockIdx.x * kFastSnWarps + wib;
     if (w >= S.n) return;
@@ -59,6 +69,18 @@ __global__ void __launch_bounds__(kFastSnWarps * 32, 2) k_deposit_sne_g3n4(const
             sm.d2[ax][t] = d * d;
         }
     }
+    if (lane < 21) {
+        const int ax = lane / 7, c = lane - ax * 7;
+        const double x0 = pick3(ax, P.x0[0], P.x0[1], P.x0[2]);
+        const double ps = pick3(ax, xs, ys, zs);
+        const int h = ax == 0 ? ih : (ax == 1 ? jh : kh);
+        const int n = ax == 0 ? P.nx : (ax == 1 ? P.ny : P.nz);
+        const int u = h - 3 + c;                                  // unwrapped cell index
+        sm.dc[ax][c] = cell_centre(x0, u, P.dx) - ps;
+        const int wq = wrap1(u, n);
+        sm.off[ax][c] = ax == 0 ? wq : (ax == 1 ? wq * P.nx : wq * P.nx * P.ny);
+        if (ax > 0) sm.goff[ax - 1][c] = (int)((u + P.g) * (ax == 1 ? P.pj : P.pk));
+    }
     __syncwarp();
     if (lane < 21) {
         const int ax = lane / 7, c = lane - ax * 7;
@@ -74,23 +96,25 @@ __global__ void __launch_bounds__(kFastSnWarps * 32, 2) k_deposit_sne_g3n4(const
     for (int r = 0; r < 11; ++r) {
         const int c = lane + 32 * r;
         bool boundary = false;
+        int pc = 0;
         if (c < kSnCells) {
-            const int a = c % 7, t = c / 7, b = t % 7, cc = t / 7;
+            pc = dec[c];
+            const int a = pc & 7, b = (pc >> 3) & 7, cc = pc >> 6;
             const bool full = (sm.dmax[2][cc] + sm.dmax[1][b]) + sm.dmax[0][a] <= rk2;
             const bool empty = (sm.dmin[2][cc] + sm.dmin[1][b]) + sm.dmin[0][a] > rk2;
             boundary = !full && !empty;
-            sm.cnt[c] = full ? 64 : 0;
+            sm.cnt[pc] = full ? 64 : 0;
         }
         const unsigned m = __ballot_sync(0xffffffffu, boundary);
-        if (boundary) sm.list[nb + __popc(m & lanemask_lt())] = (unsigned short)c;
+        if (boundary) sm.list[nb + __popc(m & lanemask_lt())] = (unsigned short)pc;
         nb += __popc(m);
     }
     __syncwarp();
     // ---- phase 2: the 64 sub-sample tests of every boundary cell ---------------------------------------------------
 #pragma unroll 1
     for (int idx = lane; idx < nb; idx += 32) {
-        const int c = sm.list[idx];
-        const int a = c % 7, t = c / 7, b = t % 7, cc = t / 7;
+        const int pc = sm.list[idx];
+        const int a = pc & 7, b = (pc >> 3) & 7, cc = pc >> 6;
         const double x0 = sm.d2[0][4 * a], x1 = sm.d2[0][4 * a + 1], x2 = sm.d2[0][4 * a + 2], x3 = sm.d2[0][4 * a + 3];
         double yv[4], zv[4];
 #pragma unroll
@@ -103,7 +127,7 @@ __global__ void __launch_bounds__(kFastSnWarps * 32, 2) k_deposit_sne_g3n4(const
                 const double sy = zv[qz] + yv[qy];
                 cnt += ((sy + x0) <= rk2) + ((sy + x1) <= rk2) + ((sy + x2) <= rk2) + ((sy + x3) <= rk2);
             }
-        sm.cnt[c] = (unsigned char)cnt;
+        sm.cnt[pc] = (unsigned char)cnt;
     }
     __syncwarp();
     // ---- phase 3: list of cells with omega > 0 -------------------------------------------------------------------
@@ -111,9 +135,10 @@ __global__ void __launch_bounds__(kFastSnWarps * 32, 2) k_deposit_sne_g3n4(const
 #pragma unroll 1
     for (int r = 0; r < 11; ++r) {
         const int c = lane + 32 * r;
-        const bool act = c < kSnCells && sm.cnt[c] != 0;
+        const int pc = c < kSnCells ? dec[c] : 0;
+        const bool act = c < kSnCells && sm.cnt[pc] != 0;
         const unsigned m = __ballot_sync(0xffffffffu, act);
-        if (act) sm.list[na + __popc(m & lanemask_lt())] = (unsigned short)c;
+        if (act) sm.list[na + __popc(m & lanemask_lt())] = (unsigned short)pc;
         na += __popc(m);
     }
     __syncwarp();
@@ -122,10 +147,10 @@ __global__ void __launch_bounds__(kFastSnWarps * 32, 2) k_deposit_sne_g3n4(const
     double m_gas = 0.0, px = 0.0, py = 0.0, pz = 0.0, v_snr = 0.0;
 #pragma unroll 1
     for (int idx = lane; idx < na; idx += 32) {
-        const int c = sm.list[idx];
-        const int a = c % 7, t = c / 7, b = t % 7, cc = t / 7;
-        const double omega = (double)sm.cnt[c] * (1.0 / 64.0);          // exact: power of two
-        const long long q = owned_index(P, ih - 3 + a, jh - 3 + b, kh - 3 + cc);
+        const int pc = sm.list[idx];
+        const int a = pc & 7, b = (pc >> 3) & 7, cc = pc >> 6;
+        const double omega = (double)sm.cnt[pc] * (1.0 / 64.0);         // exact: power of two
+        const int q = sm.off[2][cc] + sm.off[1][b] + sm.off[0][a];
         const double rho = U.rho[q], mx = U.mx[q], my = U.my[q], mz = U.mz[q];
         const double rinv = 1.0 / rho;
         const double mcell = omega * rho * P.V;
@@ -140,26 +165,24 @@ __global__ void __launch_bounds__(kFastSnWarps * 32, 2) k_deposit_sne_g3n4(const
     // ---- phase 5: Eq. 17 and the atomic additions (O5) -----------------------------------------------------------
     const double inv_vsnr = 1.0 / sc.v_snr;
     const double e_dens = (e_sn + sc.e_kin);
+    double *const sbuf = buf + P.Nb + (ih - 3 + P.gx);
 #pragma unroll 1
     for (int idx = lane; idx < na; idx += 32) {
-        const int c = sm.list[idx];
-        const int a = c % 7, t = c / 7, b = t % 7, cc = t / 7;
-        const int i = ih - 3 + a, j = jh - 3 + b, k = kh - 3 + cc;
-        const double omega = (double)sm.cnt[c] * (1.0 / 64.0);
-        const long long q = owned_index(P, i, j, k);
+        const int pc = sm.list[idx];
+        const int a = pc & 7, b = (pc >> 3) & 7, cc = pc >> 6;
+        const double omega = (double)sm.cnt[pc] * (1.0 / 64.0);
+        const int q = sm.off[2][cc] + sm.off[1][b] + sm.off[0][a];
         const double rho = U.rho[q], mx = U.mx[q], my = U.my[q], mz = U.mz[q];
         const double rinv = 1.0 / rho;
         const double vx = mx * rinv, vy = my * rinv, vz = mz * rinv;
-        const double ddx = cell_centre(P.x0[0], i, P.dx) - xs;
-        const double ddy = cell_centre(P.x0[1], j, P.dx) - ys;
-        const double ddz = cell_centre(P.x0[2], k, P.dx) - zs;
+        const double ddx = sm.dc[0][a], ddy = sm.dc[1][b], ddz = sm.dc[2][cc];
         const double r2 = dist2(ddx, ddy, ddz);
         const double ir = r2 > 0.0 ? rsqrt(r2) : 0.0;                  // rhat = 0 at r = 0 (R21)
         const double drho = omega * m_ej * inv_vsnr;
         const double pscale = (sc.p_rad * inv_vsnr) * omega * ir;
         const double prx = pscale * ddx, pry = pscale * ddy, prz = pscale * ddz;
         const double wr = omega * rho;
-        double *dst = buf + P.Nb + ghost_index(P, i, j, k);
+        double *dst = sbuf + (sm.goff[1][cc] + sm.goff[0][b] + a);
         atomicAdd(dst, drho);
         atomicAdd(dst + P.Nb, wr * (sc.vcx - vx) + drho * sc.vcx + prx);
         atomicAdd(dst + 2 * P.Nb, wr * (sc.vcy - vy) + drho * sc.vcy + pry);
