@@ -388,11 +388,12 @@ __device__ __forceinline__ void stv(double *p, const double v[VEC]) {
 }
 
 template <int VEC, bool LAM>
-__global__ void __launch_bounds__(256) k_apply_limited(const DevP P, const DevState U, const double *__restrict__ buf,
+__global__ void __launch_bounds__(256, 3) k_apply_limited(const DevP P, const DevState U, const double *__restrict__ buf,
                                                        double *__restrict__ ret, double *__restrict__ lam_out,
                                                        unsigned int n_items, unsigned int items_per_row) {
-    const unsigned int item = blockIdx.x * blockDim.x + threadIdx.x;
-    if (item >= n_items) return;
+    const unsigned int item_raw = blockIdx.x * blockDim.x + threadIdx.x;
+    const bool valid = item_raw < n_items;
+    const unsigned int item = valid ? item_raw : 0u;
     const unsigned int row = item / items_per_row;
     const unsigned int i0 = (item - row * items_per_row) * VEC;
     const unsigned int k = row / (unsigned int)P.ny, j = row - k * (unsigned int)P.ny;
@@ -406,10 +407,12 @@ __global__ void __launch_bounds__(256) k_apply_limited(const DevP P, const DevSt
     for (int ch = 0; ch < kBufChannels; ++ch)
 #pragma unroll
         for (int v = 0; v < VEC; ++v) any |= (b[ch][v] != 0.0);
-    if (!any) {
-        if (LAM) { double one[VEC]; for (int v = 0; v < VEC; ++v) one[v] = 1.0; stv<VEC>(lam_out + q, one); }
-        return;                                 // dU^sum = 0: U unchanged, nothing to write
-    }
+    any = any && valid;
+    // Skip at WARP granularity: a warp covers 32*VEC consecutive cells of each field (512 B per stream at VEC = 2), so
+    // the state traffic is either whole coalesced lines or nothing (sector-sparse reads waste DRAM bursts).
+    const bool wany = __any_sync(0xffffffffu, any);
+    if (LAM && valid && !any) { double one[VEC]; for (int v = 0; v < VEC; ++v) one[v] = 1.0; stv<VEC>(lam_out + q, one); }
+    if (!wany || !valid) return;                // dU^sum = 0 on the whole segment: U unchanged, nothing to read or write
     double *fld[6] = { U.rho, U.mx, U.my, U.mz, U.etot, U.eint };
     double u[6][VEC];
 #pragma unroll
@@ -430,6 +433,7 @@ __global__ void __launch_bounds__(256) k_apply_limited(const DevP P, const DevSt
             ret[3 * P.N + q + v] = vold[2];
         }
     }
+    if (!any) return;                           // lanes of a touched segment whose own cells are untouched
 #pragma unroll
     for (int f = 0; f < 6; ++f) stv<VEC>(fld[f] + q, u[f]);
     if (LAM) stv<VEC>(lam_out + q, lam);
