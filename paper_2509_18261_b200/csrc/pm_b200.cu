@@ -18,6 +18,10 @@
 
 using namespace pm;
 
+// Preferred shared-memory carve-out (% of the 256 KB L1) of the sink kernels: measured on config 5, 25 / 50 / 75 / 100 %
+// give 1.06 / 0.56 / 0.54 / 0.79 ms (deposit) and 0.93 / 0.44 / 0.37 / 0.56 ms (return); the SN kernel is best at the default.
+constexpr int kSinkCarveout = 75;
+
 // ---------------------------------------------------------------------------------------------------------------
 // context
 // ---------------------------------------------------------------------------------------------------------------
@@ -27,6 +31,7 @@ struct pm_ctx {
     pm_params prm;
     DevP P;
     int device;
+    int sm_count;
     cudaStream_t stream;
     double *buf;        // kBufChannels * Nb
     double *ret;        // kRetWords * N (NULL when rk_sink == 0)
@@ -546,6 +551,11 @@ extern "C" int pm_create(const pm_params *prm, int device, void *cuda_stream, pm
     P.ntile = P.nsbx * P.nsby * P.nsbz * 64;
 
     cudaError_t e = cudaSetDevice(device);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, device);
+    if (e == cudaSuccess) {   // L1 / shared-memory split of the particle kernels (measured)
+        e = cudaFuncSetAttribute(k_deposit_sinks_g4, cudaFuncAttributePreferredSharedMemoryCarveout, kSinkCarveout);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_return_sinks_g4, cudaFuncAttributePreferredSharedMemoryCarveout, kSinkCarveout);
+    }
     if (e == cudaSuccess) e = cudaMalloc(&c->buf, (size_t)kBufChannels * P.Nb * sizeof(double));
     if (e == cudaSuccess && gs > 0) e = cudaMalloc(&c->ret, (size_t)kRetWords * N * sizeof(double));
     if (e == cudaSuccess && (prm->flags & PM_FLAG_DEBUG_LAMBDA)) e = cudaMalloc(&c->lam, (size_t)N * sizeof(double));
@@ -640,7 +650,7 @@ extern "C" int pm_deposit(pm_ctx *c, const pm_state *st, const pm_sinks *sk, con
     }
     {   // a0: reset (L59 "all cells initialized to zero")
         const long long n2 = (long long)kBufChannels * P.Nb / 2;
-        k_zero_buffer<<<148 * 8, 256, 0, c->stream>>>(reinterpret_cast<double2 *>(c->buf), n2);
+        k_zero_buffer<<<c->sm_count * 8, 256, 0, c->stream>>>(reinterpret_cast<double2 *>(c->buf), n2);
         if ((rc = check_launch(c, "k_zero_buffer")) != PM_OK) return rc;
     }
     const DevState U = { st->rho, st->mx, st->my, st->mz, st->etot, st->eint };

@@ -1,0 +1,202 @@
+// pm_sn_fast.cuh -- specialised supernova deposit (a1, a4, a5) for kernel half-width 3 with 4 sub-samples per axis,
+// the shape every BASELINE config uses.  Same arithmetic contract as the generic k_deposit_sne (every omega count is
+// the exact number of sub-samples with (dz^2 + dy^2) + dx^2 <= r_K^2), but:
+//   * box sizes are compile-time, so index decoding is multiply-shift instead of runtime division;
+//   * cells are first classified, then COMPACTED with warp ballots, so the expensive work (64 sub-sample tests of a
+//     boundary cell; gather / scatter of a cell with omega > 0) runs on full warps instead of diverged ones;
+//   * 1/rho and 1/r are formed once per cell and multiplied (<= 1 ulp from the oracle's divisions, far inside the
+//     1e-12 parity tolerance; no integer depends on them).
+// One fused kernel on purpose: its arithmetic phases (tables, classification, sub-sample tests) and its memory phases
+// (gather, fp64 RED scatter) belong to different warps at any moment and overlap on the SM.  A split into a geometry
+// kernel and a gather/scatter kernel was measured slower.
+#pragma once
+#include "pm_device.cuh"
+
+namespace pm {
+
+constexpr int kFastSnWarps = 8;
+constexpr int kSnB = 7, kSnCells = 343, kSnNs = 4;
+
+// Box cell (a, b, c) = (x, y, z offsets in 0..6) packed as a | b << 3 | c << 6 (< 448).
+struct __align__(16) SnWarpSmem {
+    double d2[3][kSnB * kSnNs];     // squared sub-sample offsets per axis
+    double dmin[3][8], dmax[3][8];  // per-cell min / max of them
+    double dc[3][8];                // cell-centre offsets from the particle per axis
+    int off[3][8];                  // wrapped owned-index contribution per axis (x: i, y: j*nx, z: k*nx*ny)
+    int goff[2][8];                 // ghosted-index contribution of y and z
+    unsigned short list[352];       // boundary-cell list, then active-cell list (packed codes)
+    unsigned char cnt[448];         // omega counts (0..64) by packed code
+};
+
+__device__ __forceinline__ unsigned lanemask_lt() {
+    unsigned m;
+    asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m));
+    return m;
+}
+
+__device__ __forceinline__ double pick3(int ax, double a, double b, double c) { return ax == 0 ? a : (ax == 1 ? b : c); }
+
+// One warp per SN particle, particles taken in bin order (perm).
+__global__ void __launch_bounds__(kFastSnWarps * 32, 3) k_deposit_sne_g3n4(const DevP P, const DevState U, const DevSNe S,
+                                                                            double *__restrict__ buf, double *__restrict__ dbg,
+                                                                            int *__restrict__ err, const int *__restrict__ perm) {
+    __shared__ SnWarpSmem sm_all[kFastSnWarps];
+    __shared__ unsigned short dec[352];          // linear box index -> packed code, shared by the CTA
+    for (int c = threadIdx.x; c < kSnCells; c += blockDim.x) {
+        const int a = c % 7, t = c / 7;
+        dec[c] = (unsigned short)(a | ((t % 7) << 3) | ((t / 7) << 6));
+    }
+    __syncthreads();
+    const int wib = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const long long w = (long long)blockIdx.x * kFastSnWarps + wib;
+    if (w >= S.n) return;
+    SnWarpSmem &sm = sm_all[wib];
+    const long long s = perm[w];
+    const double xs = S.x[s], ys = S.y[s], zs = S.z[s];
+    const int ih = host_cell(xs, P.x0[0], P.inv_dx), jh = host_cell(ys, P.x0[1], P.inv_dx), kh = host_cell(zs, P.x0[2], P.inv_dx);
+    if (ih < 0 || ih >= P.nx || jh < 0 || jh >= P.ny || kh < 0 || kh >= P.nz) {
+        if (lane == 0) atomicOr(err, 1);
+        return;
+    }
+    // ---- phase 0: per-axis tables -------------------------------------------------------------------------------
+#pragma unroll
+    for (int r = 0; r < 3; ++r) {
+        const int e = lane + 32 * r;
+        if (e < 3 * kSnB * kSnNs) {
+            const int ax = e / (kSnB * kSnNs), t = e - ax * (kSnB * kSnNs);
+            const int c = t >> 2, q = t & 3;
+            const double x0 = pick3(ax, P.x0[0], P.x0[1], P.x0[2]);
+            const double ps = pick3(ax, xs, ys, zs);
+            const int h = ax == 0 ? ih : (ax == 1 ? jh : kh);
+            const double d = sub_centre(x0, h - 3 + c, q, kSnNs, P.dx) - ps;
+            sm.d2[ax][t] = d * d;
+        }
+    }
+    if (lane < 21) {
+        const int ax = lane / 7, c = lane - ax * 7;
+        const double x0 = pick3(ax, P.x0[0], P.x0[1], P.x0[2]);
+        const double ps = pick3(ax, xs, ys, zs);
+        const int h = ax == 0 ? ih : (ax == 1 ? jh : kh);
+        const int n = ax == 0 ? P.nx : (ax == 1 ? P.ny : P.nz);
+        const int u = h - 3 + c;                                  // unwrapped cell index
+        sm.dc[ax][c] = cell_centre(x0, u, P.dx) - ps;
+        const int wq = wrap1(u, n);
+        sm.off[ax][c] = ax == 0 ? wq : (ax == 1 ? wq * P.nx : wq * P.nx * P.ny);
+        if (ax > 0) sm.goff[ax - 1][c] = (int)((u + P.g) * (ax == 1 ? P.pj : P.pk));
+    }
+    __syncwarp();
+    if (lane < 21) {
+        const int ax = lane / 7, c = lane - ax * 7;
+        const double v0 = sm.d2[ax][4 * c], v1 = sm.d2[ax][4 * c + 1], v2 = sm.d2[ax][4 * c + 2], v3 = sm.d2[ax][4 * c + 3];
+        sm.dmin[ax][c] = fmin(fmin(v0, v1), fmin(v2, v3));
+        sm.dmax[ax][c] = fmax(fmax(v0, v1), fmax(v2, v3));
+    }
+    __syncwarp();
+    // ---- phase 1: classify the 343 cells; full -> 64, empty -> 0, boundary -> list ---------------------------------
+    const double rk2 = P.rk2_sn;
+    int nb = 0;
+#pragma unroll 1
+    for (int r = 0; r < 11; ++r) {
+        const int c = lane + 32 * r;
+        bool boundary = false;
+        int pc = 0;
+        if (c < kSnCells) {
+            pc = dec[c];
+            const int a = pc & 7, b = (pc >> 3) & 7, cc = pc >> 6;
+            const bool full = (sm.dmax[2][cc] + sm.dmax[1][b]) + sm.dmax[0][a] <= rk2;
+            const bool empty = (sm.dmin[2][cc] + sm.dmin[1][b]) + sm.dmin[0][a] > rk2;
+            boundary = !full && !empty;
+            sm.cnt[pc] = full ? 64 : 0;
+        }
+        const unsigned m = __ballot_sync(0xffffffffu, boundary);
+        if (boundary) sm.list[nb + __popc(m & lanemask_lt())] = (unsigned short)pc;
+        nb += __popc(m);
+    }
+    __syncwarp();
+    // ---- phase 2: the 64 sub-sample tests of every boundary cell ---------------------------------------------------
+#pragma unroll 1
+    for (int idx = lane; idx < nb; idx += 32) {
+        const int pc = sm.list[idx];
+        const int a = pc & 7, b = (pc >> 3) & 7, cc = pc >> 6;
+        const double x0 = sm.d2[0][4 * a], x1 = sm.d2[0][4 * a + 1], x2 = sm.d2[0][4 * a + 2], x3 = sm.d2[0][4 * a + 3];
+        double yv[4], zv[4];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) { yv[q] = sm.d2[1][4 * b + q]; zv[q] = sm.d2[2][4 * cc + q]; }
+        int cnt = 0;
+#pragma unroll
+        for (int qz = 0; qz < 4; ++qz)
+#pragma unroll
+            for (int qy = 0; qy < 4; ++qy) {
+                const double sy = zv[qz] + yv[qy];
+                cnt += ((sy + x0) <= rk2) + ((sy + x1) <= rk2) + ((sy + x2) <= rk2) + ((sy + x3) <= rk2);
+            }
+        sm.cnt[pc] = (unsigned char)cnt;
+    }
+    __syncwarp();
+    // ---- phase 3: list of cells with omega > 0 -------------------------------------------------------------------
+    int na = 0;
+#pragma unroll 1
+    for (int r = 0; r < 11; ++r) {
+        const int c = lane + 32 * r;
+        const int pc = c < kSnCells ? dec[c] : 0;
+        const bool act = c < kSnCells && sm.cnt[pc] != 0;
+        const unsigned m = __ballot_sync(0xffffffffu, act);
+        if (act) sm.list[na + __popc(m & lanemask_lt())] = (unsigned short)pc;
+        na += __popc(m);
+    }
+    __syncwarp();
+    // ---- phase 4: stencil sums (O4) --------------------------------------------------------------------------------
+    const double vsx = S.vx[s], vsy = S.vy[s], vsz = S.vz[s], e_sn = S.e_sn[s], m_ej = S.m_ej[s];
+    double m_gas = 0.0, px = 0.0, py = 0.0, pz = 0.0, v_snr = 0.0;
+#pragma unroll 1
+    for (int idx = lane; idx < na; idx += 32) {
+        const int pc = sm.list[idx];
+        const int a = pc & 7, b = (pc >> 3) & 7, cc = pc >> 6;
+        const double omega = (double)sm.cnt[pc] * (1.0 / 64.0);         // exact: power of two
+        const int q = sm.off[2][cc] + sm.off[1][b] + sm.off[0][a];
+        const double rho = U.rho[q], mx = U.mx[q], my = U.my[q], mz = U.mz[q];
+        const double rinv = 1.0 / rho;
+        const double mcell = omega * rho * P.V;
+        m_gas += mcell;
+        px += mcell * (mx * rinv);
+        py += mcell * (my * rinv);
+        pz += mcell * (mz * rinv);
+        v_snr += omega * P.V;
+    }
+    m_gas = warp_sum(m_gas); px = warp_sum(px); py = warp_sum(py); pz = warp_sum(pz); v_snr = warp_sum(v_snr);
+    const SnScalars sc = sn_scalars(P, m_gas, px, py, pz, v_snr, vsx, vsy, vsz, e_sn, m_ej);
+    // ---- phase 5: Eq. 17 and the atomic additions (O5) -----------------------------------------------------------
+    const double inv_vsnr = 1.0 / sc.v_snr;
+    const double e_dens = (e_sn + sc.e_kin);
+    double *const sbuf = buf + P.Nb + (ih - 3 + P.gx);
+#pragma unroll 1
+    for (int idx = lane; idx < na; idx += 32) {
+        const int pc = sm.list[idx];
+        const int a = pc & 7, b = (pc >> 3) & 7, cc = pc >> 6;
+        const double omega = (double)sm.cnt[pc] * (1.0 / 64.0);
+        const int q = sm.off[2][cc] + sm.off[1][b] + sm.off[0][a];
+        const double rho = U.rho[q], mx = U.mx[q], my = U.my[q], mz = U.mz[q];
+        const double rinv = 1.0 / rho;
+        const double vx = mx * rinv, vy = my * rinv, vz = mz * rinv;
+        const double ddx = sm.dc[0][a], ddy = sm.dc[1][b], ddz = sm.dc[2][cc];
+        const double r2 = dist2(ddx, ddy, ddz);
+        const double ir = r2 > 0.0 ? rsqrt(r2) : 0.0;                  // rhat = 0 at r = 0 (R21)
+        const double drho = omega * m_ej * inv_vsnr;
+        const double pscale = (sc.p_rad * inv_vsnr) * omega * ir;
+        const double prx = pscale * ddx, pry = pscale * ddy, prz = pscale * ddz;
+        const double wr = omega * rho;
+        double *dst = sbuf + (sm.goff[1][cc] + sm.goff[0][b] + a);
+        atomicAdd(dst, drho);
+        atomicAdd(dst + P.Nb, wr * (sc.vcx - vx) + drho * sc.vcx + prx);
+        atomicAdd(dst + 2 * P.Nb, wr * (sc.vcy - vy) + drho * sc.vcy + pry);
+        atomicAdd(dst + 3 * P.Nb, wr * (sc.vcz - vz) + drho * sc.vcz + prz);
+        atomicAdd(dst + 4 * P.Nb, omega * e_dens * inv_vsnr + ((sc.vcx * prx + sc.vcy * pry) + sc.vcz * prz));
+    }
+    if (dbg && lane == 0) {
+        const long long n = S.n;
+        dbg[s] = sc.m_snr; dbg[n + s] = sc.v_snr; dbg[2 * n + s] = sc.vcx; dbg[3 * n + s] = sc.vcy; dbg[4 * n + s] = sc.vcz;
+        dbg[5 * n + s] = sc.n_h; dbg[6 * n + s] = sc.r_m; dbg[7 * n + s] = sc.p_rad; dbg[8 * n + s] = (double)sc.regime;
+    }
+}
+
+}  // namespace pm

@@ -15,7 +15,8 @@ import torch
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libpm_b200.so")
 SRC = [os.path.join(_HERE, "csrc", "pm_b200.cu")]
-HDRS = [os.path.join(_HERE, "csrc", "pm_device.cuh"), os.path.join(_HERE, "csrc", "pm_fast.cuh"), os.path.join(os.path.dirname(_HERE), "include", "pm.h")]
+HDRS = [os.path.join(_HERE, "csrc", "pm_device.cuh"), os.path.join(_HERE, "csrc", "pm_fast.cuh"),
+        os.path.join(_HERE, "csrc", "pm_sn_fast.cuh"), os.path.join(_HERE, "csrc", "pm_sink_fast.cuh"), os.path.join(os.path.dirname(_HERE), "include", "pm.h")]
 
 PM_OK, PM_EINVAL, PM_ENOMEM, PM_ECUDA, PM_EORDER, PM_EDOMAIN = 0, -1, -2, -3, -4, -5
 PM_FLAG_DEBUG_SCALARS, PM_FLAG_DEBUG_LAMBDA, PM_FLAG_GENERIC_KERNELS = 1, 2, 4
