@@ -51,7 +51,7 @@ class ClockSampler:
     def start(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
-                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                          "--format=csv,noheader,nounits", "-lms", "20"],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.t = threading.Thread(target=self._read, daemon=True)
             self.t.start()
@@ -140,6 +140,36 @@ def run_reference(args, rank, world):
 
 
 # ---------------------------------------------------------------------------------------------
+def reduce_max(x: float, world: int, device) -> float:
+    """Max over ranks of a host scalar (the contract's timing rule); a no-op at world == 1."""
+    if world <= 1:
+        return float(x)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([x], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t[0])
+
+
+def whole_job_value(cells_per_rank: int, steps: int, world: int, total_ms: float) -> float:
+    """Mcell-updates/s of the whole job: every rank (replica) updates cells_per_rank cells per step."""
+    return world * cells_per_rank * steps / (total_ms * 1e-3) / 1e6
+
+
+def algorithmic_bytes(N, Nb, nk, nn, t4, ts4, tn4):
+    """Bytes each kernel group must move per step (SURVEY.md 8(d) per-cell figures times
+    the fraction of 32-byte sectors (4 cells) that hold a touched cell -- the smallest unit HBM moves)."""
+    return {
+        "bin": 8.0 * 3 * (nk + nn) + 4.0 * 3 * (nk + nn),            # positions read, keys + perm written and read
+        "zero": 8.0 * 6 * Nb,                                        # store only
+        "sinks": 8.0 * 5 * ts4 * N + 8.0 * 1 * ts4 * N + 8.0 * 10 * nk,   # gather 5 fields, write back 1 channel once
+        "sne": 8.0 * 4 * tn4 * N + 8.0 * 5 * tn4 * N + 8.0 * 8 * nn,      # gather 4 fields, write back 5 channels once
+        "fold": 3 * 8.0 * 6 * (Nb - N),                              # read ghosts, read-modify-write owned images
+        "apply": N * (48.0 + 96.0 * t4 + 32.0 * ts4),                # 6 buffer words; 6 + 6 state words and 4 return words where touched
+        "return": 8.0 * 4 * ts4 * N + 8.0 * 12 * nk,
+    }
+
+
 def run_ours(args, rank, world, local_rank):
     import numpy as np
     import torch
@@ -164,8 +194,9 @@ def run_ours(args, rank, world, local_rank):
     else:
         w = inputs.scaled_mixed(n, args.particles, seed_index=5)
     N = n ** 3
+    Nb = (n + 8) ** 3
     npart = w.sinks.n + w.sne.n
-    ctx = pm.Context(w.params, device=str(dev))
+    ctx = pm.Context(w.params, device=str(dev), flags=pm.PM_FLAG_TIMING)
     st = pm.DeviceState.from_host(w.state, dev)
     sk = pm.DeviceSinks.from_host(w.sinks, dev)
     sn = pm.DeviceSNe.from_host(w.sne, dev)
@@ -182,19 +213,23 @@ def run_ours(args, rank, world, local_rank):
         ctx.pm_return_to_particles(sk)
         if ev: ev[4].record()
 
-    for _ in range(max(args.warmup, 3)):
+    warm = max(args.warmup, 3)
+    for _ in range(warm):
         one_step()
     ctx.pm_check()
-    # activity fractions of the buffer the timed steps will see (for the algorithmic-bytes figure)
+    # activity fractions of the buffer the timed steps will see, at 32-byte sector (4-cell) granularity
     ctx.pm_deposit(st, sk, sn, w.dt)
     ctx.pm_fold_ghosts()
-    own = [ctx.debug_buffer(ch)[1] for ch in range(6)]
-    sink_touched = own[0] != 0
-    touched = sink_touched.clone()
-    for ch in range(1, 6):
-        touched |= own[ch] != 0
+    sink_touched = ctx.debug_buffer(0)[1] != 0
+    sn_touched = ctx.debug_buffer(1)[1] != 0          # SN d rho > 0 wherever an SN stencil has omega > 0
+    touched = sink_touched | sn_touched
+
+    def frac4(m):
+        return float(m.reshape(-1, 4).any(dim=1).double().mean())
+
     t_frac, ts_frac = float(touched.double().mean()), float(sink_touched.double().mean())
-    del touched, sink_touched, own
+    t4, ts4, tn4 = frac4(touched), frac4(sink_touched), frac4(sn_touched)
+    del touched, sink_touched, sn_touched
     ctx.pm_apply_limited(st)
     ctx.pm_return_to_particles(sk)
 
@@ -209,14 +244,21 @@ def run_ours(args, rank, world, local_rank):
     clocks = sampler.stop()
     launches = ctx.pm_launch_count() - launches0
     ctx.pm_check()
-    total_ms = evs[0][0].elapsed_time(evs[-1][4])
+    total_ms = reduce_max(evs[0][0].elapsed_time(evs[-1][4]), world, dev)
     stage_ms = {nm: sum(e[i].elapsed_time(e[i + 1]) for e in evs) / args.steps for i, nm in enumerate(stage_names)}
-    t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    total_ms = float(t[0])
     ms_per_step = total_ms / args.steps
-    value = world * N * args.steps / (total_ms * 1e-3) / 1e6
+    value = whole_job_value(N, args.steps, world, total_ms)
+    # per-kernel device times: the library's own CUDA events on the launching stream (PM_FLAG_TIMING), three more steps
+    ksamples = []
+    for _ in range(3):
+        one_step()
+        ksamples.append(ctx.pm_kernel_times())
+    kernel_ms = {k: float(np.median([s[k] for s in ksamples])) for k in pm.KERNEL_GROUPS}
+    red_probe = None
+    if rank == 0 and world == 1:
+        red_probe = {"l2_resident_64MB_5ch": ctx.pm_probe_red_f64(64 << 20, 5),
+                     "hbm_footprint_5GB_5ch": ctx.pm_probe_red_f64(5 << 30, 5), "unit": "1e9 fp64 RED lanes/s",
+                     "pattern": "rows of 7 consecutive doubles, 5 planes (pm_probe_red_f64)"}
 
     # ---- e2e through pm_step_host with pinned host buffers --------------------------------------
     e2e_steps = max(1, min(args.steps, args.e2e_steps))
@@ -224,66 +266,65 @@ def run_ours(args, rank, world, local_rank):
     hk = w.sinks.copy()
     for f in ("dm", "dpx", "dpy", "dpz"):
         setattr(hk, f, np.zeros(hk.n))
-    ctx2 = ctx                                  # same ctx: staging is allocated on first use
     del st
     torch.cuda.empty_cache()
-    ctx2.pm_step_host(hst, hk, w.sne, w.dt)     # warm-up (allocates staging)
+    ctx.pm_step_host(hst, hk, w.sne, w.dt)      # warm-up (allocates staging)
     barrier()
     t0 = time.perf_counter()
     for _ in range(e2e_steps):
-        ctx2.pm_step_host(hst, hk, w.sne, w.dt)
+        ctx.pm_step_host(hst, hk, w.sne, w.dt)
     torch.cuda.synchronize(dev)
-    e2e_s = (time.perf_counter() - t0) / e2e_steps
-    te = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(te, op=dist.ReduceOp.MAX)
-    e2e_s = float(te[0])
+    e2e_s = reduce_max((time.perf_counter() - t0) / e2e_steps, world, dev)
     h2d = 6 * N * 8 + 7 * w.sinks.n * 8 + 8 * w.sne.n * 8
     d2h = 6 * N * 8 + 8 * w.sinks.n * 8
 
     if rank == 0:
         peak, peak_src = measured_peak()
-        # algorithmic bytes of the dominant kernel (k_apply_limited), DESIGN.md "Algorithmic bytes":
-        # every cell reads its 6 buffer words; a touched cell reads + writes 6 state words; a cell a sink
-        # removed mass from also writes the 4 return words.
-        apply_bytes = N * (48.0 + 96.0 * t_frac + 32.0 * ts_frac)
-        dense_bytes = N * 176.0
-        apply_s = stage_ms["apply"] * 1e-3
-        step_bytes = None
+        abytes = algorithmic_bytes(N, Nb, w.sinks.n, w.sne.n, t4, ts4, tn4)
+        kernels = {}
+        for k in pm.KERNEL_GROUPS:
+            if kernel_ms[k] > 0:
+                gbs = abytes[k] / (kernel_ms[k] * 1e-3) / 1e9
+                kernels[k] = {"ms": kernel_ms[k], "algorithmic_bytes": abytes[k], "achieved_gbs": gbs,
+                              "frac_of_measured_peak": gbs / peak, "traffic": ncu_traffic(k)}
+        dom = max(kernels, key=lambda k: kernels[k]["ms"])
+        kname = {"sne": "k_deposit_sne_g3n4", "apply": "k_apply_limited", "zero": "k_zero_buffer", "sinks": "k_deposit_sinks_g4",
+                 "fold": "k_fold_ghosts", "return": "k_return_sinks_g4", "bin": "k_bin_*"}[dom]
+        step_bytes = sum(abytes.values())
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+            "warmup": warm, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": w.name, "cells": N, "particles": npart, "sinks": w.sinks.n, "sne": w.sne.n,
                        "multi_gpu": "replicas only" if world > 1 else "single GPU",
                        "l2_policy": "inputs larger than L2 (state 6 fields + 6-channel buffer, GBs >> 126 MB)",
-                       "touched_cell_fraction": t_frac, "sink_touched_fraction": ts_frac},
+                       "touched_cell_fraction": t_frac, "sink_touched_fraction": ts_frac,
+                       "touched_sector_fraction": t4, "sink_sector_fraction": ts4, "sn_sector_fraction": tn4},
             "particles_per_s": world * npart * args.steps / (total_ms * 1e-3),
             "stage_ms": stage_ms,
+            "kernel_ms": kernel_ms,
             "clocks": clocks,
             "e2e": {"value": world * N / e2e_s / 1e6, "unit": UNIT, "h2d_bytes_per_step": h2d,
                     "d2h_bytes_per_step": d2h, "ms_per_step": e2e_s * 1e3, "steps": e2e_steps,
                     "api": "pm_step_host (pinned host buffers)"},
             "gpu_launches": launches,
-            "roofline": {"bound": "hbm", "kernel": "k_apply_limited", "achieved": apply_bytes / apply_s / 1e9,
-                         "peak": peak, "unit": "GB/s", "frac": apply_bytes / apply_s / 1e9 / peak,
-                         "peak_source": peak_src, "traffic": ncu_traffic("k_apply_limited"),
-                         "algorithmic_bytes_per_launch": apply_bytes,
-                         "dense_equivalent_gbs": dense_bytes / apply_s / 1e9,
-                         "frac_of_8tbs_nominal": apply_bytes / apply_s / 1e9 / 8000.0},
+            "roofline": {"bound": "hbm", "kernel": kname, "achieved": kernels[dom]["achieved_gbs"], "peak": peak,
+                         "unit": "GB/s", "frac": kernels[dom]["frac_of_measured_peak"], "peak_source": peak_src,
+                         "traffic": kernels[dom]["traffic"], "algorithmic_bytes_per_launch": abytes[dom],
+                         "launch_ms": kernels[dom]["ms"], "share_of_step": kernels[dom]["ms"] / sum(kernel_ms.values()),
+                         "timing": "CUDA events recorded by the library on the launching stream (PM_FLAG_TIMING), median of 3 steps",
+                         "frac_of_8tbs_nominal": kernels[dom]["achieved_gbs"] / 8000.0},
+            "kernels": kernels,
+            "step_roofline": {"algorithmic_bytes_per_step": step_bytes,
+                              "achieved_gbs": step_bytes / (ms_per_step * 1e-3) / 1e9,
+                              "frac_of_measured_peak": step_bytes / (ms_per_step * 1e-3) / 1e9 / peak,
+                              "frac_of_8tbs_nominal": step_bytes / (ms_per_step * 1e-3) / 1e9 / 8000.0,
+                              "dense_survey_bytes": 8.0 * 6 * Nb + 8.0 * 5 * N + 120.0 * npart + 144.0 * (Nb - N) + 176.0 * N + 32.0 * ts4 * N},
         }
-        # whole-step roofline (SURVEY 8(d) algorithmic bytes of the step, with the same activity fractions)
-        Nb = (n + 8) ** 3
-        step_bytes = (8.0 * 6 * Nb                       # buffer written once
-                      + 8.0 * 5 * min(1.0, t_frac) * N   # gather reads, each touched state cell once (upper bound)
-                      + 8.0 * 15 * npart                 # particle records
-                      + 3 * 8.0 * 6 * (Nb - N)           # fold
-                      + apply_bytes
-                      + 8.0 * 4 * ts_frac * N)           # return reads
-        line["step_roofline"] = {"algorithmic_bytes_per_step": step_bytes,
-                                 "achieved_gbs": step_bytes / (ms_per_step * 1e-3) / 1e9,
-                                 "frac_of_measured_peak": step_bytes / (ms_per_step * 1e-3) / 1e9 / peak,
-                                 "frac_of_8tbs_nominal": step_bytes / (ms_per_step * 1e-3) / 1e9 / 8000.0}
+        if red_probe:
+            n_red = 5.0 * 183.0 * w.sne.n     # ~183 cells with omega > 0 per SN (SURVEY.md 8 probe), 5 channels
+            red_probe["sn_deposit_achieved"] = n_red / (kernel_ms["sne"] * 1e-3) / 1e9 if kernel_ms["sne"] > 0 else None
+            line["red_throughput"] = red_probe
         if world == 1 and not args.no_cpu_baseline:
             r = time_oracle(ORACLE_SAMPLE_N, 1)
             line["cpu_baseline"] = {k: r[k] for k in ("value", "unit", "cores", "kind", "sample")}

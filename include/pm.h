@@ -74,7 +74,8 @@ typedef struct {
 enum {
     PM_FLAG_DEBUG_SCALARS = 1,   /* keep per-particle scalars (pm_debug_sink_scalars / pm_debug_sn_scalars) */
     PM_FLAG_DEBUG_LAMBDA = 2,    /* keep the Eq. 21 lambda of every cell (pm_debug_lambda) */
-    PM_FLAG_GENERIC_KERNELS = 4  /* always use the generic (any radius, any n_sub) deposit / return kernels */
+    PM_FLAG_GENERIC_KERNELS = 4, /* always use the generic (any radius, any n_sub) deposit / return kernels */
+    PM_FLAG_TIMING = 8           /* bracket every kernel with CUDA events on the ctx's stream (pm_kernel_times) */
 };
 
 typedef struct { double *rho, *mx, *my, *mz, *etot, *eint; } pm_state;
@@ -129,6 +130,19 @@ const char *pm_last_error(const pm_ctx *ctx);
 
 /* Number of kernels this ctx has launched so far (bench.py's gpu_launches). */
 int64_t pm_launch_count(const pm_ctx *ctx);
+
+/* Device time of each kernel group in the most recent step, in milliseconds, measured with CUDA events recorded on the
+ * ctx's stream around the launches (needs PM_FLAG_TIMING; synchronises).  ms (HOST, n >= PM_NUM_KERNELS floats):
+ * PM_K_BIN (the four binning kernels), PM_K_ZERO, PM_K_SINKS, PM_K_SNE, PM_K_FOLD, PM_K_APPLY, PM_K_RETURN;
+ * a group that did not run reports 0. */
+enum { PM_K_BIN = 0, PM_K_ZERO = 1, PM_K_SINKS = 2, PM_K_SNE = 3, PM_K_FOLD = 4, PM_K_APPLY = 5, PM_K_RETURN = 6, PM_NUM_KERNELS = 7 };
+int pm_kernel_times(pm_ctx *ctx, float *ms, int32_t n);
+
+/* Measured fp64 RED (atomic add without return) throughput of this device for the deposit's access pattern: every
+ * warp adds to rows of 7 consecutive doubles at pseudo-random row positions in `channels` planes spread over
+ * `footprint_bytes` of ctx-allocated scratch (freed before returning).  *gops (HOST) receives 1e9 lane-additions per
+ * second.  footprint below the 126 MB L2 measures the L2 atomic units, far above it the HBM-miss path.  Synchronises. */
+int pm_probe_red_f64(pm_ctx *ctx, int64_t footprint_bytes, int32_t channels, double *gops);
 
 /* ---- test-only views (not timed) ---------------------------------------------------------------------------- */
 

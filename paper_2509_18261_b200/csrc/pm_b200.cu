@@ -54,6 +54,9 @@ struct pm_ctx {
     double *stg_sne;    long long stg_sne_cap;
     // particle binning: keys[np] | perm[np] | counts[2*ntile + 1]
     int *bin_mem;       long long bin_cap;
+    bool timing;        // PM_FLAG_TIMING
+    cudaEvent_t ev[PM_NUM_KERNELS][2];
+    bool ev_used[PM_NUM_KERNELS];
     bool force_generic; // PM_FLAG_GENERIC_KERNELS: never take the specialised (g = 3 / n_sub = 4, g = 4) kernels
     char msg[256];
 };
@@ -67,6 +70,13 @@ static int check_launch(pm_ctx *c, const char *name) {
     c->launches += 1;
     if (e != cudaSuccess) { snprintf(c->msg, sizeof(c->msg), "launch of %s failed: %s", name, cudaGetErrorString(e)); return PM_ECUDA; }
     return PM_OK;
+}
+
+// PM_FLAG_TIMING: events on the launching stream around kernel group k (which = 0 before, 1 after)
+static void tick(pm_ctx *c, int k, int which) {
+    if (!c->timing) return;
+    cudaEventRecord(c->ev[k][which], c->stream);
+    if (which) c->ev_used[k] = true;
 }
 
 // ---------------------------------------------------------------------------------------------------------------
@@ -580,6 +590,9 @@ extern "C" int pm_create(const pm_params *prm, int device, void *cuda_stream, pm
         return rc;
     }
     c->force_generic = (prm->flags & PM_FLAG_GENERIC_KERNELS) != 0;
+    c->timing = (prm->flags & PM_FLAG_TIMING) != 0;
+    if (c->timing)
+        for (int k = 0; k < PM_NUM_KERNELS; ++k) { cudaEventCreate(&c->ev[k][0]); cudaEventCreate(&c->ev[k][1]); }
     c->stage = ST_IDLE;
     *out = c;
     return PM_OK;
@@ -591,6 +604,8 @@ extern "C" int pm_destroy(pm_ctx *c) {
     cudaStreamSynchronize(c->stream);
     double *ptrs[] = { c->buf, c->ret, c->lam, c->sink_scal, c->dbg_sink, c->dbg_sn, c->stg_state, c->stg_sinks, c->stg_sne };
     for (double *p : ptrs) if (p) cudaFree(p);
+    if (c->timing)
+        for (int k = 0; k < PM_NUM_KERNELS; ++k) { cudaEventDestroy(c->ev[k][0]); cudaEventDestroy(c->ev[k][1]); }
     if (c->bin_mem) cudaFree(c->bin_mem);
     if (c->err_flag) cudaFree(c->err_flag);
     if (c->err_host) cudaFreeHost(c->err_host);
@@ -620,6 +635,7 @@ extern "C" int pm_deposit(pm_ctx *c, const pm_state *st, const pm_sinks *sk, con
     if (dbg && (rc = grow(c, &c->dbg_sink, &c->cap_dbg_sink, 8 * nk)) != PM_OK) return rc;
     if (dbg && (rc = grow(c, &c->dbg_sn, &c->cap_dbg_sn, 9 * nn)) != PM_OK) return rc;
 
+    for (int k = 0; k < PM_NUM_KERNELS; ++k) c->ev_used[k] = false;
     const long long np = nk + nn;
     int *keys = nullptr, *perm = nullptr, *counts = nullptr;
     if (np > 0) {   // a1: bin particles by host tile
@@ -638,6 +654,7 @@ extern "C" int pm_deposit(pm_ctx *c, const pm_state *st, const pm_sinks *sk, con
         int *sums = counts + nkeys;
         PM_CUDA(c, cudaMemsetAsync(counts, 0, (size_t)nkeys * sizeof(int), c->stream));
         const unsigned blocks = (unsigned)((np + 255) / 256);
+        tick(c, PM_K_BIN, 0);
         k_bin_count<<<blocks, 256, 0, c->stream>>>(P, nk ? sk->x : nullptr, nk ? sk->y : nullptr, nk ? sk->z : nullptr, nk,
                                                    nn ? sn->x : nullptr, nn ? sn->y : nullptr, nn ? sn->z : nullptr, nn, keys, counts);
         if ((rc = check_launch(c, "k_bin_count")) != PM_OK) return rc;
@@ -647,31 +664,38 @@ extern "C" int pm_deposit(pm_ctx *c, const pm_state *st, const pm_sinks *sk, con
         if ((rc = check_launch(c, "k_bin_scan_sums")) != PM_OK) return rc;
         k_bin_fill<<<blocks, 256, 0, c->stream>>>(keys, counts, sums, perm, np, nk);
         if ((rc = check_launch(c, "k_bin_fill")) != PM_OK) return rc;
+        tick(c, PM_K_BIN, 1);
     }
     {   // a0: reset (L59 "all cells initialized to zero")
         const long long n2 = (long long)kBufChannels * P.Nb / 2;
+        tick(c, PM_K_ZERO, 0);
         k_zero_buffer<<<c->sm_count * 8, 256, 0, c->stream>>>(reinterpret_cast<double2 *>(c->buf), n2);
         if ((rc = check_launch(c, "k_zero_buffer")) != PM_OK) return rc;
+        tick(c, PM_K_ZERO, 1);
     }
     const DevState U = { st->rho, st->mx, st->my, st->mz, st->etot, st->eint };
     if (nk > 0) {
         const DevSinks S = { nk, sk->x, sk->y, sk->z, sk->vx, sk->vy, sk->vz, sk->m, sk->dm, sk->dpx, sk->dpy, sk->dpz };
         const unsigned blocks = (unsigned)((nk + 3) / 4);
+        tick(c, PM_K_SINKS, 0);
         if (P.gs == 4 && !c->force_generic)
             k_deposit_sinks_g4<<<blocks, kFastSinkWarps * 32, 0, c->stream>>>(P, U, S, dt, c->buf, c->sink_scal, dbg ? c->dbg_sink : nullptr, c->err_flag, perm);
         else
             k_deposit_sinks<<<blocks, 128, 0, c->stream>>>(P, U, S, dt, c->buf, c->sink_scal, dbg ? c->dbg_sink : nullptr, c->err_flag, perm);
         if ((rc = check_launch(c, "k_deposit_sinks")) != PM_OK) return rc;
+        tick(c, PM_K_SINKS, 1);
     }
     if (nn > 0) {
         const DevSNe S = { nn, sn->x, sn->y, sn->z, sn->vx, sn->vy, sn->vz, sn->e_sn, sn->m_ej };
         const unsigned blocks = (unsigned)((nn + kSnWarps - 1) / kSnWarps);
         const size_t smem = kSnWarps * sn_table_bytes(2 * P.gn + 1, P.nsub);
+        tick(c, PM_K_SNE, 0);
         if (P.gn == 3 && P.nsub == 4 && !c->force_generic)
             k_deposit_sne_g3n4<<<blocks, kFastSnWarps * 32, 0, c->stream>>>(P, U, S, c->buf, dbg ? c->dbg_sn : nullptr, c->err_flag, perm + nk);
         else
             k_deposit_sne<<<blocks, kSnWarps * 32, smem, c->stream>>>(P, U, S, c->buf, dbg ? c->dbg_sn : nullptr, c->err_flag, perm + nk);
         if ((rc = check_launch(c, "k_deposit_sne")) != PM_OK) return rc;
+        tick(c, PM_K_SNE, 1);
     }
     c->n_sinks_dep = nk; c->n_sne_dep = nn; c->dt = dt;
     c->stage = ST_DEPOSITED;
@@ -689,8 +713,10 @@ extern "C" int pm_fold_ghosts(pm_ctx *c) {
     const long long n_x = (long long)(P.nz - g2) * (P.ny - g2) * g2;
     const long long n_edge = n_z + n_y + n_x;
     const unsigned blocks = (unsigned)((n_edge + 255) / 256);
+    tick(c, PM_K_FOLD, 0);
     k_fold_ghosts<<<blocks, 256, 0, c->stream>>>(P, c->buf, n_edge, n_z, n_y);
     int rc = check_launch(c, "k_fold_ghosts");
+    tick(c, PM_K_FOLD, 1);
     if (rc != PM_OK) return rc;
     c->stage = ST_FOLDED;
     return PM_OK;
@@ -714,8 +740,10 @@ extern "C" int pm_apply_limited(pm_ctx *c, pm_state *st) {
     const DevState U = { st->rho, st->mx, st->my, st->mz, st->etot, st->eint };
     const bool vec2 = (c->P.nx % 2 == 0) && aligned16(st->rho) && aligned16(st->mx) && aligned16(st->my) &&
                       aligned16(st->mz) && aligned16(st->etot) && aligned16(st->eint);
+    tick(c, PM_K_APPLY, 0);
     if (vec2) launch_apply<2>(c, U); else launch_apply<1>(c, U);
     int rc = check_launch(c, "k_apply_limited");
+    tick(c, PM_K_APPLY, 1);
     if (rc != PM_OK) return rc;
     c->stage = ST_APPLIED;
     return PM_OK;
@@ -732,12 +760,14 @@ extern "C" int pm_return_to_particles(pm_ctx *c, pm_sinks *sk) {
         const DevSinks S = { nk, sk->x, sk->y, sk->z, sk->vx, sk->vy, sk->vz, sk->m, sk->dm, sk->dpx, sk->dpy, sk->dpz };
         const unsigned blocks = (unsigned)((nk + 3) / 4);
         const int *perm = c->bin_mem + c->n_sinks_dep + c->n_sne_dep;
+        tick(c, PM_K_RETURN, 0);
         if (c->P.gs == 4 && !c->force_generic)
             k_return_sinks_g4<<<blocks, kFastSinkWarps * 32, 0, c->stream>>>(c->P, S, c->dt, c->sink_scal, c->ret, perm);
         else
             k_return_sinks<<<blocks, 128, 0, c->stream>>>(c->P, S, c->dt, c->sink_scal, c->ret, perm);
         int rc = check_launch(c, "k_return_sinks");
         if (rc != PM_OK) return rc;
+        tick(c, PM_K_RETURN, 1);
     }
     c->stage = ST_IDLE;
     return PM_OK;
@@ -855,4 +885,63 @@ extern "C" int pm_debug_stencil(pm_ctx *c, int kind, double x, double y, double 
     cudaFree(d_ijk);
     *side = 2 * g + 1;
     return rc;
+}
+
+// ---- measurement helpers ---------------------------------------------------------------------------------------------
+extern "C" int pm_kernel_times(pm_ctx *c, float *ms, int32_t n) {
+    if (!c || !ms || n < PM_NUM_KERNELS) return PM_EINVAL;
+    if (!c->timing) PM_FAIL(c, PM_EINVAL, "pm_kernel_times needs PM_FLAG_TIMING");
+    PM_CUDA(c, cudaSetDevice(c->device));
+    PM_CUDA(c, cudaStreamSynchronize(c->stream));
+    for (int k = 0; k < PM_NUM_KERNELS; ++k) {
+        ms[k] = 0.0f;
+        if (c->ev_used[k]) PM_CUDA(c, cudaEventElapsedTime(&ms[k], c->ev[k][0], c->ev[k][1]));
+    }
+    return PM_OK;
+}
+
+// fp64 RED throughput for the deposit's pattern: rows of 7 consecutive doubles (4 rows + 4 idle lanes per warp
+// instruction), the same row position in `channels` planes, pseudo-random row positions over the footprint.
+__device__ __forceinline__ unsigned probe_hash(unsigned x) {
+    x ^= x >> 16; x *= 0x7feb352dU; x ^= x >> 15; x *= 0x846ca68bU; x ^= x >> 16;
+    return x;
+}
+
+__global__ void __launch_bounds__(256) k_probe_red(double *__restrict__ buf, unsigned long long plane, int channels, int iters) {
+    const unsigned tid = blockIdx.x * blockDim.x + threadIdx.x;
+    const unsigned warp = tid >> 5, lane = tid & 31;
+    const unsigned row = lane / 7, col = lane - row * 7;
+    if (row >= 4) return;
+    const unsigned long long nrow = plane / 8;
+    for (int it = 0; it < iters; ++it) {
+        const unsigned long long r = probe_hash((warp * 4 + row) * 977u + it * 0x9e3779b9u) % nrow;
+        double *p = buf + r * 8 + col + (probe_hash(warp + it) & 1);
+        for (int f = 0; f < channels; ++f) atomicAdd(p + f * plane, 1.0);
+    }
+}
+
+extern "C" int pm_probe_red_f64(pm_ctx *c, int64_t footprint_bytes, int32_t channels, double *gops) {
+    if (!c || !gops || channels < 1 || channels > 8 || footprint_bytes < (int64_t)channels * 4096) return PM_EINVAL;
+    PM_CUDA(c, cudaSetDevice(c->device));
+    const unsigned long long plane = ((unsigned long long)footprint_bytes / 8 / channels) & ~7ull;
+    double *buf = nullptr;
+    cudaError_t e = cudaMalloc(&buf, (plane * channels + 16) * sizeof(double));
+    if (e != cudaSuccess) { cudaGetLastError(); PM_FAIL(c, PM_ENOMEM, "pm_probe_red_f64: cudaMalloc failed: %s", cudaGetErrorString(e)); }
+    cudaEvent_t a, b;
+    cudaEventCreate(&a); cudaEventCreate(&b);
+    const int blocks = c->sm_count * 16, iters = 64;
+    cudaMemsetAsync(buf, 0, (plane * channels + 16) * sizeof(double), c->stream);
+    k_probe_red<<<blocks, 256, 0, c->stream>>>(buf, plane, channels, iters);        // warm-up
+    cudaEventRecord(a, c->stream);
+    k_probe_red<<<blocks, 256, 0, c->stream>>>(buf, plane, channels, iters);
+    cudaEventRecord(b, c->stream);
+    e = cudaStreamSynchronize(c->stream);
+    float ms = 0.0f;
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, a, b);
+    cudaEventDestroy(a); cudaEventDestroy(b);
+    cudaFree(buf);
+    if (e != cudaSuccess) { snprintf(c->msg, sizeof(c->msg), "pm_probe_red_f64: %s", cudaGetErrorString(e)); return PM_ECUDA; }
+    const double ops = (double)blocks * 8 * 28 * iters * channels;      // 8 warps per CTA, 28 active lanes
+    *gops = ops / (ms * 1e-3) / 1e9;
+    return PM_OK;
 }

@@ -1,0 +1,58 @@
+"""Host-side logic of bench.py on CPU: the whole-job aggregate and the max-over-ranks rule with world_size 2 (gloo).
+The path itself does not shard ("replicas only"), so the only multi-rank logic is this aggregation."""
+import os
+import socket
+import sys
+
+import pytest
+import torch
+import torch.distributed as dist
+import torch.multiprocessing as mp
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+import bench  # noqa: E402
+
+
+def _free_port():
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+def _worker(rank, world, port, out):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        ms = 10.0 + 5.0 * rank                      # rank 1 is the slow replica
+        total = bench.reduce_max(ms, world, torch.device("cpu"))
+        out[rank] = (total, bench.whole_job_value(1000, 4, world, total))
+    finally:
+        dist.destroy_process_group()
+
+
+def test_replicas_max_over_ranks_gloo_world2():
+    world, port = 2, _free_port()
+    with mp.Manager() as m:
+        out = m.dict()
+        mp.spawn(_worker, args=(world, port, out), nprocs=world, join=True)
+        res = dict(out)
+    assert res[0][0] == res[1][0] == 15.0                       # the max, on every rank
+    assert res[0][1] == pytest.approx(2 * 1000 * 4 / 15e-3 / 1e6)   # units of BOTH replicas over the slowest rank's time
+
+
+def test_single_rank_is_identity():
+    assert bench.reduce_max(3.25, 1, None) == 3.25
+    assert bench.whole_job_value(512 ** 3, 10, 1, 116.0) == pytest.approx(512 ** 3 * 10 / 0.116 / 1e6)
+
+
+def test_algorithmic_bytes_dense_limits():
+    """With every sector touched the per-kernel figures reduce to SURVEY.md 8(d): apply 176 B/cell, zero 48 B per buffer cell."""
+    N, Nb = 512 ** 3, 520 ** 3
+    b = bench.algorithmic_bytes(N, Nb, 10 ** 5, 9 * 10 ** 5, 1.0, 1.0, 1.0)
+    assert b["apply"] == 176.0 * N
+    assert b["zero"] == 48.0 * Nb
+    assert b["fold"] == 3 * 48.0 * (Nb - N)
+    b0 = bench.algorithmic_bytes(N, Nb, 0, 0, 0.0, 0.0, 0.0)
+    assert b0["apply"] == 48.0 * N and b0["sne"] == 0.0 and b0["sinks"] == 0.0

@@ -336,3 +336,25 @@ def test_step_host_matches_device_path():
     assert np.allclose(g.sinks.m.cpu().numpy(), hk.m, rtol=1e-12)
     assert np.allclose(g.sinks.dm.cpu().numpy(), hk.dm, rtol=1e-12)
     assert ctx.pm_launch_count() == 10
+
+
+def test_kernel_times_and_red_probe():
+    """pm_kernel_times (PM_FLAG_TIMING) reports every group that ran; pm_probe_red_f64 returns a positive rate."""
+    w = inputs.scaled_mixed(48, 1200, seed_index=5)
+    dev = torch.device("cuda:0")
+    ctx = pm.Context(w.params, device="cuda:0", flags=pm.PM_FLAG_TIMING)
+    st = pm.DeviceState.from_host(w.state, dev)
+    sk = pm.DeviceSinks.from_host(w.sinks, dev)
+    sn = pm.DeviceSNe.from_host(w.sne, dev)
+    ctx.step(st, sk, sn, w.dt)
+    ms = ctx.pm_kernel_times()
+    assert set(ms) == set(pm.KERNEL_GROUPS)
+    assert all(v > 0.0 for v in ms.values()), ms
+    ctx.pm_deposit(st, None, sn, w.dt)            # no sinks: that group reports 0
+    ctx.pm_fold_ghosts(); ctx.pm_apply_limited(st); ctx.pm_return_to_particles(None)
+    ms = ctx.pm_kernel_times()
+    assert ms["sinks"] == 0.0 and ms["return"] == 0.0 and ms["sne"] > 0.0
+    assert ctx.pm_probe_red_f64(8 << 20, 5) > 1.0
+    plain = pm.Context(w.params, device="cuda:0")
+    with pytest.raises(pm.PmError):
+        plain.pm_kernel_times()
