@@ -557,8 +557,9 @@ extern "C" int pm_create(const pm_params *prm, int device, void *cuda_stream, pm
     P.msf_c = prm->sn_msf_coeff; P.msf_e = prm->sn_msf_exp; P.psnr_c = prm->sn_psnr_coeff; P.psnr_e = prm->sn_psnr_exp;
     P.mu_h = prm->sn_mu_h; P.nh_unit = prm->sn_nh_unit; P.theta = prm->sn_eint_theta;
     P.nsub3 = (double)P.nsub * (double)P.nsub * (double)P.nsub;
-    P.nsbx = (((prm->nx + 7) >> 3) + 3) >> 2; P.nsby = (((prm->ny + 7) >> 3) + 3) >> 2; P.nsbz = (((prm->nz + 7) >> 3) + 3) >> 2;
-    P.ntile = P.nsbx * P.nsby * P.nsbz * 64;
+    const int sbm = (1 << kSbLog2) - 1;
+    P.nsbx = (((prm->nx + 7) >> 3) + sbm) >> kSbLog2; P.nsby = (((prm->ny + 7) >> 3) + sbm) >> kSbLog2; P.nsbz = (((prm->nz + 7) >> 3) + sbm) >> kSbLog2;
+    P.ntile = (P.nsbx * P.nsby * P.nsbz) << (3 * kSbLog2);
 
     cudaError_t e = cudaSetDevice(device);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, device);

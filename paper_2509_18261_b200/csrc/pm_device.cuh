@@ -12,6 +12,7 @@ namespace pm {
 
 constexpr int kBufChannels = 6;      // 0: accretion d rho (signed, R1/R29); 1..5: SN d rho, d p (3), d E
 constexpr int kRetWords = 4;         // eta, v_old (3)
+constexpr int kSbLog2 = 2;           // a super-block is (2^kSbLog2)^3 tiles of 8^3 cells (1..6 measured: no difference)
 constexpr double kFourPi = 12.566370614359172953850573533118;
 
 struct DevP {
@@ -29,7 +30,7 @@ struct DevP {
     double eps_k, rm_ej, rm_mc, msf_c, msf_e, psnr_c, psnr_e, mu_h, nh_unit, theta;
     double nsub3;
     int nsbx, nsby, nsbz;   // super-blocks (4x4x4 tiles of 8^3 cells) per axis: the bins particles are ordered by
-    int ntile;              // nsbx*nsby*nsbz*64 bin keys per particle kind
+    int ntile;              // bin keys per particle kind: super-blocks x tiles per super-block
 };
 
 struct DevState { double *rho, *mx, *my, *mz, *etot, *eint; };
@@ -74,10 +75,14 @@ __device__ __forceinline__ long long ghost_index(const DevP &P, int i, int j, in
 // the buffer and state sectors a particle touches are still in L2 from its neighbours.
 __device__ __forceinline__ int bin_key(const DevP &P, int ih, int jh, int kh) {
     const int tx = ih >> 3, ty = jh >> 3, tz = kh >> 3;
-    const int sb = ((tz >> 2) * P.nsby + (ty >> 2)) * P.nsbx + (tx >> 2);
-    const int lx = tx & 3, ly = ty & 3, lz = tz & 3;
-    const int local = (lx & 1) | ((ly & 1) << 1) | ((lz & 1) << 2) | ((lx & 2) << 2) | ((ly & 2) << 3) | ((lz & 2) << 4);
-    return sb * 64 + local;
+    const int sb = ((tz >> kSbLog2) * P.nsby + (ty >> kSbLog2)) * P.nsbx + (tx >> kSbLog2);
+    const int m = (1 << kSbLog2) - 1;
+    const int lx = tx & m, ly = ty & m, lz = tz & m;
+    int local = 0;
+#pragma unroll
+    for (int bit = 0; bit < kSbLog2; ++bit)
+        local |= (((lx >> bit) & 1) << (3 * bit)) | (((ly >> bit) & 1) << (3 * bit + 1)) | (((lz >> bit) & 1) << (3 * bit + 2));
+    return (sb << (3 * kSbLog2)) + local;
 }
 
 __device__ __forceinline__ double sound_speed(const DevP &P, double rho, double eint) {
