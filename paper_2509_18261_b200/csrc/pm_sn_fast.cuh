@@ -36,22 +36,18 @@ __device__ __forceinline__ unsigned lanemask_lt() {
 
 __device__ __forceinline__ double pick3(int ax, double a, double b, double c) { return ax == 0 ? a : (ax == 1 ? b : c); }
 
-// One warp per SN particle, particles taken in bin order (perm).
-__global__ void __launch_bounds__(kFastSnWarps * 32, 3) k_deposit_sne_g3n4(const DevP P, const DevState U, const DevSNe S,
-                                                                            double *__restrict__ buf, double *__restrict__ dbg,
-                                                                            int *__restrict__ err, const int *__restrict__ perm) {
-    __shared__ SnWarpSmem sm_all[kFastSnWarps];
-    __shared__ unsigned short dec[352];          // linear box index -> packed code, shared by the CTA
+// The whole deposit of ONE supernova by one warp (all 32 lanes must call).  s = particle index; sm = this warp's shared
+// scratch; dec = the CTA's linear-box-index -> packed-code table (sn_fill_dec).
+__device__ __forceinline__ void sn_fill_dec(unsigned short *dec) {
     for (int c = threadIdx.x; c < kSnCells; c += blockDim.x) {
         const int a = c % 7, t = c / 7;
         dec[c] = (unsigned short)(a | ((t % 7) << 3) | ((t / 7) << 6));
     }
-    __syncthreads();
-    const int wib = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const long long w = (long long)blockIdx.x * kFastSnWarps + wib;
-    if (w >= S.n) return;
-    SnWarpSmem &sm = sm_all[wib];
-    const long long s = perm[w];
+}
+
+__device__ __forceinline__ void sn_deposit_one(const DevP &P, const DevState &U, const DevSNe &S, double *__restrict__ buf,
+                                               double *__restrict__ dbg, int *__restrict__ err, const long long s,
+                                               SnWarpSmem &sm, const unsigned short *dec, const int lane) {
     const double xs = S.x[s], ys = S.y[s], zs = S.z[s];
     const int ih = host_cell(xs, P.x0[0], P.inv_dx), jh = host_cell(ys, P.x0[1], P.inv_dx), kh = host_cell(zs, P.x0[2], P.inv_dx);
     if (ih < 0 || ih >= P.nx || jh < 0 || jh >= P.ny || kh < 0 || kh >= P.nz) {
@@ -197,6 +193,20 @@ __global__ void __launch_bounds__(kFastSnWarps * 32, 3) k_deposit_sne_g3n4(const
         dbg[s] = sc.m_snr; dbg[n + s] = sc.v_snr; dbg[2 * n + s] = sc.vcx; dbg[3 * n + s] = sc.vcy; dbg[4 * n + s] = sc.vcz;
         dbg[5 * n + s] = sc.n_h; dbg[6 * n + s] = sc.r_m; dbg[7 * n + s] = sc.p_rad; dbg[8 * n + s] = (double)sc.regime;
     }
+}
+
+// One warp per SN particle, particles taken in bin order (perm).
+__global__ void __launch_bounds__(kFastSnWarps * 32, 3) k_deposit_sne_g3n4(const DevP P, const DevState U, const DevSNe S,
+                                                                            double *__restrict__ buf, double *__restrict__ dbg,
+                                                                            int *__restrict__ err, const int *__restrict__ perm) {
+    __shared__ SnWarpSmem sm_all[kFastSnWarps];
+    __shared__ unsigned short dec[352];          // linear box index -> packed code, shared by the CTA
+    sn_fill_dec(dec);
+    __syncthreads();
+    const int wib = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const long long w = (long long)blockIdx.x * kFastSnWarps + wib;
+    if (w >= S.n) return;
+    sn_deposit_one(P, U, S, buf, dbg, err, perm[w], sm_all[wib], dec, lane);
 }
 
 }  // namespace pm

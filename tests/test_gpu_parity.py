@@ -358,3 +358,11 @@ def test_kernel_times_and_red_probe():
     plain = pm.Context(w.params, device="cuda:0")
     with pytest.raises(pm.PmError):
         plain.pm_kernel_times()
+
+
+@pytest.mark.parametrize("n,npart", [(72, 3000), (130, 6000)])
+def test_mixed_ragged_grids_clustered(n, npart):
+    """Grid sizes that are no multiple of the 8-cell tile or the 64-cell super-block, few dense clusters (heavy stencil overlap)."""
+    w = inputs.scaled_mixed(n, npart, seed_index=5, n_clusters=3)
+    g, o, _ = parity.run_and_compare(w, steps=1)
+    g.ctx.close()
