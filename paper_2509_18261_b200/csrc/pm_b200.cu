@@ -692,7 +692,7 @@ extern "C" int pm_deposit(pm_ctx *c, const pm_state *st, const pm_sinks *sk, con
         const size_t smem = kSnWarps * sn_table_bytes(2 * P.gn + 1, P.nsub);
         tick(c, PM_K_SNE, 0);
         if (P.gn == 3 && P.nsub == 4 && !c->force_generic)
-            k_deposit_sne_g3n4<<<blocks, kFastSnWarps * 32, 0, c->stream>>>(P, U, S, c->buf, dbg ? c->dbg_sn : nullptr, c->err_flag, perm + nk);
+            k_deposit_sne_g3n4<<<(unsigned)((nn + kFastSnWarps - 1) / kFastSnWarps), kFastSnWarps * 32, 0, c->stream>>>(P, U, S, c->buf, dbg ? c->dbg_sn : nullptr, c->err_flag, perm + nk);
         else
             k_deposit_sne<<<blocks, kSnWarps * 32, smem, c->stream>>>(P, U, S, c->buf, dbg ? c->dbg_sn : nullptr, c->err_flag, perm + nk);
         if ((rc = check_launch(c, "k_deposit_sne")) != PM_OK) return rc;

@@ -4,8 +4,9 @@
 //   * box sizes are compile-time, so index decoding is multiply-shift instead of runtime division;
 //   * cells are first classified, then COMPACTED with warp ballots, so the expensive work (64 sub-sample tests of a
 //     boundary cell; gather / scatter of a cell with omega > 0) runs on full warps instead of diverged ones;
-//   * 1/rho and 1/r are formed once per cell and multiplied (<= 1 ulp from the oracle's divisions, far inside the
-//     1e-12 parity tolerance; no integer depends on them).
+//   * no division per cell: P_gas = sum (omega V) m and omega rho (v_COM - v) = omega (rho v_COM - m); rhat = d * rsqrt(r^2);
+//     value arithmetic uses explicit fma() (a few ulp from the oracle's forms, far inside the parity tolerances; no
+//     integer depends on it).
 // One fused kernel on purpose: its arithmetic phases (tables, classification, sub-sample tests) and its memory phases
 // (gather, fp64 RED scatter) belong to different warps at any moment and overlap on the SM.  A split into a geometry
 // kernel and a gather/scatter kernel was measured slower.
@@ -14,7 +15,10 @@
 
 namespace pm {
 
-constexpr int kFastSnWarps = 8;
+// 4 warps per CTA, 8 CTAs per SM (64 registers, no spills): the kernel is latency-bound, and 32 resident warps measured
+// 4.57 ms against 5.40 ms for 8 warps x 3 CTAs (74 registers); 36 and 40 warps need spills and are no faster.
+constexpr int kFastSnWarps = 4;
+constexpr int kFastSnMinBlocks = 8;
 constexpr int kSnB = 7, kSnCells = 343, kSnNs = 4;
 
 // Box cell (a, b, c) = (x, y, z offsets in 0..6) packed as a | b << 3 | c << 6 (< 448).
@@ -143,27 +147,28 @@ __device__ __forceinline__ void sn_deposit_one(const DevP &P, const DevState &U,
     __syncwarp();
     // ---- phase 4: stencil sums (O4) --------------------------------------------------------------------------------
     const double vsx = S.vx[s], vsy = S.vy[s], vsz = S.vz[s], e_sn = S.e_sn[s], m_ej = S.m_ej[s];
+    const double v64 = P.V * (1.0 / 64.0);
     double m_gas = 0.0, px = 0.0, py = 0.0, pz = 0.0, v_snr = 0.0;
 #pragma unroll 1
     for (int idx = lane; idx < na; idx += 32) {
         const int pc = sm.list[idx];
         const int a = pc & 7, b = (pc >> 3) & 7, cc = pc >> 6;
-        const double omega = (double)sm.cnt[pc] * (1.0 / 64.0);         // exact: power of two
+        const double wv = (double)sm.cnt[pc] * v64;                      // omega V; omega = count / 64 is exact
         const int q = sm.off[2][cc] + sm.off[1][b] + sm.off[0][a];
         const double rho = U.rho[q], mx = U.mx[q], my = U.my[q], mz = U.mz[q];
-        const double rinv = 1.0 / rho;
-        const double mcell = omega * rho * P.V;
-        m_gas += mcell;
-        px += mcell * (mx * rinv);
-        py += mcell * (my * rinv);
-        pz += mcell * (mz * rinv);
-        v_snr += omega * P.V;
+        m_gas = fma(wv, rho, m_gas);                                     // P_gas = sum (omega V) m: no division by rho
+        px = fma(wv, mx, px);
+        py = fma(wv, my, py);
+        pz = fma(wv, mz, pz);
+        v_snr += wv;
     }
     m_gas = warp_sum(m_gas); px = warp_sum(px); py = warp_sum(py); pz = warp_sum(pz); v_snr = warp_sum(v_snr);
     const SnScalars sc = sn_scalars(P, m_gas, px, py, pz, v_snr, vsx, vsy, vsz, e_sn, m_ej);
     // ---- phase 5: Eq. 17 and the atomic additions (O5) -----------------------------------------------------------
     const double inv_vsnr = 1.0 / sc.v_snr;
-    const double e_dens = (e_sn + sc.e_kin);
+    const double k_rho = m_ej * inv_vsnr;                 // d rho = omega M_ej / V_snr
+    const double k_e = (e_sn + sc.e_kin) * inv_vsnr;     // (E_sn + E_kin) / V_snr per unit omega
+    const double k_p = sc.p_rad * inv_vsnr;
     double *const sbuf = buf + P.Nb + (ih - 3 + P.gx);
 #pragma unroll 1
     for (int idx = lane; idx < na; idx += 32) {
@@ -172,21 +177,19 @@ __device__ __forceinline__ void sn_deposit_one(const DevP &P, const DevState &U,
         const double omega = (double)sm.cnt[pc] * (1.0 / 64.0);
         const int q = sm.off[2][cc] + sm.off[1][b] + sm.off[0][a];
         const double rho = U.rho[q], mx = U.mx[q], my = U.my[q], mz = U.mz[q];
-        const double rinv = 1.0 / rho;
-        const double vx = mx * rinv, vy = my * rinv, vz = mz * rinv;
         const double ddx = sm.dc[0][a], ddy = sm.dc[1][b], ddz = sm.dc[2][cc];
         const double r2 = dist2(ddx, ddy, ddz);
         const double ir = r2 > 0.0 ? rsqrt(r2) : 0.0;                  // rhat = 0 at r = 0 (R21)
-        const double drho = omega * m_ej * inv_vsnr;
-        const double pscale = (sc.p_rad * inv_vsnr) * omega * ir;
+        const double drho = omega * k_rho;
+        const double pscale = (k_p * omega) * ir;
         const double prx = pscale * ddx, pry = pscale * ddy, prz = pscale * ddz;
-        const double wr = omega * rho;
         double *dst = sbuf + (sm.goff[1][cc] + sm.goff[0][b] + a);
+        // omega rho (v_COM - v) = omega (rho v_COM - m): no division by rho
         atomicAdd(dst, drho);
-        atomicAdd(dst + P.Nb, wr * (sc.vcx - vx) + drho * sc.vcx + prx);
-        atomicAdd(dst + 2 * P.Nb, wr * (sc.vcy - vy) + drho * sc.vcy + pry);
-        atomicAdd(dst + 3 * P.Nb, wr * (sc.vcz - vz) + drho * sc.vcz + prz);
-        atomicAdd(dst + 4 * P.Nb, omega * e_dens * inv_vsnr + ((sc.vcx * prx + sc.vcy * pry) + sc.vcz * prz));
+        atomicAdd(dst + P.Nb, fma(omega, fma(rho, sc.vcx, -mx), fma(drho, sc.vcx, prx)));
+        atomicAdd(dst + 2 * P.Nb, fma(omega, fma(rho, sc.vcy, -my), fma(drho, sc.vcy, pry)));
+        atomicAdd(dst + 3 * P.Nb, fma(omega, fma(rho, sc.vcz, -mz), fma(drho, sc.vcz, prz)));
+        atomicAdd(dst + 4 * P.Nb, fma(omega, k_e, fma(sc.vcx, prx, fma(sc.vcy, pry, sc.vcz * prz))));
     }
     if (dbg && lane == 0) {
         const long long n = S.n;
@@ -196,7 +199,7 @@ __device__ __forceinline__ void sn_deposit_one(const DevP &P, const DevState &U,
 }
 
 // One warp per SN particle, particles taken in bin order (perm).
-__global__ void __launch_bounds__(kFastSnWarps * 32, 3) k_deposit_sne_g3n4(const DevP P, const DevState U, const DevSNe S,
+__global__ void __launch_bounds__(kFastSnWarps * 32, kFastSnMinBlocks) k_deposit_sne_g3n4(const DevP P, const DevState U, const DevSNe S,
                                                                             double *__restrict__ buf, double *__restrict__ dbg,
                                                                             int *__restrict__ err, const int *__restrict__ perm) {
     __shared__ SnWarpSmem sm_all[kFastSnWarps];
