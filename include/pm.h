@@ -153,7 +153,8 @@ int pm_probe_red_f64(pm_ctx *ctx, int64_t footprint_bytes, int32_t channels, dou
  * *ghost = g. */
 int pm_debug_buffer(pm_ctx *ctx, int channel, const double **dev_ptr, int64_t dims[3], int64_t *origin, int32_t *ghost);
 
-/* Return mesh word 0 = eta (Eq. 4), 1..3 = pre-step cell velocity; nx*ny*nz each, valid where buffer channel 0 != 0. */
+/* Return mesh: one record of 4 doubles per cell (eta of Eq. 4, pre-step velocity x, y, z), valid where buffer channel
+ * 0 != 0.  *dev_ptr points at word `word` of cell 0; the same word of cell q is at dev_ptr[4 q]. */
 int pm_debug_return_mesh(pm_ctx *ctx, int word, const double **dev_ptr);
 
 /* lambda of Eq. 21 per cell (needs PM_FLAG_DEBUG_LAMBDA). */

@@ -34,7 +34,7 @@ struct pm_ctx {
     int sm_count;
     cudaStream_t stream;
     double *buf;        // kBufChannels * Nb
-    double *ret;        // kRetWords * N (NULL when rk_sink == 0)
+    double *ret;        // N records of kRetWords doubles (eta, v_old x/y/z): one 32-byte sector per cell (NULL when rk_sink == 0)
     double *lam;        // N (debug only)
     double *sink_scal;  // 3 * cap_sinks: mdot, r_acc, sum w
     long long cap_sinks;
@@ -442,10 +442,9 @@ __global__ void __launch_bounds__(256, 3) k_apply_limited(const DevP P, const De
 #pragma unroll
         for (int f = 0; f < 6; ++f) u[f][v] = uc[f];
         if (bc[0] != 0.0 && ret) {              // Step 4 needs eta and the pre-step velocity where a sink removed mass
-            ret[q + v] = eta;
-            ret[P.N + q + v] = vold[0];
-            ret[2 * P.N + q + v] = vold[1];
-            ret[3 * P.N + q + v] = vold[2];
+            double2 *r = reinterpret_cast<double2 *>(ret + 4 * (q + v));      // one whole 32-byte sector per cell
+            r[0] = make_double2(eta, vold[0]);
+            r[1] = make_double2(vold[1], vold[2]);
         }
     }
     if (!any) return;                           // lanes of a touched segment whose own cells are untouched
@@ -479,11 +478,12 @@ __global__ void __launch_bounds__(128) k_return_sinks(const DevP P, const DevSin
             const double amt = sink_cell_amount(P, r2, r_acc, wsum, mdot, dt);
             if (amt > 0.0) {                     // amt == 0 deposits nothing, so the return mesh has no entry there
                 const long long q = owned_index(P, i, j, k);
-                const double gain = ret[q] * amt * P.V;
+                const double2 r0 = reinterpret_cast<const double2 *>(ret + 4 * q)[0], r1 = reinterpret_cast<const double2 *>(ret + 4 * q)[1];
+                const double gain = r0.x * amt * P.V;
                 dm += gain;
-                dpx += gain * ret[P.N + q];
-                dpy += gain * ret[2 * P.N + q];
-                dpz += gain * ret[3 * P.N + q];
+                dpx += gain * r0.y;
+                dpy += gain * r1.x;
+                dpz += gain * r1.y;
             }
         }
     }
@@ -846,7 +846,7 @@ extern "C" int pm_debug_buffer(pm_ctx *c, int channel, const double **dev_ptr, i
 
 extern "C" int pm_debug_return_mesh(pm_ctx *c, int word, const double **dev_ptr) {
     if (!c || !dev_ptr || word < 0 || word >= kRetWords || !c->ret) return PM_EINVAL;
-    *dev_ptr = c->ret + (long long)word * c->P.N;
+    *dev_ptr = c->ret + word;          // record of cell q at 4 q: stride kRetWords between cells
     return PM_OK;
 }
 

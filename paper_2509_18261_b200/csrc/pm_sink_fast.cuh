@@ -1,7 +1,7 @@
 // pm_sink_fast.cuh -- specialised sink deposit (a1-a3) and return (a8) kernels for kernel half-width 4 (9^3 box),
 // the shape every BASELINE config uses.  Membership is the same bit-exact test as the generic kernels,
 // (dz^2 + dy^2) + dx^2 <= r_K^2 on cell-centre offsets, but evaluated by ROW (81 rows of 9 cells, one row per lane,
-// squared offsets tabulated per axis); members are compacted into a list that carries the owned and ghosted indices.
+// squared offsets tabulated per axis); members are compacted into a list of packed (a, b, c) codes.
 // The Gaussian weight is separable, exp(-r^2/r_acc^2) = e_z e_y e_x, so a sink costs 27 exponentials instead of one
 // per member cell per pass (the product differs from the oracle's single exp by a few ulp plus the same
 // conditioning term r^2/r_acc^2 * eps both carry).  No division per cell:
@@ -12,6 +12,7 @@
 namespace pm {
 
 constexpr int kFastSinkWarps = 4;
+constexpr int kFastSinkMinBlocks = 10;   // 48 registers, 40 warps per SM (1 / 10 / 12 / 16 measured: 0.66 / 0.53 / 0.56 / 0.61 ms)
 constexpr int kSkB = 9, kSkRows = 81, kSkMaxMembers = 512;   // members lie within r_K + sqrt(3)/2 cells: < 484
 
 struct __align__(16) SinkWarpSmem {
@@ -19,7 +20,6 @@ struct __align__(16) SinkWarpSmem {
     double ex[3][10];                  // exp(-d2 / r_acc^2) per axis
     int off[3][10];                    // wrapped owned-index contribution per axis
     int goff[2][10];                   // ghosted-index contribution of y and z
-    int2 idx[kSkMaxMembers];           // member list: (owned index, ghosted index relative to the box-origin row)
     unsigned short code[kSkMaxMembers];  // a | b << 4 | c << 8
 };
 
@@ -69,12 +69,10 @@ __device__ __forceinline__ int sink_member_list_g4(const DevP &P, SinkWarpSmem &
         const int r = lane + 32 * t;
         if (mask[t]) {
             const int b = r % 9, c = r / 9;
-            const int qrow = sm.off[2][c] + sm.off[1][b], grow = sm.goff[1][c] + sm.goff[0][b];
             const int crow = (b << 4) | (c << 8);
 #pragma unroll
             for (int a = 0; a < 9; ++a)
                 if (mask[t] >> a & 1) {
-                    sm.idx[pos] = make_int2(qrow + sm.off[0][a], grow + a);
                     sm.code[pos] = (unsigned short)(crow | a);
                     ++pos;
                 }
@@ -94,11 +92,18 @@ __device__ __forceinline__ void sink_axis_weights(SinkWarpSmem &sm, int lane, do
     __syncwarp();
 }
 
+__device__ __forceinline__ int sink_owned(const SinkWarpSmem &sm, int code) {
+    return sm.off[2][code >> 8] + sm.off[1][(code >> 4) & 15] + sm.off[0][code & 15];
+}
+__device__ __forceinline__ int sink_ghosted(const SinkWarpSmem &sm, int code) {
+    return sm.goff[1][code >> 8] + sm.goff[0][(code >> 4) & 15] + (code & 15);
+}
+
 __device__ __forceinline__ double sink_weight(const SinkWarpSmem &sm, int code) {
     return (sm.ex[2][code >> 8] * sm.ex[1][(code >> 4) & 15]) * sm.ex[0][code & 15];
 }
 
-__global__ void __launch_bounds__(kFastSinkWarps * 32) k_deposit_sinks_g4(const DevP P, const DevState U, const DevSinks S,
+__global__ void __launch_bounds__(kFastSinkWarps * 32, kFastSinkMinBlocks) k_deposit_sinks_g4(const DevP P, const DevState U, const DevSinks S,
                                                                           const double dt, double *__restrict__ buf0,
                                                                           double *__restrict__ scal, double *__restrict__ dbg,
                                                                           int *__restrict__ err, const int *__restrict__ perm) {
@@ -121,7 +126,7 @@ __global__ void __launch_bounds__(kFastSinkWarps * 32) k_deposit_sinks_g4(const 
     double sum_rho = 0.0, srx = 0.0, sry = 0.0, srz = 0.0, src = 0.0;
 #pragma unroll 2
     for (int i = lane; i < nm; i += 32) {
-        const int q = sm.idx[i].x;
+        const int q = sink_owned(sm, sm.code[i]);
         const double rho = U.rho[q], mx = U.mx[q], my = U.my[q], mz = U.mz[q];
         sum_rho += rho;
         srx += fma(-rho, vsx, mx);                 // rho (v - v_s) = m - rho v_s
@@ -139,7 +144,10 @@ __global__ void __launch_bounds__(kFastSinkWarps * 32) k_deposit_sinks_g4(const 
     wsum = warp_sum(wsum);
     const double k = sc.mdot * dt / (wsum * P.V);         // a = mdot (w / sum w) dt / V
     double *const sbuf = buf0 + (ih - 4 + P.gx);
-    for (int i = lane; i < nm; i += 32) atomicAdd(sbuf + sm.idx[i].y, -(sink_weight(sm, sm.code[i]) * k));   // R1: signed
+    for (int i = lane; i < nm; i += 32) {
+        const int code = sm.code[i];
+        atomicAdd(sbuf + sink_ghosted(sm, code), -(sink_weight(sm, code) * k));   // R1: signed
+    }
     if (lane == 0) {
         scal[s] = sc.mdot; scal[S.n + s] = sc.r_acc; scal[2 * S.n + s] = wsum;
         if (dbg) {
@@ -150,7 +158,7 @@ __global__ void __launch_bounds__(kFastSinkWarps * 32) k_deposit_sinks_g4(const 
     }
 }
 
-__global__ void __launch_bounds__(kFastSinkWarps * 32) k_return_sinks_g4(const DevP P, const DevSinks S, const double dt,
+__global__ void __launch_bounds__(kFastSinkWarps * 32, kFastSinkMinBlocks) k_return_sinks_g4(const DevP P, const DevSinks S, const double dt,
                                                                          const double *__restrict__ scal,
                                                                          const double *__restrict__ ret,
                                                                          const int *__restrict__ perm) {
@@ -170,14 +178,17 @@ __global__ void __launch_bounds__(kFastSinkWarps * 32) k_return_sinks_g4(const D
     double dm = 0.0, dpx = 0.0, dpy = 0.0, dpz = 0.0;
 #pragma unroll 2
     for (int i = lane; i < nm; i += 32) {
-        const double wgt = sink_weight(sm, sm.code[i]);
+        const int code = sm.code[i];
+        const double wgt = sink_weight(sm, code);
         if (wgt * kV > 0.0) {                   // a == 0 deposited nothing, so the return mesh has no entry there
-            const int q = sm.idx[i].x;
-            const double gain = ret[q] * (wgt * kV);
+            const int q = sink_owned(sm, code);
+            const double2 *r = reinterpret_cast<const double2 *>(ret + 4 * (long long)q);   // (eta, v_old): one sector
+            const double2 r0 = r[0], r1 = r[1];
+            const double gain = r0.x * (wgt * kV);
             dm += gain;
-            dpx = fma(gain, ret[P.N + q], dpx);
-            dpy = fma(gain, ret[2 * P.N + q], dpy);
-            dpz = fma(gain, ret[3 * P.N + q], dpz);
+            dpx = fma(gain, r0.y, dpx);
+            dpy = fma(gain, r1.x, dpy);
+            dpz = fma(gain, r1.y, dpz);
         }
     }
     dm = warp_sum(dm); dpx = warp_sum(dpx); dpy = warp_sum(dpy); dpz = warp_sum(dpz);

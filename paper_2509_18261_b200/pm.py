@@ -320,7 +320,8 @@ class Context:
         ptr = C.c_void_p()
         self._chk(self.L.pm_debug_return_mesh(self.h, word, C.byref(ptr)), "pm_debug_return_mesh")
         nx, ny, nz = self.params["nx"], self.params["ny"], self.params["nz"]
-        return _from_ptr(ptr.value, nx * ny * nz, self.device).view(nz, ny, nx)
+        n = nx * ny * nz
+        return _from_ptr(ptr.value, 4 * n - word, self.device)[::4][:n].view(nz, ny, nx)
 
     def debug_lambda(self):
         ptr = C.c_void_p()
