@@ -19,8 +19,8 @@
 using namespace pm;
 
 // Preferred shared-memory carve-out (% of the 256 KB L1) of the sink kernels: measured on config 5, 25 / 50 / 75 / 100 %
-// give 1.06 / 0.56 / 0.54 / 0.79 ms (deposit) and 0.93 / 0.44 / 0.37 / 0.56 ms (return); the SN kernel is best at the default.
-constexpr int kSinkCarveout = 75;
+// give 0.52 / 0.50 / 0.53 / 0.79 ms (deposit) and 0.22 / 0.20 / 0.20 / 0.27 ms (return); the SN kernel is best at the default.
+constexpr int kSinkCarveout = 50;
 
 // ---------------------------------------------------------------------------------------------------------------
 // context
@@ -365,23 +365,27 @@ __global__ void __launch_bounds__(256) k_fold_ghosts(const DevP P, double *__res
     const int oy = j < g ? ny : (j >= ny - g ? -ny : 0);
     const int oz = k < g ? nz : (k >= nz - g ? -nz : 0);
     const long long base = ghost_index(P, i, j, k);
+    // images m = 4 cz + 2 cy + cx in ascending order (the fixed order z image, y image, x image); all loads of all channels
+    // are issued before any store
+    long long img[8];
+    bool ok[8];
+#pragma unroll
+    for (int m = 1; m < 8; ++m) {
+        const int cx = m & 1, cy = (m >> 1) & 1, cz = m >> 2;
+        ok[m] = (!cx || ox) && (!cy || oy) && (!cz || oz);
+        img[m] = ghost_index(P, i + cx * ox, j + cy * oy, k + cz * oz);
+    }
+    double acc[kBufChannels];
 #pragma unroll
     for (int ch = 0; ch < kBufChannels; ++ch) {
-        double *b = buf + (long long)ch * P.Nb;
-        double acc = b[base];
-        for (int cz = 0; cz < 2; ++cz) {
-            if (cz && !oz) break;
-            for (int cy = 0; cy < 2; ++cy) {
-                if (cy && !oy) break;
-                for (int cx = 0; cx < 2; ++cx) {
-                    if (cx && !ox) break;
-                    if (!(cz | cy | cx)) continue;
-                    acc += b[ghost_index(P, i + cx * ox, j + cy * oy, k + cz * oz)];
-                }
-            }
-        }
-        b[base] = acc;
+        const double *b = buf + (long long)ch * P.Nb;
+        double a = b[base];
+#pragma unroll
+        for (int m = 1; m < 8; ++m) if (ok[m]) a += b[img[m]];
+        acc[ch] = a;
     }
+#pragma unroll
+    for (int ch = 0; ch < kBufChannels; ++ch) buf[(long long)ch * P.Nb + base] = acc[ch];
 }
 
 // ---------------------------------------------------------------------------------------------------------------
