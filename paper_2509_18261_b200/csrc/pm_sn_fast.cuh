@@ -19,6 +19,7 @@ namespace pm {
 // 4.57 ms against 5.40 ms for 8 warps x 3 CTAs (74 registers); 36 and 40 warps need spills and are no faster.
 constexpr int kFastSnWarps = 4;
 constexpr int kFastSnMinBlocks = 8;
+constexpr int kSnGatherBatch = 2;   // list entries per lane whose loads are in flight together (2 / 3 / 6 measured alike)
 constexpr int kSnB = 7, kSnCells = 343, kSnNs = 4;
 
 // Box cell (a, b, c) = (x, y, z offsets in 0..6) packed as a | b << 3 | c << 6 (< 448).
@@ -149,18 +150,31 @@ __device__ __forceinline__ void sn_deposit_one(const DevP &P, const DevState &U,
     const double vsx = S.vx[s], vsy = S.vy[s], vsz = S.vz[s], e_sn = S.e_sn[s], m_ej = S.m_ej[s];
     const double v64 = P.V * (1.0 / 64.0);
     double m_gas = 0.0, px = 0.0, py = 0.0, pz = 0.0, v_snr = 0.0;
+    // batches of kSnGatherBatch list entries per lane: all their loads are in flight together (the gather is latency-bound)
 #pragma unroll 1
-    for (int idx = lane; idx < na; idx += 32) {
-        const int pc = sm.list[idx];
-        const int a = pc & 7, b = (pc >> 3) & 7, cc = pc >> 6;
-        const double wv = (double)sm.cnt[pc] * v64;                      // omega V; omega = count / 64 is exact
-        const int q = sm.off[2][cc] + sm.off[1][b] + sm.off[0][a];
-        const double rho = U.rho[q], mx = U.mx[q], my = U.my[q], mz = U.mz[q];
-        m_gas = fma(wv, rho, m_gas);                                     // P_gas = sum (omega V) m: no division by rho
-        px = fma(wv, mx, px);
-        py = fma(wv, my, py);
-        pz = fma(wv, mz, pz);
-        v_snr += wv;
+    for (int base = lane; base < na; base += 32 * kSnGatherBatch) {
+        int q[kSnGatherBatch];
+        double wv[kSnGatherBatch];
+#pragma unroll
+        for (int u = 0; u < kSnGatherBatch; ++u) {
+            const int idx = base + 32 * u;
+            const bool on = idx < na;
+            const int pc = on ? sm.list[idx] : 0;
+            const int a = pc & 7, b = (pc >> 3) & 7, cc = pc >> 6;
+            q[u] = on ? sm.off[2][cc] + sm.off[1][b] + sm.off[0][a] : 0;
+            wv[u] = on ? (double)sm.cnt[pc] * v64 : 0.0;                  // omega V; omega = count / 64 is exact
+        }
+        double rho[kSnGatherBatch], mx[kSnGatherBatch], my[kSnGatherBatch], mz[kSnGatherBatch];
+#pragma unroll
+        for (int u = 0; u < kSnGatherBatch; ++u) { rho[u] = U.rho[q[u]]; mx[u] = U.mx[q[u]]; my[u] = U.my[q[u]]; mz[u] = U.mz[q[u]]; }
+#pragma unroll
+        for (int u = 0; u < kSnGatherBatch; ++u) {
+            m_gas = fma(wv[u], rho[u], m_gas);                           // P_gas = sum (omega V) m: no division by rho
+            px = fma(wv[u], mx[u], px);
+            py = fma(wv[u], my[u], py);
+            pz = fma(wv[u], mz[u], pz);
+            v_snr += wv[u];
+        }
     }
     m_gas = warp_sum(m_gas); px = warp_sum(px); py = warp_sum(py); pz = warp_sum(pz); v_snr = warp_sum(v_snr);
     const SnScalars sc = sn_scalars(P, m_gas, px, py, pz, v_snr, vsx, vsy, vsz, e_sn, m_ej);
