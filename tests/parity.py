@@ -70,8 +70,9 @@ class GpuRun:
 
     def totals(self):
         """(mass, momentum[3]) of gas + sinks, summed on the device in fp64."""
-        mass = float(self.state.rho.sum())
-        mom = [float(f.sum()) for f in (self.state.mx, self.state.my, self.state.mz)]
+        V = float(self.w.params["dx"]) ** 3
+        mass = V * float(self.state.rho.sum())
+        mom = [V * float(f.sum()) for f in (self.state.mx, self.state.my, self.state.mz)]
         if self.sinks is not None:
             mass += float(self.sinks.m.sum())
             mom = [p + float((self.sinks.m * v).sum()) for p, v in

@@ -366,3 +366,33 @@ def test_mixed_ragged_grids_clustered(n, npart):
     w = inputs.scaled_mixed(n, npart, seed_index=5, n_clusters=3)
     g, o, _ = parity.run_and_compare(w, steps=1)
     g.ctx.close()
+
+
+@pytest.mark.parametrize("rk_sink,rk_sn,dx", [(3.3, 2.6, 1.0), (4.0 * 0.37, 3.0 * 0.37, 0.37), (3.01, 2.01, 1.0)])
+def test_fast_kernels_other_radii_and_spacing(rk_sink, rk_sn, dx):
+    """The specialised kernels serve every radius with ceil(r_K / dx) = 4 (sinks) / 3 (SNe), any dx and origin: member masks,
+    omega counts and the separable Gaussian must follow r_K and dx, not the BASELINE values 4 dx / 3 dx."""
+    w = inputs.scaled_mixed(40, 500, seed_index=5)
+    n = 40
+    w.params.update(dx=dx, x0=(-1.3, 2.2, 0.11), rk_sink=rk_sink, rk_sn=rk_sn)
+    for p in (w.sinks, w.sne):                      # positions were drawn in [0, n): map them into the shifted, scaled box
+        p.x[:] = p.x * dx + w.params["x0"][0]; p.y[:] = p.y * dx + w.params["x0"][1]; p.z[:] = p.z * dx + w.params["x0"][2]
+    for p in (w.sinks, w.sne):
+        for arr, o in ((p.x, 0), (p.y, 1), (p.z, 2)):
+            np.clip(arr, w.params["x0"][o], np.nextafter(w.params["x0"][o] + n * dx, -np.inf), out=arr)
+    parity.run_and_compare(w, steps=2)
+
+
+def test_generic_and_fast_kernels_agree_bitwise_on_integers():
+    """Member counts (sinks) and regimes (SNe) from the generic and the specialised kernels are identical."""
+    w = inputs.scaled_mixed(40, 500, seed_index=5)
+    outs = []
+    for flags in (0, pm.PM_FLAG_GENERIC_KERNELS):
+        g = parity.GpuRun(w, flags=pm.PM_FLAG_DEBUG_SCALARS | pm.PM_FLAG_DEBUG_LAMBDA | flags)
+        g.ctx.pm_deposit(g.state, g.sinks, g.sne, w.dt)
+        outs.append((g.ctx.debug_sink_scalars().cpu().numpy()[7].copy(), g.ctx.debug_sn_scalars().cpu().numpy()[8].copy(),
+                     g.ctx.debug_sn_scalars().cpu().numpy()[1].copy()))
+        g.ctx.pm_fold_ghosts(); g.ctx.pm_apply_limited(g.state); g.ctx.pm_return_to_particles(g.sinks); g.ctx.pm_check()
+    assert np.array_equal(outs[0][0], outs[1][0])
+    assert np.array_equal(outs[0][1], outs[1][1])
+    assert np.allclose(outs[0][2], outs[1][2], rtol=1e-13, atol=0)     # V_snr = (sum of omega counts) V / 64
