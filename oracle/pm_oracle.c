@@ -16,6 +16,8 @@
  * It shares no code, header, table or helper with the CUDA path.  No blocking, fusion or reordering:
  * particles are processed in index order, cells in (k, j, i) order, sums are plain left-to-right.
  *
+ * Appendix A rounding (orc_repro_*): pinned by the permutation brute force and the worked 2-term case in tests.
+ *
  * Parity unpinned (defined by DESIGN.md readings only, no independent pin exists):
  *   - rho_inf away from uniform gas (R4: arithmetic mean over member cells);
  *   - the Eq. 21 fall-back branch (R25: no admissible root => lambda = 0, e_int clipped at 0).
@@ -478,6 +480,67 @@ int orc_deposit(const orc_params *p, const orc_state *U, orc_sinks *sk, orc_sne 
     return 0;
 }
 
+/* ------------------------------------------------------------------------------------------ */
+/* Appendix A "Particle to buffer mesh", reading R34 of DESIGN.md.          */
+/* The paper accumulates E := E + eps |dU^buf| after every addition, r = E / |dU^buf|, and     */
+/* clears the N_bit = log2 r + 52 + M least significant mantissa bits.  E as printed depends   */
+/* on the order of the additions; we use the order-independent upper bound                      */
+/*     E <= eps (k - 1) T,   T = sum_s |dU^s|,  k = number of particles that contributed,      */
+/* (every partial sum is <= T in magnitude and the first addition, into zero, is exact), and   */
+/* take log2 as the difference of binary exponents rounded up (integer arithmetic only):       */
+/*     N_bit = ilogb((k - 1) T) - ilogb(|dU^buf|) + 1 + M,  clamped to [0, 52].                 */
+/* k <= 1 or dU^buf == 0: nothing to round.  Clearing bits truncates toward zero.               */
+/* ------------------------------------------------------------------------------------------ */
+int32_t orc_repro_bits(double x, double T, int32_t k, int32_t M) {
+    if (k <= 1 || x == 0.0 || !(T > 0.0)) return 0;
+    int nb = ilogb((double)(k - 1) * T) - ilogb(fabs(x)) + 1 + M;
+    if (nb < 0) nb = 0;
+    if (nb > 52) nb = 52;
+    return nb;
+}
+
+double orc_repro_round(double x, double T, int32_t k, int32_t M) {
+    const int32_t nb = orc_repro_bits(x, T, k, M);
+    if (nb == 0) return x;
+    uint64_t u;
+    memcpy(&u, &x, sizeof(u));
+    u &= ~((((uint64_t)1) << nb) - 1);
+    memcpy(&x, &u, sizeof(u));
+    return x;
+}
+
+/* Round the deposited buffers of one step (after orc_deposit, before orc_apply).  Needs Sabs and both counts.
+ * Accretion group: the terms of A[0] share a sign, so T = |A[0]|; the other five accretion channels are rebuilt from the
+ * rounded A[0] in the rank-one form of R29, A[f] = A[0] U_f / rho, with the PRE-step state U.  SN group: T of d rho and
+ * d E are their own sums of |terms|; the three momentum channels share T = sum_s (|dp_x| + |dp_y| + |dp_z|). */
+int orc_repro_buffers(const orc_params *p, const orc_state *U, orc_mesh_out *mo, int32_t M) {
+    const int64_t N = (int64_t)p->nx * p->ny * p->nz;
+    if (!mo->sn_count || !mo->sink_count) return -1;
+    for (int f = 0; f < 5; ++f) if (!mo->Sabs[f]) return -1;
+    for (int64_t c = 0; c < N; ++c) {
+        const int32_t kk = mo->sink_count[c], kn = mo->sn_count[c];
+        if (kk > 0) {
+            const double a0 = orc_repro_round(mo->A[0][c], fabs(mo->A[0][c]), kk, M);
+            const double rho = U->rho[c];
+            mo->A[0][c] = a0;
+            mo->A[1][c] = a0 * (U->mx[c] / rho);
+            mo->A[2][c] = a0 * (U->my[c] / rho);
+            mo->A[3][c] = a0 * (U->mz[c] / rho);
+            mo->A[4][c] = a0 * (U->etot[c] / rho);
+            mo->A[5][c] = a0 * (U->eint[c] / rho);
+        }
+        if (kn > 0) {
+            const double Tp = (mo->Sabs[1][c] + mo->Sabs[2][c]) + mo->Sabs[3][c];
+            mo->S[0][c] = orc_repro_round(mo->S[0][c], mo->Sabs[0][c], kn, M);
+            mo->S[1][c] = orc_repro_round(mo->S[1][c], Tp, kn, M);
+            mo->S[2][c] = orc_repro_round(mo->S[2][c], Tp, kn, M);
+            mo->S[3][c] = orc_repro_round(mo->S[3][c], Tp, kn, M);
+            mo->S[4][c] = orc_repro_round(mo->S[4][c], mo->Sabs[4][c], kn, M);
+        }
+    }
+    return 0;
+}
+
 /* Steps 3+5 (O7) on every cell, in place; sn_touched[c] != 0 marks cells with an SN contribution. */
 int orc_apply(const orc_params *p, orc_state *U, const orc_mesh_out *mo, const int32_t *sn_touched) {
     const int64_t N = (int64_t)p->nx * p->ny * p->nz;
@@ -561,6 +624,24 @@ int orc_step(const orc_params *p, orc_state *U, orc_sinks *sk, orc_sne *sn, doub
 /* every particle whose kernel can reach it, then apply_cell.  Outputs are arrays of length     */
 /* n_cells: A (6), S (5), Aabs(6), Sabs(5), eta, lam, new state (6), sn_count.                  */
 /* ------------------------------------------------------------------------------------------ */
+/* One step with the Appendix A rounding of the buffers between deposit and apply (M = margin bits). */
+int orc_step_repro(const orc_params *p, orc_state *U, orc_sinks *sk, orc_sne *sn, double dt, orc_mesh_out *mo,
+                   double *scratch_old, int32_t M) {
+    const int64_t N = (int64_t)p->nx * p->ny * p->nz;
+    if (!mo->sn_count || !mo->eta) return -1;
+    orc_state Uo = { scratch_old, scratch_old + N, scratch_old + 2 * N, scratch_old + 3 * N, scratch_old + 4 * N, scratch_old + 5 * N };
+    memcpy(Uo.rho, U->rho, (size_t)N * 8); memcpy(Uo.mx, U->mx, (size_t)N * 8); memcpy(Uo.my, U->my, (size_t)N * 8);
+    memcpy(Uo.mz, U->mz, (size_t)N * 8); memcpy(Uo.etot, U->etot, (size_t)N * 8); memcpy(Uo.eint, U->eint, (size_t)N * 8);
+    int rc = orc_deposit(p, U, sk, sn, dt, mo);
+    if (rc) return rc;
+    rc = orc_repro_buffers(p, U, mo, M);
+    if (rc) return rc;
+    rc = orc_apply(p, U, mo, mo->sn_count);
+    if (rc) return rc;
+    if (sk && sk->n > 0) rc = orc_return(p, &Uo, mo->eta, sk, dt);
+    return rc;
+}
+
 static inline int64_t periodic_delta(int64_t a, int64_t b, int64_t n) {   /* a - b wrapped to [-n/2, n/2) */
     int64_t d = (a - b) % n;
     if (d < -(n / 2)) d += n;

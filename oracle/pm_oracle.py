@@ -97,6 +97,14 @@ def lib():
         L.orc_step.restype = C.c_int
         L.orc_step.argtypes = [C.POINTER(OrcParams), C.POINTER(OrcState), C.POINTER(OrcSinks), C.POINTER(OrcSNe),
                                C.c_double, C.POINTER(OrcMeshOut), c_dp]
+        L.orc_step_repro.restype = C.c_int
+        L.orc_step_repro.argtypes = L.orc_step.argtypes + [C.c_int32]
+        L.orc_repro_bits.restype = C.c_int32
+        L.orc_repro_bits.argtypes = [C.c_double, C.c_double, C.c_int32, C.c_int32]
+        L.orc_repro_round.restype = C.c_double
+        L.orc_repro_round.argtypes = [C.c_double, C.c_double, C.c_int32, C.c_int32]
+        L.orc_repro_buffers.restype = C.c_int
+        L.orc_repro_buffers.argtypes = [C.POINTER(OrcParams), C.POINTER(OrcState), C.POINTER(OrcMeshOut), C.c_int32]
         L.orc_sample_cells.restype = C.c_int
         L.orc_sample_cells.argtypes = [C.POINTER(OrcParams), C.POINTER(OrcState), C.POINTER(OrcSinks), C.POINTER(OrcSNe),
                                        C.c_double, c_lp, C.c_int64, c_dp, c_dp, c_dp, c_dp, c_dp, c_dp, c_dp, c_ip]
@@ -225,12 +233,22 @@ class Oracle:
         rc = self.L.orc_return(C.byref(self.p), C.byref(cs), _dp(self.eta), C.byref(ck), dt)
         assert rc == 0
 
-    def step(self, dt: float):
+    def step(self, dt: float, repro_M=None):
+        """One whole step; repro_M = margin bits M of Appendix A (None: no rounding of the buffers)."""
         if self._old is None:
             self._old = np.empty(6 * self.N)
         cs, ck, cn, cm = self._cstate(), self._csinks(), self._csne(), self._cmesh()
-        rc = self.L.orc_step(C.byref(self.p), C.byref(cs), C.byref(ck), C.byref(cn), dt, C.byref(cm), _dp(self._old))
+        if repro_M is None:
+            rc = self.L.orc_step(C.byref(self.p), C.byref(cs), C.byref(ck), C.byref(cn), dt, C.byref(cm), _dp(self._old))
+        else:
+            rc = self.L.orc_step_repro(C.byref(self.p), C.byref(cs), C.byref(ck), C.byref(cn), dt, C.byref(cm), _dp(self._old), int(repro_M))
         assert rc == 0, f"orc_step rc={rc}"
+
+    def repro_buffers(self, M: int):
+        """Appendix A rounding of the deposited buffers (call between deposit() and apply())."""
+        cs, cm = self._cstate(), self._cmesh()
+        rc = self.L.orc_repro_buffers(C.byref(self.p), C.byref(cs), C.byref(cm), int(M))
+        assert rc == 0
 
     def state_old(self):
         """Views of the pre-step state kept by the last step()."""
@@ -294,3 +312,11 @@ def return_from_list(eta: np.ndarray, cells: np.ndarray, a: np.ndarray, V: float
     a = np.ascontiguousarray(a, dtype=np.float64)
     eta = np.ascontiguousarray(eta.reshape(-1), dtype=np.float64)
     return float(L.orc_return_from_list(_dp(eta), _lp(cells), _dp(a), cells.shape[0], V))
+
+
+def repro_bits(x: float, T: float, k: int, M: int) -> int:
+    return int(lib().orc_repro_bits(float(x), float(T), int(k), int(M)))
+
+
+def repro_round(x: float, T: float, k: int, M: int) -> float:
+    return float(lib().orc_repro_round(float(x), float(T), int(k), int(M)))
