@@ -75,7 +75,10 @@ enum {
     PM_FLAG_DEBUG_SCALARS = 1,   /* keep per-particle scalars (pm_debug_sink_scalars / pm_debug_sn_scalars) */
     PM_FLAG_DEBUG_LAMBDA = 2,    /* keep the Eq. 21 lambda of every cell (pm_debug_lambda) */
     PM_FLAG_GENERIC_KERNELS = 4, /* always use the generic (any radius, any n_sub) deposit / return kernels */
-    PM_FLAG_TIMING = 8           /* bracket every kernel with CUDA events on the ctx's stream (pm_kernel_times) */
+    PM_FLAG_TIMING = 8,          /* bracket every kernel with CUDA events on the ctx's stream (pm_kernel_times) */
+    PM_FLAG_REPRODUCIBLE = 16    /* Appendix A (L586-615): four more buffer channels (error scales, contribution counts) and a
+                                  * rounding pass at the end of pm_fold_ghosts: buffers no longer depend on the order of the
+                                  * atomic additions, except with probability ~2^-M per cell */
 };
 
 typedef struct { double *rho, *mx, *my, *mz, *etot, *eint; } pm_state;
@@ -114,6 +117,9 @@ int pm_apply_limited(pm_ctx *ctx, pm_state *state);
 
 /* Step 4.  Must be given the same sinks (same n, same positions) as the preceding pm_deposit. */
 int pm_return_to_particles(pm_ctx *ctx, pm_sinks *sinks);
+
+/* Margin M of Appendix A (N_bit = log2 r + 52 + M; default 28, the paper's example, L612).  Needs PM_FLAG_REPRODUCIBLE. */
+int pm_set_repro_margin(pm_ctx *ctx, int32_t M);
 
 /* Synchronise the ctx's stream and report PM_ECUDA / PM_EDOMAIN raised by earlier asynchronous work. */
 int pm_check(pm_ctx *ctx);

@@ -78,6 +78,8 @@ typedef struct {
     double *lam;         /* Eq. 21 lambda for the SN momentum (1 where no SN touches) */
     int32_t *sn_count;   /* number of SN particles contributing to the cell */
     int32_t *sink_count; /* number of sinks contributing to the cell */
+    double *Tp;          /* Appendix A (L600-606): sum over SNe of |dp_x^s| + |dp_y^s| + |dp_z^s|, the magnitudes of the values ADDED */
+    double *Te;          /* ... and of |dE^s|; one addition per particle and cell, as in the paper's E update */
 } orc_mesh_out;
 
 #define FOUR_PI 12.566370614359172953850573533118
@@ -422,6 +424,7 @@ int orc_deposit(const orc_params *p, const orc_state *U, orc_sinks *sk, orc_sne 
     for (int f = 0; f < 5; ++f) { if (!mo->S[f]) return -1; zero_mesh(mo->S[f], N); zero_mesh(mo->Sabs[f], N); }
     if (mo->sn_count) memset(mo->sn_count, 0, (size_t)N * sizeof(int32_t));
     if (mo->sink_count) memset(mo->sink_count, 0, (size_t)N * sizeof(int32_t));
+    zero_mesh(mo->Tp, N); zero_mesh(mo->Te, N);
     if (2 * kernel_halfwidth(p->rk_sink, p->dx) + 1 > p->nx && sk && sk->n > 0) return -2;   /* R32 */
 
     for (int64_t s = 0; sk && s < sk->n; ++s) {
@@ -474,6 +477,8 @@ int orc_deposit(const orc_params *p, const orc_state *U, orc_sinks *sk, orc_sne 
                         mo->S[f][c] += d[f];
                         if (mo->Sabs[f]) mo->Sabs[f][c] += da[f];
                     }
+                    if (mo->Tp) mo->Tp[c] += (fabs(d[1]) + fabs(d[2])) + fabs(d[3]);
+                    if (mo->Te) mo->Te[c] += fabs(d[4]);
                     if (mo->sn_count) mo->sn_count[c] += 1;
                 }
     }
@@ -509,14 +514,15 @@ double orc_repro_round(double x, double T, int32_t k, int32_t M) {
     return x;
 }
 
-/* Round the deposited buffers of one step (after orc_deposit, before orc_apply).  Needs Sabs and both counts.
+/* Round the deposited buffers of one step (after orc_deposit, before orc_apply).  Needs Tp, Te and both counts.
+ * T is the sum of the magnitudes of the values added to the buffer, one per particle and cell (the paper updates E once
+ * per addition of a particle's dU^s, L600-606) -- not of the sub-terms of Eq. 17 that Sabs holds for the test tolerances.
  * Accretion group: the terms of A[0] share a sign, so T = |A[0]|; the other five accretion channels are rebuilt from the
- * rounded A[0] in the rank-one form of R29, A[f] = A[0] U_f / rho, with the PRE-step state U.  SN group: T of d rho and
- * d E are their own sums of |terms|; the three momentum channels share T = sum_s (|dp_x| + |dp_y| + |dp_z|). */
+ * rounded A[0] in the rank-one form of R29, A[f] = A[0] U_f / rho, with the PRE-step state U.  SN group: d rho has
+ * same-sign terms (T = |S[0]|), d E uses Te, and the three momentum channels share Tp. */
 int orc_repro_buffers(const orc_params *p, const orc_state *U, orc_mesh_out *mo, int32_t M) {
     const int64_t N = (int64_t)p->nx * p->ny * p->nz;
-    if (!mo->sn_count || !mo->sink_count) return -1;
-    for (int f = 0; f < 5; ++f) if (!mo->Sabs[f]) return -1;
+    if (!mo->sn_count || !mo->sink_count || !mo->Tp || !mo->Te) return -1;
     for (int64_t c = 0; c < N; ++c) {
         const int32_t kk = mo->sink_count[c], kn = mo->sn_count[c];
         if (kk > 0) {
@@ -530,12 +536,12 @@ int orc_repro_buffers(const orc_params *p, const orc_state *U, orc_mesh_out *mo,
             mo->A[5][c] = a0 * (U->eint[c] / rho);
         }
         if (kn > 0) {
-            const double Tp = (mo->Sabs[1][c] + mo->Sabs[2][c]) + mo->Sabs[3][c];
-            mo->S[0][c] = orc_repro_round(mo->S[0][c], mo->Sabs[0][c], kn, M);
+            const double Tp = mo->Tp[c];
+            mo->S[0][c] = orc_repro_round(mo->S[0][c], fabs(mo->S[0][c]), kn, M);
             mo->S[1][c] = orc_repro_round(mo->S[1][c], Tp, kn, M);
             mo->S[2][c] = orc_repro_round(mo->S[2][c], Tp, kn, M);
             mo->S[3][c] = orc_repro_round(mo->S[3][c], Tp, kn, M);
-            mo->S[4][c] = orc_repro_round(mo->S[4][c], mo->Sabs[4][c], kn, M);
+            mo->S[4][c] = orc_repro_round(mo->S[4][c], mo->Te[c], kn, M);
         }
     }
     return 0;

@@ -61,7 +61,7 @@ class OrcSNe(C.Structure):
 
 class OrcMeshOut(C.Structure):
     _fields_ = [("A", c_dp * 6), ("S", c_dp * 5), ("Aabs", c_dp * 6), ("Sabs", c_dp * 5),
-                ("eta", c_dp), ("lam", c_dp), ("sn_count", c_ip), ("sink_count", c_ip)]
+                ("eta", c_dp), ("lam", c_dp), ("sn_count", c_ip), ("sink_count", c_ip), ("Tp", c_dp), ("Te", c_dp)]
 
 
 def build(force: bool = False) -> str:
@@ -170,6 +170,8 @@ class Oracle:
         self.lam = np.ones(N)
         self.sn_count = np.zeros(N, dtype=np.int32)
         self.sink_count = np.zeros(N, dtype=np.int32)
+        self.Tp = np.zeros(N) if keep_abs else None      # Appendix A error scales (sum of |values added| per cell)
+        self.Te = np.zeros(N) if keep_abs else None
         self.sink_diag = {k: np.zeros(sinks.n) for k in SINK_DIAG}
         self.sink_diag["n_member"] = np.zeros(sinks.n, dtype=np.int32)
         self.sn_diag = {k: np.zeros(sne.n) for k in SN_DIAG}
@@ -214,6 +216,7 @@ class Oracle:
             o.Sabs[f] = _dp(self.Sabs[f])
         o.eta, o.lam = _dp(self.eta), _dp(self.lam)
         o.sn_count, o.sink_count = _ip(self.sn_count), _ip(self.sink_count)
+        o.Tp, o.Te = _dp(self.Tp), _dp(self.Te)
         return o
 
     # -- stages ------------------------------------------------------------------------------

@@ -33,7 +33,7 @@ struct pm_ctx {
     int device;
     int sm_count;
     cudaStream_t stream;
-    double *buf;        // kBufChannels * Nb
+    double *buf;        // nch * Nb
     double *ret;        // N records of kRetWords doubles (eta, v_old x/y/z): one 32-byte sector per cell (NULL when rk_sink == 0)
     double *lam;        // N (debug only)
     double *sink_scal;  // 3 * cap_sinks: mdot, r_acc, sum w
@@ -54,6 +54,8 @@ struct pm_ctx {
     double *stg_sne;    long long stg_sne_cap;
     // particle binning: keys[np] | perm[np] | counts[2*ntile + 1]
     int *bin_mem;       long long bin_cap;
+    int nch;            // buffer channels allocated: 6, or 10 with PM_FLAG_REPRODUCIBLE
+    bool repro; int repro_M;
     bool timing;        // PM_FLAG_TIMING
     cudaEvent_t ev[PM_NUM_KERNELS][2];
     bool ev_used[PM_NUM_KERNELS];
@@ -168,6 +170,7 @@ __global__ void __launch_bounds__(256) k_bin_fill(const int *__restrict__ keys, 
 // ---------------------------------------------------------------------------------------------------------------
 // a1-a3: sinks.  One warp per sink; lanes stride over the (2g+1)^3 box in (k,j,i) order.
 // ---------------------------------------------------------------------------------------------------------------
+template <bool REPRO>
 __global__ void __launch_bounds__(128) k_deposit_sinks(const DevP P, const DevState U, const DevSinks S, const double dt,
                                                        double *__restrict__ buf0, double *__restrict__ scal,
                                                        double *__restrict__ dbg, int *__restrict__ err,
@@ -223,7 +226,9 @@ __global__ void __launch_bounds__(128) k_deposit_sinks(const DevP P, const DevSt
                                 cell_centre(P.x0[2], k, P.dx) - zs);
         if (r2 <= P.rk2_sink) {
             const double amt = sink_cell_amount(P, r2, sc.r_acc, wsum, sc.mdot, dt);
-            atomicAdd(buf0 + ghost_index(P, i, j, k), -amt);          // R1: signed change
+            double *dst = buf0 + ghost_index(P, i, j, k);
+            atomicAdd(dst, -amt);                                     // R1: signed change
+            if (REPRO) atomicAdd(dst + kChKsink * P.Nb, 1.0);         // Appendix A: contribution count
         }
     }
     if (lane == 0) {
@@ -241,6 +246,7 @@ __global__ void __launch_bounds__(128) k_deposit_sinks(const DevP P, const DevSt
 // ---------------------------------------------------------------------------------------------------------------
 constexpr int kSnWarps = 8;
 
+template <bool REPRO>
 __global__ void __launch_bounds__(kSnWarps * 32) k_deposit_sne(const DevP P, const DevState U, const DevSNe S,
                                                                 double *__restrict__ buf, double *__restrict__ dbg,
                                                                 int *__restrict__ err, const int *__restrict__ perm) {
@@ -292,6 +298,11 @@ __global__ void __launch_bounds__(kSnWarps * 32) k_deposit_sne(const DevP P, con
         double *dst = buf + P.Nb + ghost_index(P, i, j, k);
 #pragma unroll
         for (int f = 0; f < 5; ++f) atomicAdd(dst + (long long)f * P.Nb, d[f]);
+        if (REPRO) {                                 // Appendix A: error scales and the contribution count (dst is channel 1)
+            atomicAdd(dst + (kChTp - 1) * P.Nb, (fabs(d[1]) + fabs(d[2])) + fabs(d[3]));
+            atomicAdd(dst + (kChTe - 1) * P.Nb, fabs(d[4]));
+            atomicAdd(dst + (kChKsn - 1) * P.Nb, 1.0);
+        }
     }
     if (dbg && lane == 0) {
         const long long n = S.n;
@@ -347,7 +358,7 @@ __device__ __forceinline__ void stv(double *p, const double v[VEC]) {
 
 // W = 2: one thread folds two x-adjacent cells with 128-bit accesses (needs g and nx even, so that a pair never straddles
 // the g-wide face strip and every pair is 16-byte aligned); W = 1 otherwise.  Counts are in units of W cells.
-template <int W>
+template <int W, int NCH>
 __global__ void __launch_bounds__(256) k_fold_ghosts(const DevP P, double *__restrict__ buf, long long n_edge,
                                                      long long n_zslab, long long n_yslab) {
     const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -394,9 +405,9 @@ __global__ void __launch_bounds__(256) k_fold_ghosts(const DevP P, double *__res
         ok[m] = (!cx || ox) && (!cy || oy) && (!cz || oz);
         img[m] = ghost_index(P, i + cx * ox, j + cy * oy, k + cz * oz);
     }
-    double acc[kBufChannels][W];
+    double acc[NCH][W];
 #pragma unroll
-    for (int ch = 0; ch < kBufChannels; ++ch) {
+    for (int ch = 0; ch < NCH; ++ch) {
         const double *b = buf + (long long)ch * P.Nb;
         double a[W];
         ldv<W>(b + base, a);
@@ -412,7 +423,30 @@ __global__ void __launch_bounds__(256) k_fold_ghosts(const DevP P, double *__res
         for (int e = 0; e < W; ++e) acc[ch][e] = a[e];
     }
 #pragma unroll
-    for (int ch = 0; ch < kBufChannels; ++ch) stv<W>(buf + (long long)ch * P.Nb + base, acc[ch]);
+    for (int ch = 0; ch < NCH; ++ch) stv<W>(buf + (long long)ch * P.Nb + base, acc[ch]);
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// Appendix A (PM_FLAG_REPRODUCIBLE): round the six folded buffer channels of every owned cell (repro_round).  The fold
+// has already summed the error scales and counts of the ghost images into the owned cell.
+// ---------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_repro_round(const DevP P, double *__restrict__ buf, int M, long long n_cells) {
+    const long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (q >= n_cells) return;
+    const int i = (int)(q % P.nx);
+    const long long row = q / P.nx;
+    const int j = (int)(row % P.ny), k = (int)(row / P.ny);
+    double *b = buf + ghost_index(P, i, j, k);
+    const double ksn = b[(long long)kChKsn * P.Nb], ksk = b[(long long)kChKsink * P.Nb];
+    if (ksk > 1.0) { const double x = b[0]; b[0] = repro_round(x, fabs(x), ksk, M); }       // same-sign terms: T = |sum|
+    if (ksn > 1.0) {
+        const double tp = b[(long long)kChTp * P.Nb], te = b[(long long)kChTe * P.Nb];
+        const double x1 = b[P.Nb];
+        b[P.Nb] = repro_round(x1, fabs(x1), ksn, M);                                         // d rho: same-sign terms
+#pragma unroll
+        for (int f = 2; f <= 4; ++f) b[(long long)f * P.Nb] = repro_round(b[(long long)f * P.Nb], tp, ksn, M);
+        b[5 * P.Nb] = repro_round(b[5 * P.Nb], te, ksn, M);
+    }
 }
 
 // ---------------------------------------------------------------------------------------------------------------
@@ -580,10 +614,14 @@ extern "C" int pm_create(const pm_params *prm, int device, void *cuda_stream, pm
     cudaError_t e = cudaSetDevice(device);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, device);
     if (e == cudaSuccess) {   // L1 / shared-memory split of the particle kernels (measured)
-        e = cudaFuncSetAttribute(k_deposit_sinks_g4, cudaFuncAttributePreferredSharedMemoryCarveout, kSinkCarveout);
+        e = cudaFuncSetAttribute(k_deposit_sinks_g4<false>, cudaFuncAttributePreferredSharedMemoryCarveout, kSinkCarveout);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_deposit_sinks_g4<true>, cudaFuncAttributePreferredSharedMemoryCarveout, kSinkCarveout);
         if (e == cudaSuccess) e = cudaFuncSetAttribute(k_return_sinks_g4, cudaFuncAttributePreferredSharedMemoryCarveout, kSinkCarveout);
     }
-    if (e == cudaSuccess) e = cudaMalloc(&c->buf, (size_t)kBufChannels * P.Nb * sizeof(double));
+    c->repro = (prm->flags & PM_FLAG_REPRODUCIBLE) != 0;
+    c->repro_M = 28;                                  // the paper's example margin (L612)
+    c->nch = c->repro ? kReproChannels : kBufChannels;
+    if (e == cudaSuccess) e = cudaMalloc(&c->buf, (size_t)c->nch * P.Nb * sizeof(double));
     if (e == cudaSuccess && gs > 0) e = cudaMalloc(&c->ret, (size_t)kRetWords * N * sizeof(double));
     if (e == cudaSuccess && (prm->flags & PM_FLAG_DEBUG_LAMBDA)) e = cudaMalloc(&c->lam, (size_t)N * sizeof(double));
     if (e == cudaSuccess) e = cudaMalloc(&c->err_flag, sizeof(int));
@@ -593,7 +631,8 @@ extern "C" int pm_create(const pm_params *prm, int device, void *cuda_stream, pm
     if (e == cudaSuccess) {
         // opt in to the dynamic shared memory the SN kernel may need (<= 8 warps x tables)
         const size_t smem = kSnWarps * sn_table_bytes(2 * (gn > 0 ? gn : 1) + 1, P.nsub);
-        if (smem > 48 * 1024) e = cudaFuncSetAttribute(k_deposit_sne, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (smem > 48 * 1024) e = cudaFuncSetAttribute(k_deposit_sne<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e == cudaSuccess && smem > 48 * 1024) e = cudaFuncSetAttribute(k_deposit_sne<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     }
     if (e != cudaSuccess) {
         int rc = (e == cudaErrorMemoryAllocation) ? PM_ENOMEM : PM_ECUDA;
@@ -627,6 +666,14 @@ extern "C" int pm_destroy(pm_ctx *c) {
     if (c->err_flag) cudaFree(c->err_flag);
     if (c->err_host) cudaFreeHost(c->err_host);
     delete c;
+    return PM_OK;
+}
+
+extern "C" int pm_set_repro_margin(pm_ctx *c, int32_t M) {
+    if (!c) return PM_EINVAL;
+    if (!c->repro) PM_FAIL(c, PM_EINVAL, "pm_set_repro_margin needs PM_FLAG_REPRODUCIBLE");
+    if (M < 0 || M > 52) PM_FAIL(c, PM_EINVAL, "pm_set_repro_margin: M must be in [0, 52]");
+    c->repro_M = M;
     return PM_OK;
 }
 
@@ -684,7 +731,7 @@ extern "C" int pm_deposit(pm_ctx *c, const pm_state *st, const pm_sinks *sk, con
         tick(c, PM_K_BIN, 1);
     }
     {   // a0: reset (L59 "all cells initialized to zero")
-        const long long n2 = (long long)kBufChannels * P.Nb / 2;
+        const long long n2 = (long long)c->nch * P.Nb / 2;
         tick(c, PM_K_ZERO, 0);
         // grid of 16 CTAs per SM (two waves): 1.03 ms against 1.14 ms for 8; cudaMemsetAsync is faster alone (0.92 ms) but the
         // step as a whole is not (the deposit kernels behind it slow down by the same amount)
@@ -698,9 +745,9 @@ extern "C" int pm_deposit(pm_ctx *c, const pm_state *st, const pm_sinks *sk, con
         const unsigned blocks = (unsigned)((nk + 3) / 4);
         tick(c, PM_K_SINKS, 0);
         if (P.gs == 4 && !c->force_generic)
-            k_deposit_sinks_g4<<<blocks, kFastSinkWarps * 32, 0, c->stream>>>(P, U, S, dt, c->buf, c->sink_scal, dbg ? c->dbg_sink : nullptr, c->err_flag, perm);
+            (c->repro ? k_deposit_sinks_g4<true> : k_deposit_sinks_g4<false>)<<<blocks, kFastSinkWarps * 32, 0, c->stream>>>(P, U, S, dt, c->buf, c->sink_scal, dbg ? c->dbg_sink : nullptr, c->err_flag, perm);
         else
-            k_deposit_sinks<<<blocks, 128, 0, c->stream>>>(P, U, S, dt, c->buf, c->sink_scal, dbg ? c->dbg_sink : nullptr, c->err_flag, perm);
+            (c->repro ? k_deposit_sinks<true> : k_deposit_sinks<false>)<<<blocks, 128, 0, c->stream>>>(P, U, S, dt, c->buf, c->sink_scal, dbg ? c->dbg_sink : nullptr, c->err_flag, perm);
         if ((rc = check_launch(c, "k_deposit_sinks")) != PM_OK) return rc;
         tick(c, PM_K_SINKS, 1);
     }
@@ -710,9 +757,9 @@ extern "C" int pm_deposit(pm_ctx *c, const pm_state *st, const pm_sinks *sk, con
         const size_t smem = kSnWarps * sn_table_bytes(2 * P.gn + 1, P.nsub);
         tick(c, PM_K_SNE, 0);
         if (P.gn == 3 && P.nsub == 4 && !c->force_generic)
-            k_deposit_sne_g3n4<<<(unsigned)((nn + kFastSnWarps - 1) / kFastSnWarps), kFastSnWarps * 32, 0, c->stream>>>(P, U, S, c->buf, dbg ? c->dbg_sn : nullptr, c->err_flag, perm + nk);
+            (c->repro ? k_deposit_sne_g3n4<true> : k_deposit_sne_g3n4<false>)<<<(unsigned)((nn + kFastSnWarps - 1) / kFastSnWarps), kFastSnWarps * 32, 0, c->stream>>>(P, U, S, c->buf, dbg ? c->dbg_sn : nullptr, c->err_flag, perm + nk);
         else
-            k_deposit_sne<<<blocks, kSnWarps * 32, smem, c->stream>>>(P, U, S, c->buf, dbg ? c->dbg_sn : nullptr, c->err_flag, perm + nk);
+            (c->repro ? k_deposit_sne<true> : k_deposit_sne<false>)<<<blocks, kSnWarps * 32, smem, c->stream>>>(P, U, S, c->buf, dbg ? c->dbg_sn : nullptr, c->err_flag, perm + nk);
         if ((rc = check_launch(c, "k_deposit_sne")) != PM_OK) return rc;
         tick(c, PM_K_SNE, 1);
     }
@@ -734,9 +781,18 @@ extern "C" int pm_fold_ghosts(pm_ctx *c) {
     const long long n_edge = n_z + n_y + n_x;
     const unsigned blocks = (unsigned)((n_edge + 255) / 256);
     tick(c, PM_K_FOLD, 0);
-    if (W == 2) k_fold_ghosts<2><<<blocks, 256, 0, c->stream>>>(P, c->buf, n_edge, n_z, n_y);
-    else k_fold_ghosts<1><<<blocks, 256, 0, c->stream>>>(P, c->buf, n_edge, n_z, n_y);
+    if (c->repro) {
+        if (W == 2) k_fold_ghosts<2, kReproChannels><<<blocks, 256, 0, c->stream>>>(P, c->buf, n_edge, n_z, n_y);
+        else k_fold_ghosts<1, kReproChannels><<<blocks, 256, 0, c->stream>>>(P, c->buf, n_edge, n_z, n_y);
+    } else {
+        if (W == 2) k_fold_ghosts<2, kBufChannels><<<blocks, 256, 0, c->stream>>>(P, c->buf, n_edge, n_z, n_y);
+        else k_fold_ghosts<1, kBufChannels><<<blocks, 256, 0, c->stream>>>(P, c->buf, n_edge, n_z, n_y);
+    }
     int rc = check_launch(c, "k_fold_ghosts");
+    if (rc == PM_OK && c->repro) {      // Appendix A: round the folded sums (error scales and counts were folded with them)
+        k_repro_round<<<(unsigned)((P.N + 255) / 256), 256, 0, c->stream>>>(P, c->buf, c->repro_M, P.N);
+        rc = check_launch(c, "k_repro_round");
+    }
     tick(c, PM_K_FOLD, 1);
     if (rc != PM_OK) return rc;
     c->stage = ST_FOLDED;

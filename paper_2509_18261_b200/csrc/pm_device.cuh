@@ -12,6 +12,12 @@ namespace pm {
 
 constexpr int kBufChannels = 6;      // 0: accretion d rho (signed, R1/R29); 1..5: SN d rho, d p (3), d E
 constexpr int kRetWords = 4;         // eta, v_old (3)
+// Appendix A mode (PM_FLAG_REPRODUCIBLE) adds four channels behind the six: error scales and contribution counts
+constexpr int kChTp = 6;             // sum_s (|dp_x| + |dp_y| + |dp_z|) of the SN terms
+constexpr int kChTe = 7;             // sum_s |dE| of the SN terms
+constexpr int kChKsn = 8;            // number of SNe that contributed (as a double)
+constexpr int kChKsink = 9;          // number of sinks that contributed
+constexpr int kReproChannels = 10;
 constexpr int kSbLog2 = 2;           // a super-block is (2^kSbLog2)^3 tiles of 8^3 cells (1..6 measured: no difference)
 constexpr double kFourPi = 12.566370614359172953850573533118;
 
@@ -293,6 +299,20 @@ __device__ __forceinline__ double apply_cell(const DevP &P, double u[6], const d
     }
     *lam_out = lam;
     return eta;
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// Appendix A (L586-615, R34): clear the N_bit least significant mantissa bits of a buffer value x that is the sum of k
+// terms with sum of magnitudes T:  N_bit = ilogb((k - 1) T) - ilogb(|x|) + 1 + M, clamped to [0, 52]  (integer arithmetic
+// on binary exponents: the order-independent bound E <= eps (k - 1) T for the paper's running error sum E).
+// ---------------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ double repro_round(double x, double T, double k, int M) {
+    if (!(k > 1.0) || x == 0.0 || !(T > 0.0)) return x;
+    int nb = ilogb((k - 1.0) * T) - ilogb(fabs(x)) + 1 + M;
+    if (nb <= 0) return x;
+    if (nb > 52) nb = 52;
+    const unsigned long long u = (unsigned long long)__double_as_longlong(x) & ~((1ull << nb) - 1ull);
+    return __longlong_as_double((long long)u);
 }
 
 }  // namespace pm

@@ -103,6 +103,7 @@ __device__ __forceinline__ double sink_weight(const SinkWarpSmem &sm, int code) 
     return (sm.ex[2][code >> 8] * sm.ex[1][(code >> 4) & 15]) * sm.ex[0][code & 15];
 }
 
+template <bool REPRO>
 __global__ void __launch_bounds__(kFastSinkWarps * 32, kFastSinkMinBlocks) k_deposit_sinks_g4(const DevP P, const DevState U, const DevSinks S,
                                                                           const double dt, double *__restrict__ buf0,
                                                                           double *__restrict__ scal, double *__restrict__ dbg,
@@ -146,7 +147,9 @@ __global__ void __launch_bounds__(kFastSinkWarps * 32, kFastSinkMinBlocks) k_dep
     double *const sbuf = buf0 + (ih - 4 + P.gx);
     for (int i = lane; i < nm; i += 32) {
         const int code = sm.code[i];
-        atomicAdd(sbuf + sink_ghosted(sm, code), -(sink_weight(sm, code) * k));   // R1: signed
+        double *dst = sbuf + sink_ghosted(sm, code);
+        atomicAdd(dst, -(sink_weight(sm, code) * k));   // R1: signed
+        if (REPRO) atomicAdd(dst + kChKsink * P.Nb, 1.0);   // Appendix A: contribution count (same-sign terms: T = |sum|)
     }
     if (lane == 0) {
         scal[s] = sc.mdot; scal[S.n + s] = sc.r_acc; scal[2 * S.n + s] = wsum;

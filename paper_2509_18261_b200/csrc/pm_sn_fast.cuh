@@ -50,6 +50,7 @@ __device__ __forceinline__ void sn_fill_dec(unsigned short *dec) {
     }
 }
 
+template <bool REPRO>
 __device__ __forceinline__ void sn_deposit_one(const DevP &P, const DevState &U, const DevSNe &S, double *__restrict__ buf,
                                                double *__restrict__ dbg, int *__restrict__ err, const long long s,
                                                SnWarpSmem &sm, const unsigned short *dec, const int lane) {
@@ -199,11 +200,20 @@ __device__ __forceinline__ void sn_deposit_one(const DevP &P, const DevState &U,
         const double prx = pscale * ddx, pry = pscale * ddy, prz = pscale * ddz;
         double *dst = sbuf + (sm.goff[1][cc] + sm.goff[0][b] + a);
         // omega rho (v_COM - v) = omega (rho v_COM - m): no division by rho
+        const double dpx = fma(omega, fma(rho, sc.vcx, -mx), fma(drho, sc.vcx, prx));
+        const double dpy = fma(omega, fma(rho, sc.vcy, -my), fma(drho, sc.vcy, pry));
+        const double dpz = fma(omega, fma(rho, sc.vcz, -mz), fma(drho, sc.vcz, prz));
+        const double de = fma(omega, k_e, fma(sc.vcx, prx, fma(sc.vcy, pry, sc.vcz * prz)));
         atomicAdd(dst, drho);
-        atomicAdd(dst + P.Nb, fma(omega, fma(rho, sc.vcx, -mx), fma(drho, sc.vcx, prx)));
-        atomicAdd(dst + 2 * P.Nb, fma(omega, fma(rho, sc.vcy, -my), fma(drho, sc.vcy, pry)));
-        atomicAdd(dst + 3 * P.Nb, fma(omega, fma(rho, sc.vcz, -mz), fma(drho, sc.vcz, prz)));
-        atomicAdd(dst + 4 * P.Nb, fma(omega, k_e, fma(sc.vcx, prx, fma(sc.vcy, pry, sc.vcz * prz))));
+        atomicAdd(dst + P.Nb, dpx);
+        atomicAdd(dst + 2 * P.Nb, dpy);
+        atomicAdd(dst + 3 * P.Nb, dpz);
+        atomicAdd(dst + 4 * P.Nb, de);
+        if (REPRO) {                                 // Appendix A: error scales and the contribution count (dst is channel 1)
+            atomicAdd(dst + (kChTp - 1) * P.Nb, (fabs(dpx) + fabs(dpy)) + fabs(dpz));
+            atomicAdd(dst + (kChTe - 1) * P.Nb, fabs(de));
+            atomicAdd(dst + (kChKsn - 1) * P.Nb, 1.0);
+        }
     }
     if (dbg && lane == 0) {
         const long long n = S.n;
@@ -213,6 +223,7 @@ __device__ __forceinline__ void sn_deposit_one(const DevP &P, const DevState &U,
 }
 
 // One warp per SN particle, particles taken in bin order (perm).
+template <bool REPRO>
 __global__ void __launch_bounds__(kFastSnWarps * 32, kFastSnMinBlocks) k_deposit_sne_g3n4(const DevP P, const DevState U, const DevSNe S,
                                                                             double *__restrict__ buf, double *__restrict__ dbg,
                                                                             int *__restrict__ err, const int *__restrict__ perm) {
@@ -223,7 +234,7 @@ __global__ void __launch_bounds__(kFastSnWarps * 32, kFastSnMinBlocks) k_deposit
     const int wib = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const long long w = (long long)blockIdx.x * kFastSnWarps + wib;
     if (w >= S.n) return;
-    sn_deposit_one(P, U, S, buf, dbg, err, perm[w], sm_all[wib], dec, lane);
+    sn_deposit_one<REPRO>(P, U, S, buf, dbg, err, perm[w], sm_all[wib], dec, lane);
 }
 
 }  // namespace pm

@@ -19,12 +19,12 @@ HDRS = [os.path.join(_HERE, "csrc", "pm_device.cuh"), os.path.join(_HERE, "csrc"
         os.path.join(_HERE, "csrc", "pm_sn_fast.cuh"), os.path.join(_HERE, "csrc", "pm_sink_fast.cuh"), os.path.join(os.path.dirname(_HERE), "include", "pm.h")]
 
 PM_OK, PM_EINVAL, PM_ENOMEM, PM_ECUDA, PM_EORDER, PM_EDOMAIN = 0, -1, -2, -3, -4, -5
-PM_FLAG_DEBUG_SCALARS, PM_FLAG_DEBUG_LAMBDA, PM_FLAG_GENERIC_KERNELS, PM_FLAG_TIMING = 1, 2, 4, 8
+PM_FLAG_DEBUG_SCALARS, PM_FLAG_DEBUG_LAMBDA, PM_FLAG_GENERIC_KERNELS, PM_FLAG_TIMING, PM_FLAG_REPRODUCIBLE = 1, 2, 4, 8, 16
 KERNEL_GROUPS = ("bin", "zero", "sinks", "sne", "fold", "apply", "return")
 STATUS_NAMES = {0: "PM_OK", -1: "PM_EINVAL", -2: "PM_ENOMEM", -3: "PM_ECUDA", -4: "PM_EORDER", -5: "PM_EDOMAIN"}
 
 EXPORTS = ["pm_create", "pm_deposit", "pm_fold_ghosts", "pm_apply_limited", "pm_return_to_particles", "pm_check",
-           "pm_step_host", "pm_destroy", "pm_last_error", "pm_launch_count", "pm_kernel_times", "pm_probe_red_f64", "pm_debug_buffer",
+           "pm_step_host", "pm_destroy", "pm_last_error", "pm_launch_count", "pm_kernel_times", "pm_probe_red_f64", "pm_set_repro_margin", "pm_debug_buffer",
            "pm_debug_return_mesh", "pm_debug_lambda", "pm_debug_sink_scalars", "pm_debug_sn_scalars",
            "pm_debug_stencil"]
 
@@ -102,6 +102,7 @@ def lib():
         L.pm_last_error.restype = C.c_char_p
         L.pm_launch_count.argtypes = [vp]
         L.pm_launch_count.restype = C.c_int64
+        L.pm_set_repro_margin.argtypes = [vp, C.c_int32]
         L.pm_kernel_times.argtypes = [vp, C.POINTER(C.c_float), C.c_int32]
         L.pm_probe_red_f64.argtypes = [vp, C.c_int64, C.c_int32, C.POINTER(C.c_double)]
         L.pm_debug_buffer.argtypes = [vp, C.c_int, C.POINTER(vp), i64p, i64p, i32p]
@@ -285,6 +286,9 @@ class Context:
             for f in DeviceSNe.IN:
                 setattr(cn, f, hp(getattr(sn, f)))
         self._chk(self.L.pm_step_host(self.h, C.byref(cs), C.byref(ck), C.byref(cn), dt), "pm_step_host")
+
+    def pm_set_repro_margin(self, M: int):
+        self._chk(self.L.pm_set_repro_margin(self.h, int(M)), "pm_set_repro_margin")
 
     def pm_kernel_times(self) -> dict:
         """ms of each kernel group in the last step (needs PM_FLAG_TIMING)."""
