@@ -156,15 +156,15 @@ def whole_job_value(cells_per_rank: int, steps: int, world: int, total_ms: float
     return world * cells_per_rank * steps / (total_ms * 1e-3) / 1e6
 
 
-def algorithmic_bytes(N, Nb, nk, nn, t4, ts4, tn4):
+def algorithmic_bytes(N, Nb, nk, nn, t4, ts4, tn4, nch=6):
     """Bytes each kernel group must move per step (SURVEY.md 8(d) per-cell figures times
     the fraction of 32-byte sectors (4 cells) that hold a touched cell -- the smallest unit HBM moves)."""
     return {
         "bin": 8.0 * 3 * (nk + nn) + 4.0 * 3 * (nk + nn),            # positions read, keys + perm written and read
-        "zero": 8.0 * 6 * Nb,                                        # store only
-        "sinks": 8.0 * 5 * ts4 * N + 8.0 * 1 * ts4 * N + 8.0 * 10 * nk,   # gather 5 fields, write back 1 channel once
-        "sne": 8.0 * 4 * tn4 * N + 8.0 * 5 * tn4 * N + 8.0 * 8 * nn,      # gather 4 fields, write back 5 channels once
-        "fold": 3 * 8.0 * 6 * (Nb - N),                              # read ghosts, read-modify-write owned images
+        "zero": 8.0 * nch * Nb,                                      # store only (10 channels in Appendix A mode)
+        "sinks": 8.0 * 5 * ts4 * N + 8.0 * (1 + (nch > 6)) * ts4 * N + 8.0 * 10 * nk,   # gather 5 fields, write back 1 (2) channels once
+        "sne": 8.0 * 4 * tn4 * N + 8.0 * (5 + 3 * (nch > 6)) * tn4 * N + 8.0 * 8 * nn,  # gather 4 fields, write back 5 (8) channels once
+        "fold": 3 * 8.0 * nch * (Nb - N) + (8.0 * 16 * t4 * N if nch > 6 else 0.0),   # read ghosts, RMW owned images (+ rounding pass: read 10, write 6 where touched)
         "apply": N * (48.0 + 96.0 * t4 + 32.0 * ts4),                # 6 buffer words; 6 + 6 state words and 4 return words where touched
         "return": 8.0 * 4 * ts4 * N + 8.0 * 12 * nk,
     }
@@ -196,7 +196,9 @@ def run_ours(args, rank, world, local_rank):
     N = n ** 3
     Nb = (n + 8) ** 3
     npart = w.sinks.n + w.sne.n
-    ctx = pm.Context(w.params, device=str(dev))          # the timed steps run without the per-kernel events
+    mode = pm.PM_FLAG_REPRODUCIBLE if args.reproducible else 0
+    nch = 10 if args.reproducible else 6
+    ctx = pm.Context(w.params, device=str(dev), flags=mode)          # the timed steps run without the per-kernel events
     st = pm.DeviceState.from_host(w.state, dev)
     sk = pm.DeviceSinks.from_host(w.sinks, dev)
     sn = pm.DeviceSNe.from_host(w.sne, dev)
@@ -250,7 +252,7 @@ def run_ours(args, rank, world, local_rank):
     value = whole_job_value(N, args.steps, world, total_ms)
     # per-kernel device times: the library's own CUDA events on the launching stream (PM_FLAG_TIMING), three more steps
     ctx.close()
-    ctx = pm.Context(w.params, device=str(dev), flags=pm.PM_FLAG_TIMING)
+    ctx = pm.Context(w.params, device=str(dev), flags=pm.PM_FLAG_TIMING | mode)
     ksamples = []
     for it in range(5):
         one_step()
@@ -283,7 +285,7 @@ def run_ours(args, rank, world, local_rank):
 
     if rank == 0:
         peak, peak_src = measured_peak()
-        abytes = algorithmic_bytes(N, Nb, w.sinks.n, w.sne.n, t4, ts4, tn4)
+        abytes = algorithmic_bytes(N, Nb, w.sinks.n, w.sne.n, t4, ts4, tn4, nch)
         kernels = {}
         for k in pm.KERNEL_GROUPS:
             if kernel_ms[k] > 0:
@@ -298,7 +300,7 @@ def run_ours(args, rank, world, local_rank):
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": warm, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": w.name, "cells": N, "particles": npart, "sinks": w.sinks.n, "sne": w.sne.n,
+            "config": {"workload": w.name + ("+appendixA_reproducible" if args.reproducible else ""), "cells": N, "particles": npart, "sinks": w.sinks.n, "sne": w.sne.n,
                        "multi_gpu": "replicas only" if world > 1 else "single GPU",
                        "l2_policy": "inputs larger than L2 (state 6 fields + 6-channel buffer, GBs >> 126 MB)",
                        "touched_cell_fraction": t_frac, "sink_touched_fraction": ts_frac,
@@ -322,7 +324,7 @@ def run_ours(args, rank, world, local_rank):
                               "achieved_gbs": step_bytes / (ms_per_step * 1e-3) / 1e9,
                               "frac_of_measured_peak": step_bytes / (ms_per_step * 1e-3) / 1e9 / peak,
                               "frac_of_8tbs_nominal": step_bytes / (ms_per_step * 1e-3) / 1e9 / 8000.0,
-                              "dense_survey_bytes": 8.0 * 6 * Nb + 8.0 * 5 * N + 120.0 * npart + 144.0 * (Nb - N) + 176.0 * N + 32.0 * ts4 * N},
+                              "dense_survey_bytes": 8.0 * nch * Nb + 8.0 * 5 * N + 120.0 * npart + 144.0 * (Nb - N) + 176.0 * N + 32.0 * ts4 * N},
         }
         if red_probe:
             n_red = 5.0 * 183.0 * w.sne.n     # ~183 cells with omega > 0 per SN (SURVEY.md 8 probe), 5 channels
@@ -347,6 +349,8 @@ def main():
     ap.add_argument("--particles", type=int, default=1_000_000)
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--reproducible", action="store_true",
+                    help="Appendix A mode (PM_FLAG_REPRODUCIBLE): 4 more buffer channels + rounding pass; a separate workload variant")
     args = ap.parse_args()
     rank, world, local_rank = env_int("RANK", 0), env_int("WORLD_SIZE", 1), env_int("LOCAL_RANK", 0)
     if args.impl == "reference":

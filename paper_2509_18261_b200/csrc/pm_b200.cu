@@ -430,22 +430,39 @@ __global__ void __launch_bounds__(256) k_fold_ghosts(const DevP P, double *__res
 // Appendix A (PM_FLAG_REPRODUCIBLE): round the six folded buffer channels of every owned cell (repro_round).  The fold
 // has already summed the error scales and counts of the ghost images into the owned cell.
 // ---------------------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) k_repro_round(const DevP P, double *__restrict__ buf, int M, long long n_cells) {
-    const long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (q >= n_cells) return;
-    const int i = (int)(q % P.nx);
-    const long long row = q / P.nx;
+template <int W>
+__global__ void __launch_bounds__(256) k_repro_round(const DevP P, double *__restrict__ buf, int M, long long n_items) {
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= n_items) return;
+    const int nxw = P.nx / W;
+    const int i = W * (int)(t % nxw);
+    const long long row = t / nxw;
     const int j = (int)(row % P.ny), k = (int)(row / P.ny);
     double *b = buf + ghost_index(P, i, j, k);
-    const double ksn = b[(long long)kChKsn * P.Nb], ksk = b[(long long)kChKsink * P.Nb];
-    if (ksk > 1.0) { const double x = b[0]; b[0] = repro_round(x, fabs(x), ksk, M); }       // same-sign terms: T = |sum|
-    if (ksn > 1.0) {
-        const double tp = b[(long long)kChTp * P.Nb], te = b[(long long)kChTe * P.Nb];
-        const double x1 = b[P.Nb];
-        b[P.Nb] = repro_round(x1, fabs(x1), ksn, M);                                         // d rho: same-sign terms
+    double ksn[W], ksk[W];
+    ldv<W>(b + (long long)kChKsn * P.Nb, ksn);
+    ldv<W>(b + (long long)kChKsink * P.Nb, ksk);
+    bool any_sn = false, any_sk = false;
 #pragma unroll
-        for (int f = 2; f <= 4; ++f) b[(long long)f * P.Nb] = repro_round(b[(long long)f * P.Nb], tp, ksn, M);
-        b[5 * P.Nb] = repro_round(b[5 * P.Nb], te, ksn, M);
+    for (int e = 0; e < W; ++e) { any_sn |= ksn[e] > 1.0; any_sk |= ksk[e] > 1.0; }
+    if (any_sk) {                                                      // same-sign terms: T = |sum|
+        double x[W];
+        ldv<W>(b, x);
+#pragma unroll
+        for (int e = 0; e < W; ++e) x[e] = repro_round(x[e], fabs(x[e]), ksk[e], M);
+        stv<W>(b, x);
+    }
+    if (any_sn) {
+        double tp[W], te[W], x[W];
+        ldv<W>(b + (long long)kChTp * P.Nb, tp);
+        ldv<W>(b + (long long)kChTe * P.Nb, te);
+#pragma unroll
+        for (int f = 1; f <= 5; ++f) {
+            ldv<W>(b + (long long)f * P.Nb, x);
+#pragma unroll
+            for (int e = 0; e < W; ++e) x[e] = repro_round(x[e], f == 1 ? fabs(x[e]) : (f == 5 ? te[e] : tp[e]), ksn[e], M);
+            stv<W>(b + (long long)f * P.Nb, x);
+        }
     }
 }
 
@@ -790,7 +807,8 @@ extern "C" int pm_fold_ghosts(pm_ctx *c) {
     }
     int rc = check_launch(c, "k_fold_ghosts");
     if (rc == PM_OK && c->repro) {      // Appendix A: round the folded sums (error scales and counts were folded with them)
-        k_repro_round<<<(unsigned)((P.N + 255) / 256), 256, 0, c->stream>>>(P, c->buf, c->repro_M, P.N);
+        if (P.nx % 2 == 0) k_repro_round<2><<<(unsigned)((P.N / 2 + 255) / 256), 256, 0, c->stream>>>(P, c->buf, c->repro_M, P.N / 2);
+        else k_repro_round<1><<<(unsigned)((P.N + 255) / 256), 256, 0, c->stream>>>(P, c->buf, c->repro_M, P.N);
         rc = check_launch(c, "k_repro_round");
     }
     tick(c, PM_K_FOLD, 1);

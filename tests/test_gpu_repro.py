@@ -102,3 +102,28 @@ def test_margin_setter_and_errors():
     o = po.Oracle(w.params, w.state.copy(), w.sinks.copy(), w.sne.copy())
     o.step(w.dt, repro_M=8)
     assert np.allclose(st.rho.cpu().numpy(), o.state.rho, rtol=1e-12)      # M = 8 keeps 40+ bits
+
+
+def test_full_size_reproducible_step_twice_identical():
+    """Config 5 (512^3, 10^6 particles) in the launch configuration bench.py --reproducible times: two independent runs of the
+    same step (different atomic order, as always) leave bit-identical buffers and state."""
+    w = inputs.make(5)
+    dev = torch.device("cuda:0")
+    outs = []
+    for rep in range(2):
+        ctx = pm.Context(w.params, device="cuda:0", flags=pm.PM_FLAG_REPRODUCIBLE)
+        st = pm.DeviceState.from_host(w.state, dev)
+        sk = pm.DeviceSinks.from_host(w.sinks, dev)
+        sn = pm.DeviceSNe.from_host(w.sne, dev)
+        ctx.pm_deposit(st, sk, sn, w.dt)
+        ctx.pm_fold_ghosts()
+        sums = [ctx.debug_buffer(ch)[1].clone() for ch in (0, 2, 5)]
+        ctx.pm_apply_limited(st)
+        ctx.pm_return_to_particles(sk)
+        ctx.pm_check()
+        outs.append((sums, st.mx.clone(), st.eint.clone(), sk.m.clone()))
+        ctx.close()
+        del st, sk, sn
+    for a, b in zip(outs[0][0], outs[1][0]):
+        assert torch.equal(a, b)
+    assert torch.equal(outs[0][1], outs[1][1]) and torch.equal(outs[0][2], outs[1][2]) and torch.equal(outs[0][3], outs[1][3])
