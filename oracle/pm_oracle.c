@@ -24,6 +24,9 @@
  *
  * Build: gcc -O2 -ffp-contract=off -fPIC -shared -o liboracle_pm.so pm_oracle.c -lm
  */
+#ifndef _GNU_SOURCE
+#define _GNU_SOURCE
+#endif
 #include <math.h>
 #include <stdint.h>
 #include <stdlib.h>
@@ -46,6 +49,7 @@ typedef struct {
     double sn_psnr_coeff, sn_psnr_exp;                   /* Eq. 20 */
     double sn_mu_h, sn_nh_unit;
     double sn_eint_theta;         /* R25: e_min = theta * rho_2 * (e_int,1 / rho_1) */
+    double truelove_J;            /* Jeans number J of Eq. 12 (0.25 in the paper, L148); 0 = Truelove terms off (R10) */
 } orc_params;
 
 /* gas state, nx*ny*nz each, x fastest, no ghosts */
@@ -183,12 +187,23 @@ static void sink_compute_scalars(const orc_params *p, const orc_state *U, double
     o->wsum = wsum;
 }
 
-/* Eq. 13 without the Truelove term (R10): mass removed per unit volume from a member cell. */
-static inline double sink_cell_amount(const orc_params *p, const sink_scalars *sc, double r2, double dt) {
+/* Eq. 12: rho_Tr = J^2 pi c_s^2 / (G dx^2) with the cell's own sound speed (R6); +inf when the terms are off (R10). */
+static inline double rho_truelove(const orc_params *p, double rho, double eint) {
+    if (!(p->truelove_J > 0.0)) return INFINITY;
+    double cs = sound_speed(p, rho, eint);
+    return p->truelove_J * p->truelove_J * M_PI * cs * cs / (p->G * p->dx * p->dx);
+}
+
+/* Eqs. 13-14: mass removed per unit volume from a member cell, max(mdot_BH, mdot_Tr) phi dt / V.  With
+ * mdot_Tr = (rho - rho_Tr) V / (phi dt) the second candidate is simply rho - rho_Tr (R37: written in that form, which
+ * stays finite when phi underflows to 0).  rho, eint are the PRE-step values of the cell. */
+static inline double sink_cell_amount(const orc_params *p, const sink_scalars *sc, double r2, double dt, double rho, double eint) {
     double w = exp(-r2 / (sc->r_acc * sc->r_acc));    /* Eq. 9 */
     double phi = w / sc->wsum;                        /* Eq. 11 */
     double V = p->dx * p->dx * p->dx;
-    return sc->mdot * phi * dt / V;
+    double a = sc->mdot * phi * dt / V;
+    double a_tr = rho - rho_truelove(p, rho, eint);   /* Eq. 14 times phi dt / V */
+    return a_tr > a ? a_tr : a;
 }
 
 static void store_sink_diag(orc_sinks *sk, int64_t s, const sink_scalars *sc) {
@@ -326,13 +341,16 @@ static void store_sn_diag(orc_sne *sn, int64_t s, const sn_scalars *sc) {
 /* ------------------------------------------------------------------------------------------ */
 static void apply_cell(const orc_params *p, double u[6], const double A[6], const double S[5], int sn_touched,
                        double *eta_out, double *lam_out) {
-    /* accretion limiter, Eqs. 15-16 with rho_Tr = +inf (R10), generalised by R11 */
+    /* accretion limiter, Eqs. 15-16: d rho_lim = max[min(d rho, f rho), rho - rho_Tr], generalised by R11 (f, floor) */
     double a = -A[0];
     double eta = 1.0;                                                  /* R12 */
     if (a > 0.0) {
         double alim = a;
         double cap = p->f_max_remove * u[0];
         if (cap < alim) alim = cap;
+        double need = u[0] - rho_truelove(p, u[0], u[5]);              /* Eq. 16: never leave the cell above rho_Tr ... */
+        if (need > alim) alim = need;
+        if (alim > a) alim = a;                                        /* ... but never remove more than was requested */
         double room = u[0] - p->rho_floor;
         if (room < 0.0) room = 0.0;
         if (room < alim) alim = room;
@@ -438,8 +456,8 @@ int orc_deposit(const orc_params *p, const orc_state *U, orc_sinks *sk, orc_sne 
                     double r2;
                     if (!sink_member(p, xs, ys, zs, i, j, k, &r2)) continue;
                     int64_t c = cell_index(p, i, j, k);
-                    double a = sink_cell_amount(p, &sc, r2, dt);
                     double rho = U->rho[c];
+                    double a = sink_cell_amount(p, &sc, r2, dt, rho, U->eint[c]);
                     /* Eq. 13 (R1: signed change; R9: same mass fraction from every field) */
                     double d[6];
                     d[0] = -a;
@@ -578,8 +596,8 @@ int orc_return(const orc_params *p, const orc_state *U_old, const double *eta, o
                     double r2;
                     if (!sink_member(p, xs, ys, zs, i, j, k, &r2)) continue;
                     int64_t c = cell_index(p, i, j, k);
-                    double a = sink_cell_amount(p, &sc, r2, dt);
                     double rho = U_old->rho[c];
+                    double a = sink_cell_amount(p, &sc, r2, dt, rho, U_old->eint[c]);
                     double gain = eta[c] * a * V;                     /* -eta dU^s V, mass */
                     dm += gain;
                     dpx += gain * (U_old->mx[c] / rho);               /* R14 */
@@ -675,7 +693,7 @@ int orc_sample_cells(const orc_params *p, const orc_state *U, const orc_sinks *s
             if (!sink_member(p, sk->x[s], sk->y[s], sk->z[s], ih + di, jh + dj, kh + dk, &r2)) continue;
             sink_scalars sc;
             sink_compute_scalars(p, U, sk->x[s], sk->y[s], sk->z[s], sk->vx[s], sk->vy[s], sk->vz[s], sk->m[s], &sc);
-            double a = sink_cell_amount(p, &sc, r2, dt);
+            double a = sink_cell_amount(p, &sc, r2, dt, rho, U->eint[c]);
             double d[6] = { -a, -a * (U->mx[c] / rho), -a * (U->my[c] / rho), -a * (U->mz[c] / rho),
                             -a * (U->etot[c] / rho), -a * (U->eint[c] / rho) };
             double cond = 1.0 + r2 / (sc.r_acc * sc.r_acc);
@@ -733,7 +751,7 @@ int32_t orc_sink_amounts(const orc_params *p, const orc_state *U, double xs, dou
             for (int64_t i = sc.ih - sc.g; i <= sc.ih + sc.g; ++i) {
                 double r2;
                 if (!sink_member(p, xs, ys, zs, i, j, k, &r2)) continue;
-                if (n < max_cells) { cells_out[n] = cell_index(p, i, j, k); a_out[n] = sink_cell_amount(p, &sc, r2, dt); }
+                if (n < max_cells) { cells_out[n] = cell_index(p, i, j, k); const int64_t cc = cell_index(p, i, j, k); a_out[n] = sink_cell_amount(p, &sc, r2, dt, U->rho[cc], U->eint[cc]); }
                 n += 1;
             }
     return n;

@@ -40,6 +40,7 @@ def default_params(n: int) -> dict:
         sn_psnr_coeff=1030.0, sn_psnr_exp=-0.17,
         sn_mu_h=1.0, sn_nh_unit=1.0,
         sn_eint_theta=1.0,
+        truelove_J=0.0,                            # Eq. 12 Jeans number; 0 = off in all BASELINE configs (paper: 0.25, L148)
     )
 
 
