@@ -69,6 +69,8 @@ typedef struct {
     double sn_psnr_coeff, sn_psnr_exp;       /* P_snr = coeff (n_H / nh_unit)^exp, Eq. 20 (L229) */
     double sn_mu_h, sn_nh_unit;              /* mass per H nucleus; unit of n_H */
     double sn_eint_theta;        /* Eq. 21 floor: e_min = theta rho_2 (e_int,1/rho_1); 1 = as printed, 0 = e_int >= 0 only (R25) */
+    double truelove_J;           /* Jeans number J of Eq. 12, rho_Tr = J^2 pi c_s^2 / (G dx^2); 0.25 in the paper (L148); 0 = the Truelove
+                                  * terms of Eqs. 13-14 and 16 are off (all BASELINE configs) */
 } pm_params;
 
 enum {

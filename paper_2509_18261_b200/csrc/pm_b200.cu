@@ -35,6 +35,7 @@ struct pm_ctx {
     cudaStream_t stream;
     double *buf;        // nch * Nb
     double *ret;        // N records of kRetWords doubles (eta, v_old x/y/z): one 32-byte sector per cell (NULL when rk_sink == 0)
+    double *ret_tr;     // N: rho_old - rho_Tr where a sink removed mass (Truelove on only; Step 4 re-evaluates Eq. 14 from it)
     double *lam;        // N (debug only)
     double *sink_scal;  // 3 * cap_sinks: mdot, r_acc, sum w
     long long cap_sinks;
@@ -174,7 +175,8 @@ template <bool REPRO>
 __global__ void __launch_bounds__(128) k_deposit_sinks(const DevP P, const DevState U, const DevSinks S, const double dt,
                                                        double *__restrict__ buf0, double *__restrict__ scal,
                                                        double *__restrict__ dbg, int *__restrict__ err,
-                                                       const int *__restrict__ perm) {
+                                                       const int *__restrict__ perm,
+                                                       double *__restrict__ ret_tr) {
     const long long w = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
     const int lane = threadIdx.x & 31;
     if (w >= S.n) return;
@@ -225,7 +227,12 @@ __global__ void __launch_bounds__(128) k_deposit_sinks(const DevP P, const DevSt
         const double r2 = dist2(cell_centre(P.x0[0], i, P.dx) - xs, cell_centre(P.x0[1], j, P.dx) - ys,
                                 cell_centre(P.x0[2], k, P.dx) - zs);
         if (r2 <= P.rk2_sink) {
-            const double amt = sink_cell_amount(P, r2, sc.r_acc, wsum, sc.mdot, dt);
+            double amt = sink_cell_amount(P, r2, sc.r_acc, wsum, sc.mdot, dt);
+            if (P.tl_num > 0.0) {                                     // Eqs. 13-14: max(mdot_BH, mdot_Tr) phi dt / V
+                const long long q = owned_index(P, i, j, k);
+                amt = fmax(amt, truelove_excess(P, U.rho[q], U.eint[q]));
+                ret_tr[q] = -CUDART_INF;                              // invalidate last step's entry (rewritten by the apply pass)
+            }
             double *dst = buf0 + ghost_index(P, i, j, k);
             atomicAdd(dst, -amt);                                     // R1: signed change
             if (REPRO) atomicAdd(dst + kChKsink * P.Nb, 1.0);         // Appendix A: contribution count
@@ -471,7 +478,8 @@ __global__ void __launch_bounds__(256) k_repro_round(const DevP P, double *__res
 // ---------------------------------------------------------------------------------------------------------------
 template <int VEC, bool LAM>
 __global__ void __launch_bounds__(256, 3) k_apply_limited(const DevP P, const DevState U, const double *__restrict__ buf,
-                                                       double *__restrict__ ret, double *__restrict__ lam_out,
+                                                       double *__restrict__ ret, double *__restrict__ ret_tr,
+                                                       double *__restrict__ lam_out,
                                                        unsigned int n_items, unsigned int items_per_row) {
     const unsigned int item_raw = blockIdx.x * blockDim.x + threadIdx.x;
     const bool valid = item_raw < n_items;
@@ -505,6 +513,7 @@ __global__ void __launch_bounds__(256, 3) k_apply_limited(const DevP P, const De
         double uc[6], bc[6], vold[3] = { 0.0, 0.0, 0.0 };
 #pragma unroll
         for (int f = 0; f < 6; ++f) { uc[f] = u[f][v]; bc[f] = b[f][v]; }
+        const double exc = ret_tr ? truelove_excess(P, uc[0], uc[5]) : 0.0;   // pre-step rho - rho_Tr (Eq. 14), for Step 4
         const double eta = apply_cell(P, uc, bc, &lam[v], vold);
 #pragma unroll
         for (int f = 0; f < 6; ++f) u[f][v] = uc[f];
@@ -512,6 +521,7 @@ __global__ void __launch_bounds__(256, 3) k_apply_limited(const DevP P, const De
             double2 *r = reinterpret_cast<double2 *>(ret + 4 * (q + v));      // one whole 32-byte sector per cell
             r[0] = make_double2(eta, vold[0]);
             r[1] = make_double2(vold[1], vold[2]);
+            if (ret_tr) ret_tr[q + v] = exc;
         }
     }
     if (!any) return;                           // lanes of a touched segment whose own cells are untouched
@@ -525,6 +535,7 @@ __global__ void __launch_bounds__(256, 3) k_apply_limited(const DevP P, const De
 // ---------------------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(128) k_return_sinks(const DevP P, const DevSinks S, const double dt,
                                                       const double *__restrict__ scal, const double *__restrict__ ret,
+                                                      const double *__restrict__ ret_tr,
                                                       const int *__restrict__ perm) {
     const long long w = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
     const int lane = threadIdx.x & 31;
@@ -542,9 +553,10 @@ __global__ void __launch_bounds__(128) k_return_sinks(const DevP P, const DevSin
         const double r2 = dist2(cell_centre(P.x0[0], i, P.dx) - xs, cell_centre(P.x0[1], j, P.dx) - ys,
                                 cell_centre(P.x0[2], k, P.dx) - zs);
         if (r2 <= P.rk2_sink) {
-            const double amt = sink_cell_amount(P, r2, r_acc, wsum, mdot, dt);
+            double amt = sink_cell_amount(P, r2, r_acc, wsum, mdot, dt);
+            const long long q = owned_index(P, i, j, k);
+            if (ret_tr) amt = fmax(amt, ret_tr[q]);     // Eq. 14 re-evaluated from the pre-step rho - rho_Tr kept by the apply pass
             if (amt > 0.0) {                     // amt == 0 deposits nothing, so the return mesh has no entry there
-                const long long q = owned_index(P, i, j, k);
                 const double2 r0 = reinterpret_cast<const double2 *>(ret + 4 * q)[0], r1 = reinterpret_cast<const double2 *>(ret + 4 * q)[1];
                 const double gain = r0.x * amt * P.V;
                 dm += gain;
@@ -593,6 +605,7 @@ extern "C" int pm_create(const pm_params *prm, int device, void *cuda_stream, pm
     if (prm->rk_sn > 0.0 && (prm->sn_nsub < 1 || prm->sn_nsub > 8)) return PM_EINVAL;
     if (prm->sn_regime < 0 || prm->sn_regime > 3) return PM_EINVAL;
     if (!(prm->f_max_remove >= 0.0 && prm->f_max_remove <= 1.0) || prm->rho_floor < 0.0) return PM_EINVAL;
+    if (!(prm->truelove_J >= 0.0) || (prm->truelove_J > 0.0 && !(prm->G > 0.0))) return PM_EINVAL;
     const int gs = prm->rk_sink > 0.0 ? ceil_div_pos(prm->rk_sink, prm->dx) : 0;
     const int gn = prm->rk_sn > 0.0 ? ceil_div_pos(prm->rk_sn, prm->dx) : 0;
     const int g = gs > gn ? gs : gn;
@@ -623,6 +636,7 @@ extern "C" int pm_create(const pm_params *prm, int device, void *cuda_stream, pm
     P.eps_k = prm->sn_eps_k; P.rm_ej = prm->sn_rm_ej; P.rm_mc = prm->sn_rm_mc;
     P.msf_c = prm->sn_msf_coeff; P.msf_e = prm->sn_msf_exp; P.psnr_c = prm->sn_psnr_coeff; P.psnr_e = prm->sn_psnr_exp;
     P.mu_h = prm->sn_mu_h; P.nh_unit = prm->sn_nh_unit; P.theta = prm->sn_eint_theta;
+    P.tl_num = prm->truelove_J * prm->truelove_J * 3.14159265358979323846; P.tl_den = prm->G * prm->dx * prm->dx;
     P.nsub3 = (double)P.nsub * (double)P.nsub * (double)P.nsub;
     const int sbm = (1 << kSbLog2) - 1;
     P.nsbx = (((prm->nx + 7) >> 3) + sbm) >> kSbLog2; P.nsby = (((prm->ny + 7) >> 3) + sbm) >> kSbLog2; P.nsbz = (((prm->nz + 7) >> 3) + sbm) >> kSbLog2;
@@ -640,6 +654,7 @@ extern "C" int pm_create(const pm_params *prm, int device, void *cuda_stream, pm
     c->nch = c->repro ? kReproChannels : kBufChannels;
     if (e == cudaSuccess) e = cudaMalloc(&c->buf, (size_t)c->nch * P.Nb * sizeof(double));
     if (e == cudaSuccess && gs > 0) e = cudaMalloc(&c->ret, (size_t)kRetWords * N * sizeof(double));
+    if (e == cudaSuccess && gs > 0 && P.tl_num > 0.0) e = cudaMalloc(&c->ret_tr, (size_t)N * sizeof(double));
     if (e == cudaSuccess && (prm->flags & PM_FLAG_DEBUG_LAMBDA)) e = cudaMalloc(&c->lam, (size_t)N * sizeof(double));
     if (e == cudaSuccess) e = cudaMalloc(&c->err_flag, sizeof(int));
     if (e == cudaSuccess) e = cudaMallocHost(&c->err_host, sizeof(int));
@@ -656,6 +671,7 @@ extern "C" int pm_create(const pm_params *prm, int device, void *cuda_stream, pm
         cudaGetLastError();
         if (c->buf) cudaFree(c->buf);
         if (c->ret) cudaFree(c->ret);
+        if (c->ret_tr) cudaFree(c->ret_tr);
         if (c->lam) cudaFree(c->lam);
         if (c->err_flag) cudaFree(c->err_flag);
         if (c->err_host) cudaFreeHost(c->err_host);
@@ -675,7 +691,7 @@ extern "C" int pm_destroy(pm_ctx *c) {
     if (!c) return PM_EINVAL;
     cudaSetDevice(c->device);
     cudaStreamSynchronize(c->stream);
-    double *ptrs[] = { c->buf, c->ret, c->lam, c->sink_scal, c->dbg_sink, c->dbg_sn, c->stg_state, c->stg_sinks, c->stg_sne };
+    double *ptrs[] = { c->buf, c->ret, c->ret_tr, c->lam, c->sink_scal, c->dbg_sink, c->dbg_sn, c->stg_state, c->stg_sinks, c->stg_sne };
     for (double *p : ptrs) if (p) cudaFree(p);
     if (c->timing)
         for (int k = 0; k < PM_NUM_KERNELS; ++k) { cudaEventDestroy(c->ev[k][0]); cudaEventDestroy(c->ev[k][1]); }
@@ -762,9 +778,9 @@ extern "C" int pm_deposit(pm_ctx *c, const pm_state *st, const pm_sinks *sk, con
         const unsigned blocks = (unsigned)((nk + 3) / 4);
         tick(c, PM_K_SINKS, 0);
         if (P.gs == 4 && !c->force_generic)
-            (c->repro ? k_deposit_sinks_g4<true> : k_deposit_sinks_g4<false>)<<<blocks, kFastSinkWarps * 32, 0, c->stream>>>(P, U, S, dt, c->buf, c->sink_scal, dbg ? c->dbg_sink : nullptr, c->err_flag, perm);
+            (c->repro ? k_deposit_sinks_g4<true> : k_deposit_sinks_g4<false>)<<<blocks, kFastSinkWarps * 32, 0, c->stream>>>(P, U, S, dt, c->buf, c->sink_scal, dbg ? c->dbg_sink : nullptr, c->err_flag, perm, c->ret_tr);
         else
-            (c->repro ? k_deposit_sinks<true> : k_deposit_sinks<false>)<<<blocks, 128, 0, c->stream>>>(P, U, S, dt, c->buf, c->sink_scal, dbg ? c->dbg_sink : nullptr, c->err_flag, perm);
+            (c->repro ? k_deposit_sinks<true> : k_deposit_sinks<false>)<<<blocks, 128, 0, c->stream>>>(P, U, S, dt, c->buf, c->sink_scal, dbg ? c->dbg_sink : nullptr, c->err_flag, perm, c->ret_tr);
         if ((rc = check_launch(c, "k_deposit_sinks")) != PM_OK) return rc;
         tick(c, PM_K_SINKS, 1);
     }
@@ -823,8 +839,8 @@ static void launch_apply(pm_ctx *c, const DevState &U) {
     const unsigned ipr = (unsigned)(P.nx / VEC);
     const unsigned n_items = (unsigned)(P.N / VEC);
     const unsigned blocks = (n_items + 255) / 256;
-    if (c->lam) k_apply_limited<VEC, true><<<blocks, 256, 0, c->stream>>>(P, U, c->buf, c->ret, c->lam, n_items, ipr);
-    else k_apply_limited<VEC, false><<<blocks, 256, 0, c->stream>>>(P, U, c->buf, c->ret, nullptr, n_items, ipr);
+    if (c->lam) k_apply_limited<VEC, true><<<blocks, 256, 0, c->stream>>>(P, U, c->buf, c->ret, c->ret_tr, c->lam, n_items, ipr);
+    else k_apply_limited<VEC, false><<<blocks, 256, 0, c->stream>>>(P, U, c->buf, c->ret, c->ret_tr, nullptr, n_items, ipr);
 }
 
 extern "C" int pm_apply_limited(pm_ctx *c, pm_state *st) {
@@ -857,9 +873,9 @@ extern "C" int pm_return_to_particles(pm_ctx *c, pm_sinks *sk) {
         const int *perm = c->bin_mem + c->n_sinks_dep + c->n_sne_dep;
         tick(c, PM_K_RETURN, 0);
         if (c->P.gs == 4 && !c->force_generic)
-            k_return_sinks_g4<<<blocks, kFastSinkWarps * 32, 0, c->stream>>>(c->P, S, c->dt, c->sink_scal, c->ret, perm);
+            k_return_sinks_g4<<<blocks, kFastSinkWarps * 32, 0, c->stream>>>(c->P, S, c->dt, c->sink_scal, c->ret, c->ret_tr, perm);
         else
-            k_return_sinks<<<blocks, 128, 0, c->stream>>>(c->P, S, c->dt, c->sink_scal, c->ret, perm);
+            k_return_sinks<<<blocks, 128, 0, c->stream>>>(c->P, S, c->dt, c->sink_scal, c->ret, c->ret_tr, perm);
         int rc = check_launch(c, "k_return_sinks");
         if (rc != PM_OK) return rc;
         tick(c, PM_K_RETURN, 1);

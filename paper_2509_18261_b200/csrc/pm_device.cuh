@@ -7,6 +7,7 @@
 #pragma once
 #include <cstdint>
 #include <cuda_runtime.h>
+#include <math_constants.h>
 
 namespace pm {
 
@@ -33,6 +34,8 @@ struct DevP {
     double G, gamma, cs_iso;
     double rk_sink, rk2_sink, rk_sn, rk2_sn;
     double lambda, fmax, rho_floor;
+    double tl_num, tl_den;   // Eq. 12: rho_Tr = ((tl_num c_s) c_s) / tl_den, tl_num = (J J) pi, tl_den = (G dx) dx -- the oracle's
+                             // operation order, so rho - rho_Tr is bit-identical; tl_num = 0: Truelove terms off
     double eps_k, rm_ej, rm_mc, msf_c, msf_e, psnr_c, psnr_e, mu_h, nh_unit, theta;
     double nsub3;
     int nsbx, nsby, nsbz;   // super-blocks (4x4x4 tiles of 8^3 cells) per axis: the bins particles are ordered by
@@ -116,7 +119,15 @@ __device__ __forceinline__ SinkScalars sink_scalars(const DevP &P, double sum_rh
     return s;
 }
 
-// Eq. 9, Eq. 11, Eq. 13 mass row (per unit volume), Truelove term off (R10)
+// Eq. 12: rho - rho_Tr of a cell, the amount per unit volume the Truelove condition asks to remove (Eq. 14 times
+// phi dt / V); -inf when the terms are off.
+__device__ __forceinline__ double truelove_excess(const DevP &P, double rho, double eint) {
+    if (!(P.tl_num > 0.0)) return -CUDART_INF;
+    const double cs = sound_speed(P, rho, eint);
+    return rho - ((P.tl_num * cs) * cs) / P.tl_den;
+}
+
+// Eq. 9, Eq. 11, Eq. 13 mass row (per unit volume); callers take max(this, truelove_excess) when Truelove is on
 __device__ __forceinline__ double sink_cell_amount(const DevP &P, double r2, double r_acc, double wsum, double mdot, double dt) {
     double w = exp(-r2 / (r_acc * r_acc));
     double phi = w / wsum;
@@ -246,6 +257,9 @@ __device__ __forceinline__ double apply_cell(const DevP &P, double u[6], const d
         double alim = a;
         const double cap = P.fmax * u[0];
         if (cap < alim) alim = cap;
+        const double need = truelove_excess(P, u[0], u[5]);   // Eq. 16: never leave the cell above rho_Tr ...
+        if (need > alim) alim = need;
+        if (alim > a) alim = a;                                //          ... but never remove more than was requested
         double room = u[0] - P.rho_floor;
         if (room < 0.0) room = 0.0;
         if (room < alim) alim = room;

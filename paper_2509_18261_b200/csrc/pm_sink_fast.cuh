@@ -107,7 +107,8 @@ template <bool REPRO>
 __global__ void __launch_bounds__(kFastSinkWarps * 32, kFastSinkMinBlocks) k_deposit_sinks_g4(const DevP P, const DevState U, const DevSinks S,
                                                                           const double dt, double *__restrict__ buf0,
                                                                           double *__restrict__ scal, double *__restrict__ dbg,
-                                                                          int *__restrict__ err, const int *__restrict__ perm) {
+                                                                          int *__restrict__ err, const int *__restrict__ perm,
+                                                                          double *__restrict__ ret_tr) {
     __shared__ SinkWarpSmem sm_all[kFastSinkWarps];
     const int wib = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const long long w = (long long)blockIdx.x * kFastSinkWarps + wib;
@@ -148,7 +149,13 @@ __global__ void __launch_bounds__(kFastSinkWarps * 32, kFastSinkMinBlocks) k_dep
     for (int i = lane; i < nm; i += 32) {
         const int code = sm.code[i];
         double *dst = sbuf + sink_ghosted(sm, code);
-        atomicAdd(dst, -(sink_weight(sm, code) * k));   // R1: signed
+        double amt = sink_weight(sm, code) * k;
+        if (P.tl_num > 0.0) {                           // Eqs. 13-14: max(mdot_BH, mdot_Tr) phi dt / V = max(a, rho - rho_Tr)
+            const int q = sink_owned(sm, code);
+            amt = fmax(amt, truelove_excess(P, U.rho[q], U.eint[q]));
+            ret_tr[q] = -CUDART_INF;                    // invalidate last step's entry; the apply pass rewrites it where mass is removed
+        }
+        atomicAdd(dst, -amt);                           // R1: signed
         if (REPRO) atomicAdd(dst + kChKsink * P.Nb, 1.0);   // Appendix A: contribution count (same-sign terms: T = |sum|)
     }
     if (lane == 0) {
@@ -164,6 +171,7 @@ __global__ void __launch_bounds__(kFastSinkWarps * 32, kFastSinkMinBlocks) k_dep
 __global__ void __launch_bounds__(kFastSinkWarps * 32, kFastSinkMinBlocks) k_return_sinks_g4(const DevP P, const DevSinks S, const double dt,
                                                                          const double *__restrict__ scal,
                                                                          const double *__restrict__ ret,
+                                                                         const double *__restrict__ ret_tr,
                                                                          const int *__restrict__ perm) {
     __shared__ SinkWarpSmem sm_all[kFastSinkWarps];
     const int wib = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -182,12 +190,13 @@ __global__ void __launch_bounds__(kFastSinkWarps * 32, kFastSinkMinBlocks) k_ret
 #pragma unroll 2
     for (int i = lane; i < nm; i += 32) {
         const int code = sm.code[i];
-        const double wgt = sink_weight(sm, code);
-        if (wgt * kV > 0.0) {                   // a == 0 deposited nothing, so the return mesh has no entry there
-            const int q = sink_owned(sm, code);
+        const int q = sink_owned(sm, code);
+        double aV = sink_weight(sm, code) * kV;                              // a V
+        if (ret_tr) aV = fmax(aV, ret_tr[q] * P.V);                          // Eq. 14 from the pre-step rho - rho_Tr
+        if (aV > 0.0) {                         // a == 0 deposited nothing, so the return mesh has no entry there
             const double2 *r = reinterpret_cast<const double2 *>(ret + 4 * (long long)q);   // (eta, v_old): one sector
             const double2 r0 = r[0], r1 = r[1];
-            const double gain = r0.x * (wgt * kV);
+            const double gain = r0.x * aV;
             dm += gain;
             dpx = fma(gain, r0.y, dpx);
             dpy = fma(gain, r1.x, dpy);

@@ -43,7 +43,7 @@ class PmParams(C.Structure):
         ("sn_msf_coeff", C.c_double), ("sn_msf_exp", C.c_double),
         ("sn_psnr_coeff", C.c_double), ("sn_psnr_exp", C.c_double),
         ("sn_mu_h", C.c_double), ("sn_nh_unit", C.c_double),
-        ("sn_eint_theta", C.c_double),
+        ("sn_eint_theta", C.c_double), ("truelove_J", C.c_double),
     ]
 
 
@@ -125,6 +125,8 @@ def make_params(p: dict, flags: int = 0) -> PmParams:
             o.flags = flags
         elif k == "x0":
             o.x0[0], o.x0[1], o.x0[2] = (float(v) for v in p["x0"])
+        elif k == "truelove_J":
+            o.truelove_J = float(p.get("truelove_J", 0.0))
         else:
             setattr(o, k, p[k])
     return o
