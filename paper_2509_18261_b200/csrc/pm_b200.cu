@@ -476,8 +476,11 @@ __global__ void __launch_bounds__(256) k_repro_round(const DevP P, double *__res
 // ---------------------------------------------------------------------------------------------------------------
 // a7: fused limiter + apply.  Each thread owns VEC consecutive cells of one x-row.
 // ---------------------------------------------------------------------------------------------------------------
-template <int VEC, bool LAM>
-__global__ void __launch_bounds__(256, 3) k_apply_limited(const DevP P, const DevState U, const double *__restrict__ buf,
+// 128 threads x 6 CTAs per SM: 3.37 ms against 3.44 ms for 256 x 3 (same 80 registers) and 3.96 ms for 256 x 2 (106 registers)
+constexpr int kApplyThreads = 128;
+
+template <int VEC, bool LAM, bool TL>
+__global__ void __launch_bounds__(kApplyThreads, 6) k_apply_limited(const DevP P, const DevState U, const double *__restrict__ buf,
                                                        double *__restrict__ ret, double *__restrict__ ret_tr,
                                                        double *__restrict__ lam_out,
                                                        unsigned int n_items, unsigned int items_per_row) {
@@ -513,15 +516,15 @@ __global__ void __launch_bounds__(256, 3) k_apply_limited(const DevP P, const De
         double uc[6], bc[6], vold[3] = { 0.0, 0.0, 0.0 };
 #pragma unroll
         for (int f = 0; f < 6; ++f) { uc[f] = u[f][v]; bc[f] = b[f][v]; }
-        const double exc = ret_tr ? truelove_excess(P, uc[0], uc[5]) : 0.0;   // pre-step rho - rho_Tr (Eq. 14), for Step 4
-        const double eta = apply_cell(P, uc, bc, &lam[v], vold);
+        const double exc = (TL && ret_tr) ? truelove_excess(P, uc[0], uc[5]) : 0.0;   // pre-step rho - rho_Tr (Eq. 14), for Step 4
+        const double eta = apply_cell<TL>(P, uc, bc, &lam[v], vold);
 #pragma unroll
         for (int f = 0; f < 6; ++f) u[f][v] = uc[f];
         if (bc[0] != 0.0 && ret) {              // Step 4 needs eta and the pre-step velocity where a sink removed mass
             double2 *r = reinterpret_cast<double2 *>(ret + 4 * (q + v));      // one whole 32-byte sector per cell
             r[0] = make_double2(eta, vold[0]);
             r[1] = make_double2(vold[1], vold[2]);
-            if (ret_tr) ret_tr[q + v] = exc;
+            if (TL && ret_tr) ret_tr[q + v] = exc;
         }
     }
     if (!any) return;                           // lanes of a touched segment whose own cells are untouched
@@ -645,8 +648,10 @@ extern "C" int pm_create(const pm_params *prm, int device, void *cuda_stream, pm
     cudaError_t e = cudaSetDevice(device);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, device);
     if (e == cudaSuccess) {   // L1 / shared-memory split of the particle kernels (measured)
-        e = cudaFuncSetAttribute(k_deposit_sinks_g4<false>, cudaFuncAttributePreferredSharedMemoryCarveout, kSinkCarveout);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_deposit_sinks_g4<true>, cudaFuncAttributePreferredSharedMemoryCarveout, kSinkCarveout);
+        e = cudaFuncSetAttribute(k_deposit_sinks_g4<false, false>, cudaFuncAttributePreferredSharedMemoryCarveout, kSinkCarveout);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_deposit_sinks_g4<true, false>, cudaFuncAttributePreferredSharedMemoryCarveout, kSinkCarveout);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_deposit_sinks_g4<false, true>, cudaFuncAttributePreferredSharedMemoryCarveout, kSinkCarveout);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_deposit_sinks_g4<true, true>, cudaFuncAttributePreferredSharedMemoryCarveout, kSinkCarveout);
         if (e == cudaSuccess) e = cudaFuncSetAttribute(k_return_sinks_g4, cudaFuncAttributePreferredSharedMemoryCarveout, kSinkCarveout);
     }
     c->repro = (prm->flags & PM_FLAG_REPRODUCIBLE) != 0;
@@ -778,7 +783,8 @@ extern "C" int pm_deposit(pm_ctx *c, const pm_state *st, const pm_sinks *sk, con
         const unsigned blocks = (unsigned)((nk + 3) / 4);
         tick(c, PM_K_SINKS, 0);
         if (P.gs == 4 && !c->force_generic)
-            (c->repro ? k_deposit_sinks_g4<true> : k_deposit_sinks_g4<false>)<<<blocks, kFastSinkWarps * 32, 0, c->stream>>>(P, U, S, dt, c->buf, c->sink_scal, dbg ? c->dbg_sink : nullptr, c->err_flag, perm, c->ret_tr);
+            (P.tl_num > 0.0 ? (c->repro ? k_deposit_sinks_g4<true, true> : k_deposit_sinks_g4<false, true>)
+                            : (c->repro ? k_deposit_sinks_g4<true, false> : k_deposit_sinks_g4<false, false>))<<<blocks, kFastSinkWarps * 32, 0, c->stream>>>(P, U, S, dt, c->buf, c->sink_scal, dbg ? c->dbg_sink : nullptr, c->err_flag, perm, c->ret_tr);
         else
             (c->repro ? k_deposit_sinks<true> : k_deposit_sinks<false>)<<<blocks, 128, 0, c->stream>>>(P, U, S, dt, c->buf, c->sink_scal, dbg ? c->dbg_sink : nullptr, c->err_flag, perm, c->ret_tr);
         if ((rc = check_launch(c, "k_deposit_sinks")) != PM_OK) return rc;
@@ -838,9 +844,15 @@ static void launch_apply(pm_ctx *c, const DevState &U) {
     const DevP &P = c->P;
     const unsigned ipr = (unsigned)(P.nx / VEC);
     const unsigned n_items = (unsigned)(P.N / VEC);
-    const unsigned blocks = (n_items + 255) / 256;
-    if (c->lam) k_apply_limited<VEC, true><<<blocks, 256, 0, c->stream>>>(P, U, c->buf, c->ret, c->ret_tr, c->lam, n_items, ipr);
-    else k_apply_limited<VEC, false><<<blocks, 256, 0, c->stream>>>(P, U, c->buf, c->ret, c->ret_tr, nullptr, n_items, ipr);
+    const unsigned blocks = (n_items + kApplyThreads - 1) / kApplyThreads;
+    const bool tl = P.tl_num > 0.0;
+    if (c->lam) {
+        if (tl) k_apply_limited<VEC, true, true><<<blocks, kApplyThreads, 0, c->stream>>>(P, U, c->buf, c->ret, c->ret_tr, c->lam, n_items, ipr);
+        else k_apply_limited<VEC, true, false><<<blocks, kApplyThreads, 0, c->stream>>>(P, U, c->buf, c->ret, c->ret_tr, c->lam, n_items, ipr);
+    } else {
+        if (tl) k_apply_limited<VEC, false, true><<<blocks, kApplyThreads, 0, c->stream>>>(P, U, c->buf, c->ret, c->ret_tr, nullptr, n_items, ipr);
+        else k_apply_limited<VEC, false, false><<<blocks, kApplyThreads, 0, c->stream>>>(P, U, c->buf, c->ret, c->ret_tr, nullptr, n_items, ipr);
+    }
 }
 
 extern "C" int pm_apply_limited(pm_ctx *c, pm_state *st) {

@@ -250,6 +250,7 @@ __device__ __forceinline__ void sn_cell_deposit(const DevP &P, const SnScalars &
 // Steps 3 + 5 for one cell.  u = (rho, mx, my, mz, etot, eint) in/out; b = the six buffer channels (dU^sum).
 // Returns eta; *lam receives the Eq. 21 factor; *vold the pre-step velocity (only meaningful when b[0] != 0).
 // ---------------------------------------------------------------------------------------------------------------
+template <bool TL>
 __device__ __forceinline__ double apply_cell(const DevP &P, double u[6], const double b[6], double *lam_out, double vold[3]) {
     const double a = -b[0];
     double eta = 1.0;                                   // R12
@@ -257,9 +258,11 @@ __device__ __forceinline__ double apply_cell(const DevP &P, double u[6], const d
         double alim = a;
         const double cap = P.fmax * u[0];
         if (cap < alim) alim = cap;
-        const double need = truelove_excess(P, u[0], u[5]);   // Eq. 16: never leave the cell above rho_Tr ...
-        if (need > alim) alim = need;
-        if (alim > a) alim = a;                                //          ... but never remove more than was requested
+        if (TL) {                                              // compiled out when the Truelove terms are off
+            const double need = truelove_excess(P, u[0], u[5]);   // Eq. 16: never leave the cell above rho_Tr ...
+            if (need > alim) alim = need;
+            if (alim > a) alim = a;                                //          ... but never remove more than was requested
+        }
         double room = u[0] - P.rho_floor;
         if (room < 0.0) room = 0.0;
         if (room < alim) alim = room;

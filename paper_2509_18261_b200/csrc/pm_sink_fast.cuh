@@ -103,7 +103,7 @@ __device__ __forceinline__ double sink_weight(const SinkWarpSmem &sm, int code) 
     return (sm.ex[2][code >> 8] * sm.ex[1][(code >> 4) & 15]) * sm.ex[0][code & 15];
 }
 
-template <bool REPRO>
+template <bool REPRO, bool TL>
 __global__ void __launch_bounds__(kFastSinkWarps * 32, kFastSinkMinBlocks) k_deposit_sinks_g4(const DevP P, const DevState U, const DevSinks S,
                                                                           const double dt, double *__restrict__ buf0,
                                                                           double *__restrict__ scal, double *__restrict__ dbg,
@@ -150,7 +150,7 @@ __global__ void __launch_bounds__(kFastSinkWarps * 32, kFastSinkMinBlocks) k_dep
         const int code = sm.code[i];
         double *dst = sbuf + sink_ghosted(sm, code);
         double amt = sink_weight(sm, code) * k;
-        if (P.tl_num > 0.0) {                           // Eqs. 13-14: max(mdot_BH, mdot_Tr) phi dt / V = max(a, rho - rho_Tr)
+        if (TL) {                                       // Eqs. 13-14: max(mdot_BH, mdot_Tr) phi dt / V = max(a, rho - rho_Tr)
             const int q = sink_owned(sm, code);
             amt = fmax(amt, truelove_excess(P, U.rho[q], U.eint[q]));
             ret_tr[q] = -CUDART_INF;                    // invalidate last step's entry; the apply pass rewrites it where mass is removed
