@@ -757,4 +757,60 @@ int32_t orc_sink_amounts(const orc_params *p, const orc_state *U, double xs, dou
     return n;
 }
 
+/* ------------------------------------------------------------------------------------------ */
+/* Sec. 3.1.2 sink particle creation (readings R38, R39 of DESIGN.md).       */
+/* A cell creates a sink if (i) rho > rho_Tr (Eq. 12), (ii) it is a STRICT local density        */
+/* maximum among the cells whose centres lie within r_K (rk_sink) of its own, periodic, and     */
+/* (iii) the retained accretion buffer is zero there ("forbidding sink particle creation in    */
+/* any cell within which dU_ijk is non-zero", L177).  The new sink sits at the cell centre      */
+/* with m = (rho - rho_Tr) V and momentum m v; the cell keeps v and its specific energies and   */
+/* drops to rho_Tr (L183).  All tests use the state as it is on entry; cells are visited in     */
+/* index order, so the output is ordered by cell index.  a0 = accretion d rho^sum (may be       */
+/* NULL: no sinks yet).  Returns the number found; at most max_new are written and applied.     */
+/* ------------------------------------------------------------------------------------------ */
+int64_t orc_create_sinks(const orc_params *p, orc_state *U, const double *a0, int64_t max_new,
+                         double *x, double *y, double *z, double *vx, double *vy, double *vz, double *m, int64_t *cells) {
+    const int64_t N = (int64_t)p->nx * p->ny * p->nz;
+    const double V = p->dx * p->dx * p->dx, rk2 = p->rk_sink * p->rk_sink;
+    const int g = kernel_halfwidth(p->rk_sink, p->dx);
+    int64_t n = 0;
+    unsigned char *flag = (unsigned char *)calloc((size_t)N, 1);
+    if (!flag) return -1;
+    for (int64_t k = 0; k < p->nz; ++k)
+        for (int64_t j = 0; j < p->ny; ++j)
+            for (int64_t i = 0; i < p->nx; ++i) {
+                const int64_t c = cell_index(p, i, j, k);
+                const double rho = U->rho[c];
+                if (!(rho > rho_truelove(p, rho, U->eint[c]))) continue;          /* (i)   */
+                if (a0 && a0[c] != 0.0) continue;                                  /* (iii) */
+                int is_max = 1;
+                for (int dk = -g; dk <= g && is_max; ++dk)
+                    for (int dj = -g; dj <= g && is_max; ++dj)
+                        for (int di = -g; di <= g; ++di) {
+                            if (!(di | dj | dk)) continue;
+                            const double ox = (double)di * p->dx, oy = (double)dj * p->dx, oz = (double)dk * p->dx;
+                            if (dist2(ox, oy, oz) > rk2) continue;
+                            if (!(U->rho[cell_index(p, i + di, j + dj, k + dk)] < rho)) { is_max = 0; break; }   /* (ii) */
+                        }
+                if (is_max) flag[c] = 1;
+            }
+    for (int64_t c = 0; c < N; ++c) {
+        if (!flag[c]) continue;
+        if (n < max_new) {
+            const int64_t i = c % p->nx, j = (c / p->nx) % p->ny, k = c / ((int64_t)p->nx * p->ny);
+            const double rho = U->rho[c], rtr = rho_truelove(p, rho, U->eint[c]);
+            const double ms = (rho - rtr) * V, keep = rtr / rho;
+            x[n] = cell_centre(p->x0[0], i, p->dx); y[n] = cell_centre(p->x0[1], j, p->dx); z[n] = cell_centre(p->x0[2], k, p->dx);
+            vx[n] = U->mx[c] / rho; vy[n] = U->my[c] / rho; vz[n] = U->mz[c] / rho;
+            m[n] = ms;
+            if (cells) cells[n] = c;
+            U->rho[c] = rtr;
+            U->mx[c] *= keep; U->my[c] *= keep; U->mz[c] *= keep; U->etot[c] *= keep; U->eint[c] *= keep;
+        }
+        n += 1;
+    }
+    free(flag);
+    return n;
+}
+
 int32_t orc_sizeof_params(void) { return (int32_t)sizeof(orc_params); }

@@ -105,6 +105,8 @@ def lib():
         L.orc_repro_round.argtypes = [C.c_double, C.c_double, C.c_int32, C.c_int32]
         L.orc_repro_buffers.restype = C.c_int
         L.orc_repro_buffers.argtypes = [C.POINTER(OrcParams), C.POINTER(OrcState), C.POINTER(OrcMeshOut), C.c_int32]
+        L.orc_create_sinks.restype = C.c_int64
+        L.orc_create_sinks.argtypes = [C.POINTER(OrcParams), C.POINTER(OrcState), c_dp, C.c_int64] + [c_dp] * 7 + [c_lp]
         L.orc_sample_cells.restype = C.c_int
         L.orc_sample_cells.argtypes = [C.POINTER(OrcParams), C.POINTER(OrcState), C.POINTER(OrcSinks), C.POINTER(OrcSNe),
                                        C.c_double, c_lp, C.c_int64, c_dp, c_dp, c_dp, c_dp, c_dp, c_dp, c_dp, c_ip]
@@ -248,6 +250,19 @@ class Oracle:
         else:
             rc = self.L.orc_step_repro(C.byref(self.p), C.byref(cs), C.byref(ck), C.byref(cn), dt, C.byref(cm), _dp(self._old), int(repro_M))
         assert rc == 0, f"orc_step rc={rc}"
+
+    def create_sinks(self, max_new: int, use_buffer: bool = True):
+        """Sec. 3.1.2 on the current state (and the retained accretion buffer A[0]).  Returns (n_found, dict of arrays)."""
+        out = {k: np.zeros(max_new) for k in ("x", "y", "z", "vx", "vy", "vz", "m")}
+        cells = np.zeros(max_new, dtype=np.int64)
+        cs = self._cstate()
+        n = self.L.orc_create_sinks(C.byref(self.p), C.byref(cs), _dp(self.A[0]) if use_buffer else C.cast(None, c_dp), max_new,
+                                    *(_dp(out[k]) for k in ("x", "y", "z", "vx", "vy", "vz", "m")), _lp(cells))
+        assert n >= 0
+        k = min(int(n), max_new)
+        res = {key: v[:k] for key, v in out.items()}
+        res["cells"] = cells[:k]
+        return int(n), res
 
     def repro_buffers(self, M: int):
         """Appendix A rounding of the deposited buffers (call between deposit() and apply())."""
