@@ -259,6 +259,23 @@ def run_ours(args, rank, world, local_rank):
         if it >= 2:
             ksamples.append(ctx.pm_kernel_times())
     kernel_ms = {k: float(np.median([s[k] for s in ksamples])) for k in pm.KERNEL_GROUPS}
+    # ---- row (f)2b, not part of the step: one sink-creation pass (Sec. 3.1.2) over the same mesh, on copies of the state ----
+    creation = None
+    if rank == 0 and world == 1 and not args.reproducible:
+        ptl = dict(w.params, truelove_J=1.5)
+        ctl = pm.Context(ptl, device=str(dev))
+        times, found = [], 0
+        for rep in range(3):
+            cp = pm.DeviceState(*(f.clone() for f in st.fields()))
+            torch.cuda.synchronize(dev)
+            t0 = time.perf_counter()
+            found, _ = ctl.pm_create_sinks(cp, 1 << 20)          # synchronises
+            times.append((time.perf_counter() - t0) * 1e3)
+            del cp
+        ctl.close()
+        creation = {"ms": min(times[1:]), "new_sinks": found, "truelove_J": 1.5,
+                    "algorithmic_bytes": 8.0 * 3 * N, "timing": "host clock around pm_create_sinks (it synchronises), best of 2 after a warm-up call"}
+        creation["achieved_gbs"] = creation["algorithmic_bytes"] / (creation["ms"] * 1e-3) / 1e9
     red_probe = None
     if rank == 0 and world == 1:
         red_probe = {"l2_resident_64MB_5ch": ctx.pm_probe_red_f64(64 << 20, 5),
@@ -326,6 +343,8 @@ def run_ours(args, rank, world, local_rank):
                               "frac_of_8tbs_nominal": step_bytes / (ms_per_step * 1e-3) / 1e9 / 8000.0,
                               "dense_survey_bytes": 8.0 * nch * Nb + 8.0 * 5 * N + 120.0 * npart + 144.0 * (Nb - N) + 176.0 * N + 32.0 * ts4 * N},
         }
+        if creation:
+            line["sink_creation"] = creation
         if red_probe:
             n_red = 5.0 * 183.0 * w.sne.n     # ~183 cells with omega > 0 per SN (SURVEY.md 8 probe), 5 channels
             red_probe["sn_deposit_achieved"] = n_red / (kernel_ms["sne"] * 1e-3) / 1e9 if kernel_ms["sne"] > 0 else None

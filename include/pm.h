@@ -123,6 +123,17 @@ int pm_return_to_particles(pm_ctx *ctx, pm_sinks *sinks);
 /* Margin M of Appendix A (N_bit = log2 r + 52 + M; default 28, the paper's example, L612).  Needs PM_FLAG_REPRODUCIBLE. */
 int pm_set_repro_margin(pm_ctx *ctx, int32_t M);
 
+/* Sink particle creation (Sec. 3.1.2); needs rk_sink > 0 and truelove_J > 0.  Call between steps (after
+ * pm_apply_limited / pm_return_to_particles, before the next pm_deposit).  A cell creates a sink if rho > rho_Tr (Eq. 12),
+ * it is a strict local density maximum among the cells whose centres lie within rk_sink of its own (periodic), and the
+ * accretion channel of the retained buffer mesh is zero there (no sink's kernel covers it, L177; before the first deposit
+ * this test is skipped).  New sink: cell centre, m = (rho - rho_Tr) V, velocity of the cell; the cell is left at rho_Tr
+ * with the same velocity and specific energies (L183).  state: DEVICE, modified in place.  x .. m: DEVICE arrays of
+ * max_new doubles, filled in increasing cell-index order.  *n_new (HOST) = number of cells found; if it exceeds max_new
+ * NOTHING is created and the state is unchanged (call again with larger arrays).  Synchronises. */
+int pm_create_sinks(pm_ctx *ctx, pm_state *state, int64_t max_new, double *x, double *y, double *z, double *vx, double *vy,
+                    double *vz, double *m, int64_t *n_new);
+
 /* Synchronise the ctx's stream and report PM_ECUDA / PM_EDOMAIN raised by earlier asynchronous work. */
 int pm_check(pm_ctx *ctx);
 

@@ -9,11 +9,14 @@
 //   k_return_sinks     a8  one warp per sink: sum eta a V (1, v_old) with a shuffle reduction
 #include "pm_device.cuh"
 #include "pm_fast.cuh"
+#include "pm_create.cuh"
 #include "../../include/pm.h"
 
 #include <cmath>
 #include <cstdio>
+#include <algorithm>
 #include <cstring>
+#include <vector>
 #include <new>
 
 using namespace pm;
@@ -57,6 +60,7 @@ struct pm_ctx {
     int *bin_mem;       long long bin_cap;
     int nch;            // buffer channels allocated: 6, or 10 with PM_FLAG_REPRODUCIBLE
     bool repro; int repro_M;
+    bool buffer_valid;  // a deposit + fold has filled the buffer mesh (sink creation reads its accretion channel)
     bool timing;        // PM_FLAG_TIMING
     cudaEvent_t ev[PM_NUM_KERNELS][2];
     bool ev_used[PM_NUM_KERNELS];
@@ -804,6 +808,7 @@ extern "C" int pm_deposit(pm_ctx *c, const pm_state *st, const pm_sinks *sk, con
     }
     c->n_sinks_dep = nk; c->n_sne_dep = nn; c->dt = dt;
     c->stage = ST_DEPOSITED;
+    c->buffer_valid = false;              // unfolded until pm_fold_ghosts
     return PM_OK;
 }
 
@@ -836,6 +841,7 @@ extern "C" int pm_fold_ghosts(pm_ctx *c) {
     tick(c, PM_K_FOLD, 1);
     if (rc != PM_OK) return rc;
     c->stage = ST_FOLDED;
+    c->buffer_valid = true;
     return PM_OK;
 }
 
@@ -894,6 +900,46 @@ extern "C" int pm_return_to_particles(pm_ctx *c, pm_sinks *sk) {
     }
     c->stage = ST_IDLE;
     return PM_OK;
+}
+
+extern "C" int pm_create_sinks(pm_ctx *c, pm_state *st, int64_t max_new, double *x, double *y, double *z, double *vx,
+                               double *vy, double *vz, double *m, int64_t *n_new) {
+    if (!c) return PM_EINVAL;
+    if (!n_new) PM_FAIL(c, PM_EINVAL, "pm_create_sinks: n_new is NULL");
+    *n_new = 0;
+    if (!state_ok(st)) PM_FAIL(c, PM_EINVAL, "pm_create_sinks: null state pointer");
+    if (c->P.gs == 0 || !(c->P.tl_num > 0.0)) PM_FAIL(c, PM_EINVAL, "pm_create_sinks needs rk_sink > 0 and truelove_J > 0");
+    if (c->stage == ST_DEPOSITED || c->stage == ST_FOLDED) PM_FAIL(c, PM_EORDER, "pm_create_sinks: finish the step (pm_apply_limited) first");
+    if (max_new < 0 || max_new >= (1ll << 31) || (max_new > 0 && !(x && y && z && vx && vy && vz && m))) PM_FAIL(c, PM_EINVAL, "pm_create_sinks: bad output arrays");
+    PM_CUDA(c, cudaSetDevice(c->device));
+    const DevP &P = c->P;
+    const int cap = (int)max_new;
+    int *d = nullptr;                                   // [0] = count, [1 .. cap] = list
+    PM_CUDA(c, cudaMalloc(&d, (size_t)(cap + 1) * sizeof(int)));
+    cudaError_t e = cudaMemsetAsync(d, 0, sizeof(int), c->stream);
+    const DevState U = { st->rho, st->mx, st->my, st->mz, st->etot, st->eint };
+    int rc = PM_OK, found = 0;
+    if (e == cudaSuccess) {
+        k_create_find<<<(unsigned)((P.N + 255) / 256), 256, 0, c->stream>>>(P, U, c->buffer_valid ? c->buf : nullptr, d + 1, cap, d);
+        rc = check_launch(c, "k_create_find");
+        e = cudaMemcpyAsync(&found, d, sizeof(int), cudaMemcpyDeviceToHost, c->stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+    }
+    if (e == cudaSuccess && rc == PM_OK && found > 0 && found <= cap) {
+        std::vector<int> cells((size_t)found);          // atomic append order -> cell-index order (the only host work)
+        e = cudaMemcpy(cells.data(), d + 1, (size_t)found * sizeof(int), cudaMemcpyDeviceToHost);
+        std::sort(cells.begin(), cells.end());
+        if (e == cudaSuccess) e = cudaMemcpyAsync(d + 1, cells.data(), (size_t)found * sizeof(int), cudaMemcpyHostToDevice, c->stream);
+        if (e == cudaSuccess) {
+            k_create_apply<<<(unsigned)((found + 127) / 128), 128, 0, c->stream>>>(P, U, d + 1, found, x, y, z, vx, vy, vz, m);
+            rc = check_launch(c, "k_create_apply");
+            e = cudaStreamSynchronize(c->stream);
+        }
+    }
+    cudaFree(d);
+    if (e != cudaSuccess) { snprintf(c->msg, sizeof(c->msg), "pm_create_sinks: %s", cudaGetErrorString(e)); return PM_ECUDA; }
+    *n_new = found;
+    return rc;
 }
 
 extern "C" int pm_check(pm_ctx *c) {

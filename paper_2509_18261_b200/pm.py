@@ -15,7 +15,7 @@ import torch
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libpm_b200.so")
 SRC = [os.path.join(_HERE, "csrc", "pm_b200.cu")]
-HDRS = [os.path.join(_HERE, "csrc", "pm_device.cuh"), os.path.join(_HERE, "csrc", "pm_fast.cuh"),
+HDRS = [os.path.join(_HERE, "csrc", "pm_device.cuh"), os.path.join(_HERE, "csrc", "pm_create.cuh"), os.path.join(_HERE, "csrc", "pm_fast.cuh"),
         os.path.join(_HERE, "csrc", "pm_sn_fast.cuh"), os.path.join(_HERE, "csrc", "pm_sink_fast.cuh"), os.path.join(os.path.dirname(_HERE), "include", "pm.h")]
 
 PM_OK, PM_EINVAL, PM_ENOMEM, PM_ECUDA, PM_EORDER, PM_EDOMAIN = 0, -1, -2, -3, -4, -5
@@ -24,7 +24,7 @@ KERNEL_GROUPS = ("bin", "zero", "sinks", "sne", "fold", "apply", "return")
 STATUS_NAMES = {0: "PM_OK", -1: "PM_EINVAL", -2: "PM_ENOMEM", -3: "PM_ECUDA", -4: "PM_EORDER", -5: "PM_EDOMAIN"}
 
 EXPORTS = ["pm_create", "pm_deposit", "pm_fold_ghosts", "pm_apply_limited", "pm_return_to_particles", "pm_check",
-           "pm_step_host", "pm_destroy", "pm_last_error", "pm_launch_count", "pm_kernel_times", "pm_probe_red_f64", "pm_set_repro_margin", "pm_debug_buffer",
+           "pm_step_host", "pm_destroy", "pm_last_error", "pm_launch_count", "pm_kernel_times", "pm_probe_red_f64", "pm_set_repro_margin", "pm_create_sinks", "pm_debug_buffer",
            "pm_debug_return_mesh", "pm_debug_lambda", "pm_debug_sink_scalars", "pm_debug_sn_scalars",
            "pm_debug_stencil"]
 
@@ -103,6 +103,7 @@ def lib():
         L.pm_launch_count.argtypes = [vp]
         L.pm_launch_count.restype = C.c_int64
         L.pm_set_repro_margin.argtypes = [vp, C.c_int32]
+        L.pm_create_sinks.argtypes = [vp, C.POINTER(PmState), C.c_int64] + [vp] * 7 + [i64p]
         L.pm_kernel_times.argtypes = [vp, C.POINTER(C.c_float), C.c_int32]
         L.pm_probe_red_f64.argtypes = [vp, C.c_int64, C.c_int32, C.POINTER(C.c_double)]
         L.pm_debug_buffer.argtypes = [vp, C.c_int, C.POINTER(vp), i64p, i64p, i32p]
@@ -288,6 +289,16 @@ class Context:
             for f in DeviceSNe.IN:
                 setattr(cn, f, hp(getattr(sn, f)))
         self._chk(self.L.pm_step_host(self.h, C.byref(cs), C.byref(ck), C.byref(cn), dt), "pm_step_host")
+
+    def pm_create_sinks(self, state: DeviceState, max_new: int):
+        """Sec. 3.1.2.  Returns (n_found, dict of device tensors x, y, z, vx, vy, vz, m of length min(n_found, max_new))."""
+        out = {k: torch.zeros(max(max_new, 1), dtype=torch.float64, device=self.device) for k in ("x", "y", "z", "vx", "vy", "vz", "m")}
+        n = C.c_int64(0)
+        cs = state.c()
+        self._chk(self.L.pm_create_sinks(self.h, C.byref(cs), int(max_new), *(out[k].data_ptr() for k in ("x", "y", "z", "vx", "vy", "vz", "m")),
+                                         C.byref(n)), "pm_create_sinks")
+        k = n.value if n.value <= max_new else 0
+        return int(n.value), {key: v[:k] for key, v in out.items()}
 
     def pm_set_repro_margin(self, M: int):
         self._chk(self.L.pm_set_repro_margin(self.h, int(M)), "pm_set_repro_margin")
