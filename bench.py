@@ -189,7 +189,10 @@ def run_ours(args, rank, world, local_rank):
         torch.cuda.synchronize(dev)
 
     n = args.n
-    if n == 512 and args.particles == 1_000_000:
+    if args.config is not None:             # one of the other BASELINE configs (parity-test workloads; not the headline line)
+        w = inputs.make(args.config)
+        n = int(w.params["nx"])
+    elif n == 512 and args.particles == 1_000_000:
         w = inputs.make(5)
     else:
         w = inputs.scaled_mixed(n, args.particles, seed_index=5)
@@ -200,8 +203,8 @@ def run_ours(args, rank, world, local_rank):
     nch = 10 if args.reproducible else 6
     ctx = pm.Context(w.params, device=str(dev), flags=mode)          # the timed steps run without the per-kernel events
     st = pm.DeviceState.from_host(w.state, dev)
-    sk = pm.DeviceSinks.from_host(w.sinks, dev)
-    sn = pm.DeviceSNe.from_host(w.sne, dev)
+    sk = pm.DeviceSinks.from_host(w.sinks, dev) if w.sinks.n else None
+    sn = pm.DeviceSNe.from_host(w.sne, dev) if w.sne.n else None
     stage_names = ("deposit", "fold", "apply", "return")
 
     def one_step(ev=None):
@@ -366,6 +369,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--n", type=int, default=512, help="cells per side (default: config 5)")
     ap.add_argument("--particles", type=int, default=1_000_000)
+    ap.add_argument("--config", type=int, default=None, choices=[1, 2, 3, 4, 5],
+                    help="time another BASELINE config instead of config 5 (for the table in DESIGN.md; the headline is config 5)")
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--reproducible", action="store_true",
