@@ -16,7 +16,8 @@ def test_truelove_mixed_workload_matches_oracle(flags, J):
     """Lognormal gas (sigma_ln = 1.5) with c_s = 1: rho_Tr = J^2 pi (2.0 / 0.64), so a good part of the sink-touched cells
     sit above it and take the Eq. 14 branch, the others the Bondi-Hoyle branch; three steps so that the return pass reads
     entries invalidated and rewritten across steps."""
-    w = inputs.scaled_mixed(40, 600, seed_index=5, n_clusters=3)
+    n = 40 if flags == 0 else 37                     # 37: odd row length, scalar apply / fold variants
+    w = inputs.scaled_mixed(n, 600, seed_index=5, n_clusters=3)
     w.params["truelove_J"] = J
     g = parity.GpuRun(w, flags=pm.PM_FLAG_DEBUG_SCALARS | pm.PM_FLAG_DEBUG_LAMBDA | flags)
     o = parity.make_oracle(w)
