@@ -42,18 +42,11 @@ __device__ __forceinline__ unsigned lanemask_lt() {
 __device__ __forceinline__ double pick3(int ax, double a, double b, double c) { return ax == 0 ? a : (ax == 1 ? b : c); }
 
 // The whole deposit of ONE supernova by one warp (all 32 lanes must call).  s = particle index; sm = this warp's shared
-// scratch; dec = the CTA's linear-box-index -> packed-code table (sn_fill_dec).
-__device__ __forceinline__ void sn_fill_dec(unsigned short *dec) {
-    for (int c = threadIdx.x; c < kSnCells; c += blockDim.x) {
-        const int a = c % 7, t = c / 7;
-        dec[c] = (unsigned short)(a | ((t % 7) << 3) | ((t / 7) << 6));
-    }
-}
-
+// scratch.
 template <bool REPRO>
 __device__ __forceinline__ void sn_deposit_one(const DevP &P, const DevState &U, const DevSNe &S, double *__restrict__ buf,
                                                double *__restrict__ dbg, int *__restrict__ err, const long long s,
-                                               SnWarpSmem &sm, const unsigned short *dec, const int lane) {
+                                               SnWarpSmem &sm, const int lane) {
     const double xs = S.x[s], ys = S.y[s], zs = S.z[s];
     const int ih = host_cell(xs, P.x0[0], P.inv_dx), jh = host_cell(ys, P.x0[1], P.inv_dx), kh = host_cell(zs, P.x0[2], P.inv_dx);
     if (ih < 0 || ih >= P.nx || jh < 0 || jh >= P.ny || kh < 0 || kh >= P.nz) {
@@ -94,25 +87,42 @@ __device__ __forceinline__ void sn_deposit_one(const DevP &P, const DevState &U,
         sm.dmax[ax][c] = fmax(fmax(v0, v1), fmax(v2, v3));
     }
     __syncwarp();
-    // ---- phase 1: classify the 343 cells; full -> 64, empty -> 0, boundary -> list ---------------------------------
+    // ---- phase 1: classify by ROWS (49 rows of 7 cells; this lane owns rows `lane` and `lane + 32`): two fp64 compares per
+    // cell give bit masks of the full and of the boundary cells; the boundary cells go to a list (any order)
     const double rk2 = P.rk2_sn;
-    int nb = 0;
-#pragma unroll 1
-    for (int r = 0; r < 11; ++r) {
-        const int c = lane + 32 * r;
-        bool boundary = false;
-        int pc = 0;
-        if (c < kSnCells) {
-            pc = dec[c];
-            const int a = pc & 7, b = (pc >> 3) & 7, cc = pc >> 6;
-            const bool full = (sm.dmax[2][cc] + sm.dmax[1][b]) + sm.dmax[0][a] <= rk2;
-            const bool empty = (sm.dmin[2][cc] + sm.dmin[1][b]) + sm.dmin[0][a] > rk2;
-            boundary = !full && !empty;
-            sm.cnt[pc] = full ? 64 : 0;
+    const int b0 = lane % 7, c0 = lane / 7;
+    const int b1 = (lane + 32) % 7, c1 = (lane + 32) / 7;
+    const bool has1 = lane < 17;
+    const int code0 = (b0 << 3) | (c0 << 6), code1 = (b1 << 3) | (c1 << 6);
+    unsigned fm0 = 0, bm0 = 0, fm1 = 0, bm1 = 0;
+    {
+        const double smax0 = sm.dmax[2][c0] + sm.dmax[1][b0], smin0 = sm.dmin[2][c0] + sm.dmin[1][b0];
+        const double smax1 = has1 ? sm.dmax[2][c1] + sm.dmax[1][b1] : 0.0, smin1 = has1 ? sm.dmin[2][c1] + sm.dmin[1][b1] : 0.0;
+#pragma unroll
+        for (int a = 0; a < 7; ++a) {
+            const double xmax = sm.dmax[0][a], xmin = sm.dmin[0][a];
+            const bool f0 = (smax0 + xmax) <= rk2, e0 = (smin0 + xmin) > rk2;
+            const bool f1 = (smax1 + xmax) <= rk2, e1 = (smin1 + xmin) > rk2;
+            fm0 |= (f0 ? 1u : 0u) << a; bm0 |= ((!f0 && !e0) ? 1u : 0u) << a;
+            fm1 |= (f1 ? 1u : 0u) << a; bm1 |= ((!f1 && !e1) ? 1u : 0u) << a;
         }
-        const unsigned m = __ballot_sync(0xffffffffu, boundary);
-        if (boundary) sm.list[nb + __popc(m & lanemask_lt())] = (unsigned short)pc;
-        nb += __popc(m);
+        if (!has1) { fm1 = 0; bm1 = 0; }
+    }
+    int nb;
+    {
+        const int mine = __popc(bm0) + __popc(bm1);
+        int incl = mine;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int v = __shfl_up_sync(0xffffffffu, incl, o);
+            if (lane >= o) incl += v;
+        }
+        nb = __shfl_sync(0xffffffffu, incl, 31);
+        int pos = incl - mine;
+#pragma unroll
+        for (int a = 0; a < 7; ++a) if (bm0 >> a & 1) sm.list[pos++] = (unsigned short)(code0 | a);
+#pragma unroll
+        for (int a = 0; a < 7; ++a) if (bm1 >> a & 1) sm.list[pos++] = (unsigned short)(code1 | a);
     }
     __syncwarp();
     // ---- phase 2: the 64 sub-sample tests of every boundary cell ---------------------------------------------------
@@ -135,16 +145,34 @@ __device__ __forceinline__ void sn_deposit_one(const DevP &P, const DevState &U,
         sm.cnt[pc] = (unsigned char)cnt;
     }
     __syncwarp();
-    // ---- phase 3: list of cells with omega > 0 -------------------------------------------------------------------
-    int na = 0;
-#pragma unroll 1
-    for (int r = 0; r < 11; ++r) {
-        const int c = lane + 32 * r;
-        const int pc = c < kSnCells ? dec[c] : 0;
-        const bool act = c < kSnCells && sm.cnt[pc] != 0;
-        const unsigned m = __ballot_sync(0xffffffffu, act);
-        if (act) sm.list[na + __popc(m & lanemask_lt())] = (unsigned short)pc;
-        na += __popc(m);
+    // ---- phase 3: list of cells with omega > 0, whole rows kept contiguous (rows 0..31, then rows 32..48); an entry is the
+    // packed code | (omega count - 1) << 9
+    int na;
+    {
+        unsigned k0[7], k1[7];                    // omega counts of this lane's cells (0: not active)
+        int n0 = 0, n1 = 0;
+#pragma unroll
+        for (int a = 0; a < 7; ++a) {
+            k0[a] = (fm0 >> a & 1) ? 64u : ((bm0 >> a & 1) ? sm.cnt[code0 | a] : 0u);
+            k1[a] = (fm1 >> a & 1) ? 64u : ((bm1 >> a & 1) ? sm.cnt[code1 | a] : 0u);
+            n0 += k0[a] != 0; n1 += k1[a] != 0;
+        }
+        const int mine = n0 | (n1 << 16);
+        int incl = mine;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int v = __shfl_up_sync(0xffffffffu, incl, o);
+            if (lane >= o) incl += v;
+        }
+        const int tot = __shfl_sync(0xffffffffu, incl, 31);
+        const int nA = tot & 0xffff;
+        na = nA + (tot >> 16);
+        int p0 = (incl - mine) & 0xffff, p1 = nA + ((incl - mine) >> 16);
+        __syncwarp();                             // phase 2's reads of the boundary list are done: reuse it
+#pragma unroll
+        for (int a = 0; a < 7; ++a) if (k0[a]) sm.list[p0++] = (unsigned short)(code0 | a | ((k0[a] - 1) << 9));
+#pragma unroll
+        for (int a = 0; a < 7; ++a) if (k1[a]) sm.list[p1++] = (unsigned short)(code1 | a | ((k1[a] - 1) << 9));
     }
     __syncwarp();
     // ---- phase 4: stencil sums (O4) --------------------------------------------------------------------------------
@@ -160,10 +188,10 @@ __device__ __forceinline__ void sn_deposit_one(const DevP &P, const DevState &U,
         for (int u = 0; u < kSnGatherBatch; ++u) {
             const int idx = base + 32 * u;
             const bool on = idx < na;
-            const int pc = on ? sm.list[idx] : 0;
-            const int a = pc & 7, b = (pc >> 3) & 7, cc = pc >> 6;
+            const int e = on ? sm.list[idx] : 0;
+            const int a = e & 7, b = (e >> 3) & 7, cc = (e >> 6) & 7;
             q[u] = on ? sm.off[2][cc] + sm.off[1][b] + sm.off[0][a] : 0;
-            wv[u] = on ? (double)sm.cnt[pc] * v64 : 0.0;                  // omega V; omega = count / 64 is exact
+            wv[u] = on ? (double)((e >> 9) + 1) * v64 : 0.0;              // omega V; omega = count / 64 is exact
         }
         double rho[kSnGatherBatch], mx[kSnGatherBatch], my[kSnGatherBatch], mz[kSnGatherBatch];
 #pragma unroll
@@ -187,9 +215,9 @@ __device__ __forceinline__ void sn_deposit_one(const DevP &P, const DevState &U,
     double *const sbuf = buf + P.Nb + (ih - 3 + P.gx);
 #pragma unroll 1
     for (int idx = lane; idx < na; idx += 32) {
-        const int pc = sm.list[idx];
-        const int a = pc & 7, b = (pc >> 3) & 7, cc = pc >> 6;
-        const double omega = (double)sm.cnt[pc] * (1.0 / 64.0);
+        const int e = sm.list[idx];
+        const int a = e & 7, b = (e >> 3) & 7, cc = (e >> 6) & 7;
+        const double omega = (double)((e >> 9) + 1) * (1.0 / 64.0);
         const int q = sm.off[2][cc] + sm.off[1][b] + sm.off[0][a];
         const double rho = U.rho[q], mx = U.mx[q], my = U.my[q], mz = U.mz[q];
         const double ddx = sm.dc[0][a], ddy = sm.dc[1][b], ddz = sm.dc[2][cc];
@@ -228,13 +256,10 @@ __global__ void __launch_bounds__(kFastSnWarps * 32, kFastSnMinBlocks) k_deposit
                                                                             double *__restrict__ buf, double *__restrict__ dbg,
                                                                             int *__restrict__ err, const int *__restrict__ perm) {
     __shared__ SnWarpSmem sm_all[kFastSnWarps];
-    __shared__ unsigned short dec[352];          // linear box index -> packed code, shared by the CTA
-    sn_fill_dec(dec);
-    __syncthreads();
     const int wib = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const long long w = (long long)blockIdx.x * kFastSnWarps + wib;
     if (w >= S.n) return;
-    sn_deposit_one<REPRO>(P, U, S, buf, dbg, err, perm[w], sm_all[wib], dec, lane);
+    sn_deposit_one<REPRO>(P, U, S, buf, dbg, err, perm[w], sm_all[wib], lane);
 }
 
 }  // namespace pm
