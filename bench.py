@@ -98,12 +98,17 @@ def measured_peak():
 
 
 def ncu_traffic(kernel: str):
-    """DRAM bytes per launch from the committed ncu --set full capture, if recorded (profiles/ncu_traffic.json)."""
+    """DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) from the committed ncu --set full capture,
+    profiles/r01_ncu_traffic.csv (made by the command in profiles/r01_ncu_full.md); None if not recorded."""
     try:
-        with open(os.path.join(ROOT, "profiles", "ncu_traffic.json")) as f:
-            return json.load(f).get(kernel)
+        with open(os.path.join(ROOT, "profiles", "r01_ncu_traffic.csv")) as f:
+            for ln in f.read().splitlines()[1:]:
+                k, v = ln.split(",")
+                if k == kernel:
+                    return float(v)
     except Exception:
-        return None
+        pass
+    return None
 
 
 # ---------------------------------------------------------------------------------------------
