@@ -129,8 +129,9 @@ int pm_set_repro_margin(pm_ctx *ctx, int32_t M);
  * accretion channel of the retained buffer mesh is zero there (no sink's kernel covers it, L177; before the first deposit
  * this test is skipped).  New sink: cell centre, m = (rho - rho_Tr) V, velocity of the cell; the cell is left at rho_Tr
  * with the same velocity and specific energies (L183).  state: DEVICE, modified in place.  x .. m: DEVICE arrays of
- * max_new doubles, filled in increasing cell-index order.  *n_new (HOST) = number of cells found; if it exceeds max_new
- * NOTHING is created and the state is unchanged (call again with larger arrays).  Synchronises. */
+ * max_new doubles, filled in increasing cell-index order (an ordered compaction on the device; only the count goes to
+ * the host).  *n_new (HOST) = number of cells found; if it exceeds max_new NOTHING is created and the state is unchanged
+ * (call again with larger arrays).  Synchronises. */
 int pm_create_sinks(pm_ctx *ctx, pm_state *state, int64_t max_new, double *x, double *y, double *z, double *vx, double *vy,
                     double *vz, double *m, int64_t *n_new);
 

@@ -14,9 +14,7 @@
 
 #include <cmath>
 #include <cstdio>
-#include <algorithm>
 #include <cstring>
-#include <vector>
 #include <new>
 
 using namespace pm;
@@ -60,6 +58,7 @@ struct pm_ctx {
     int *bin_mem;       long long bin_cap;
     int nch;            // buffer channels allocated: 6, or 10 with PM_FLAG_REPRODUCIBLE
     bool repro; int repro_M;
+    int *create_mem; long long create_cap;   // sink creation scratch: [0] = count, [1 ..] = list
     bool buffer_valid;  // a deposit + fold has filled the buffer mesh (sink creation reads its accretion channel)
     bool timing;        // PM_FLAG_TIMING
     cudaEvent_t ev[PM_NUM_KERNELS][2];
@@ -666,7 +665,7 @@ extern "C" int pm_create(const pm_params *prm, int device, void *cuda_stream, pm
     if (e == cudaSuccess && gs > 0 && P.tl_num > 0.0) e = cudaMalloc(&c->ret_tr, (size_t)N * sizeof(double));
     if (e == cudaSuccess && (prm->flags & PM_FLAG_DEBUG_LAMBDA)) e = cudaMalloc(&c->lam, (size_t)N * sizeof(double));
     if (e == cudaSuccess) e = cudaMalloc(&c->err_flag, sizeof(int));
-    if (e == cudaSuccess) e = cudaMallocHost(&c->err_host, sizeof(int));
+    if (e == cudaSuccess) e = cudaMallocHost(&c->err_host, 2 * sizeof(int));   // [0] error flag, [1] sink-creation count
     if (e == cudaSuccess) e = cudaMemsetAsync(c->err_flag, 0, sizeof(int), c->stream);
     if (e == cudaSuccess && c->ret) e = cudaMemsetAsync(c->ret, 0, (size_t)kRetWords * N * sizeof(double), c->stream);
     if (e == cudaSuccess) {
@@ -705,6 +704,7 @@ extern "C" int pm_destroy(pm_ctx *c) {
     if (c->timing)
         for (int k = 0; k < PM_NUM_KERNELS; ++k) { cudaEventDestroy(c->ev[k][0]); cudaEventDestroy(c->ev[k][1]); }
     if (c->bin_mem) cudaFree(c->bin_mem);
+    if (c->create_mem) cudaFree(c->create_mem);
     if (c->err_flag) cudaFree(c->err_flag);
     if (c->err_host) cudaFreeHost(c->err_host);
     delete c;
@@ -914,32 +914,37 @@ extern "C" int pm_create_sinks(pm_ctx *c, pm_state *st, int64_t max_new, double 
     PM_CUDA(c, cudaSetDevice(c->device));
     const DevP &P = c->P;
     const int cap = (int)max_new;
-    int *d = nullptr;                                   // [0] = count, [1 .. cap] = list
-    PM_CUDA(c, cudaMalloc(&d, (size_t)(cap + 1) * sizeof(int)));
-    cudaError_t e = cudaMemsetAsync(d, 0, sizeof(int), c->stream);
+    const int nblocks = (int)((P.N + 255) / 256), nscan = (nblocks + kScanChunk - 1) / kScanChunk;
+    // scratch (ints): total | block counts [nblocks] | chunk sums [nscan] | list [cap]; then the flags (bytes, one per cell)
+    const long long need = 1 + (long long)nblocks + nscan + cap + (P.N + 3) / 4;
+    if (need > c->create_cap) {
+        if (c->create_mem) { PM_CUDA(c, cudaFree(c->create_mem)); c->create_mem = nullptr; c->create_cap = 0; }
+        PM_CUDA(c, cudaMalloc(&c->create_mem, (size_t)need * sizeof(int)));
+        c->create_cap = need;
+    }
+    int *total = c->create_mem, *bcount = total + 1, *sums = bcount + nblocks, *list = sums + nscan;
+    unsigned char *flag = reinterpret_cast<unsigned char *>(list + cap);
     const DevState U = { st->rho, st->mx, st->my, st->mz, st->etot, st->eint };
-    int rc = PM_OK, found = 0;
-    if (e == cudaSuccess) {
-        k_create_find<<<(unsigned)((P.N + 255) / 256), 256, 0, c->stream>>>(P, U, c->buffer_valid ? c->buf : nullptr, d + 1, cap, d);
-        rc = check_launch(c, "k_create_find");
-        e = cudaMemcpyAsync(&found, d, sizeof(int), cudaMemcpyDeviceToHost, c->stream);
-        if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+    int rc;
+    PM_CUDA(c, cudaMemsetAsync(total, 0, (size_t)(1 + nblocks) * sizeof(int), c->stream));
+    k_create_find<<<nblocks, 256, 0, c->stream>>>(P, U, c->buffer_valid ? c->buf : nullptr, flag, bcount);
+    if ((rc = check_launch(c, "k_create_find")) != PM_OK) return rc;
+    k_bin_scan_local<<<nscan, 256, 0, c->stream>>>(bcount, nblocks, sums);
+    if ((rc = check_launch(c, "k_bin_scan_local")) != PM_OK) return rc;
+    k_bin_scan_sums<<<1, 1024, 0, c->stream>>>(sums, nscan);
+    if ((rc = check_launch(c, "k_bin_scan_sums")) != PM_OK) return rc;
+    k_create_compact<<<nblocks, 256, 0, c->stream>>>(P.N, flag, bcount, sums, kScanChunk, list, cap, total);
+    if ((rc = check_launch(c, "k_create_compact")) != PM_OK) return rc;
+    PM_CUDA(c, cudaMemcpyAsync(c->err_host + 1, total, sizeof(int), cudaMemcpyDeviceToHost, c->stream));   // the only host traffic
+    PM_CUDA(c, cudaStreamSynchronize(c->stream));
+    const int found = c->err_host[1];
+    if (found > 0 && found <= cap) {
+        k_create_apply<<<(unsigned)((found + 127) / 128), 128, 0, c->stream>>>(P, U, list, found, x, y, z, vx, vy, vz, m);
+        if ((rc = check_launch(c, "k_create_apply")) != PM_OK) return rc;
+        PM_CUDA(c, cudaStreamSynchronize(c->stream));
     }
-    if (e == cudaSuccess && rc == PM_OK && found > 0 && found <= cap) {
-        std::vector<int> cells((size_t)found);          // atomic append order -> cell-index order (the only host work)
-        e = cudaMemcpy(cells.data(), d + 1, (size_t)found * sizeof(int), cudaMemcpyDeviceToHost);
-        std::sort(cells.begin(), cells.end());
-        if (e == cudaSuccess) e = cudaMemcpyAsync(d + 1, cells.data(), (size_t)found * sizeof(int), cudaMemcpyHostToDevice, c->stream);
-        if (e == cudaSuccess) {
-            k_create_apply<<<(unsigned)((found + 127) / 128), 128, 0, c->stream>>>(P, U, d + 1, found, x, y, z, vx, vy, vz, m);
-            rc = check_launch(c, "k_create_apply");
-            e = cudaStreamSynchronize(c->stream);
-        }
-    }
-    cudaFree(d);
-    if (e != cudaSuccess) { snprintf(c->msg, sizeof(c->msg), "pm_create_sinks: %s", cudaGetErrorString(e)); return PM_ECUDA; }
     *n_new = found;
-    return rc;
+    return PM_OK;
 }
 
 extern "C" int pm_check(pm_ctx *c) {
