@@ -78,9 +78,9 @@ enum {
     PM_FLAG_DEBUG_LAMBDA = 2,    /* keep the Eq. 21 lambda of every cell (pm_debug_lambda) */
     PM_FLAG_GENERIC_KERNELS = 4, /* always use the generic (any radius, any n_sub) deposit / return kernels */
     PM_FLAG_TIMING = 8,          /* bracket every kernel with CUDA events on the ctx's stream (pm_kernel_times) */
-    PM_FLAG_REPRODUCIBLE = 16    /* Appendix A (L586-615): four more buffer channels (error scales, contribution counts) and a
-                                  * rounding pass at the end of pm_fold_ghosts: buffers no longer depend on the order of the
-                                  * atomic additions, except with probability ~2^-M per cell */
+    PM_FLAG_REPRODUCIBLE = 16    /* Appendix A (L586-615): four more buffer channels (error scales, contribution counts); the apply
+                                  * pass rounds the folded sums as it reads them: the step no longer depends on the order of
+                                  * the atomic additions, except with probability ~2^-M per cell */
 };
 
 typedef struct { double *rho, *mx, *my, *mz, *etot, *eint; } pm_state;
@@ -176,6 +176,11 @@ int pm_debug_buffer(pm_ctx *ctx, int channel, const double **dev_ptr, int64_t di
 /* Return mesh: one record of 4 doubles per cell (eta of Eq. 4, pre-step velocity x, y, z), valid where buffer channel
  * 0 != 0.  *dev_ptr points at word `word` of cell 0; the same word of cell q is at dev_ptr[4 q]. */
 int pm_debug_return_mesh(pm_ctx *ctx, int word, const double **dev_ptr);
+
+/* PM_FLAG_REPRODUCIBLE only: apply the Appendix A rounding to the folded buffers in place (call after pm_fold_ghosts), so that
+ * pm_debug_buffer shows the values the apply pass will use.  In the timed path the apply pass rounds the sums as it
+ * reads them and the buffers keep the unrounded sums; the rounding is idempotent, so calling this first changes nothing. */
+int pm_debug_round_buffers(pm_ctx *ctx);
 
 /* lambda of Eq. 21 per cell (needs PM_FLAG_DEBUG_LAMBDA). */
 int pm_debug_lambda(pm_ctx *ctx, const double **dev_ptr);

@@ -482,10 +482,10 @@ __global__ void __launch_bounds__(256) k_repro_round(const DevP P, double *__res
 // 128 threads x 6 CTAs per SM: 3.37 ms against 3.44 ms for 256 x 3 (same 80 registers) and 3.96 ms for 256 x 2 (106 registers)
 constexpr int kApplyThreads = 128;
 
-template <int VEC, bool LAM, bool TL>
+template <int VEC, bool LAM, bool TL, bool REPRO>
 __global__ void __launch_bounds__(kApplyThreads, 6) k_apply_limited(const DevP P, const DevState U, const double *__restrict__ buf,
                                                        double *__restrict__ ret, double *__restrict__ ret_tr,
-                                                       double *__restrict__ lam_out,
+                                                       double *__restrict__ lam_out, const int repro_M,
                                                        unsigned int n_items, unsigned int items_per_row) {
     const unsigned int item_raw = blockIdx.x * blockDim.x + threadIdx.x;
     const bool valid = item_raw < n_items;
@@ -498,6 +498,22 @@ __global__ void __launch_bounds__(kApplyThreads, 6) k_apply_limited(const DevP P
     double b[kBufChannels][VEC];
 #pragma unroll
     for (int ch = 0; ch < kBufChannels; ++ch) ldv<VEC>(buf + (long long)ch * P.Nb + gq, b[ch]);
+    if (REPRO) {   // Appendix A: round the folded sums here, where they are read anyway (rounding never turns a non-zero sum into zero)
+        double ksn[VEC], ksk[VEC], tp[VEC], te[VEC];
+        ldv<VEC>(buf + (long long)kChKsn * P.Nb + gq, ksn);
+        ldv<VEC>(buf + (long long)kChKsink * P.Nb + gq, ksk);
+        ldv<VEC>(buf + (long long)kChTp * P.Nb + gq, tp);
+        ldv<VEC>(buf + (long long)kChTe * P.Nb + gq, te);
+#pragma unroll
+        for (int v = 0; v < VEC; ++v) {
+            b[0][v] = repro_round(b[0][v], fabs(b[0][v]), ksk[v], repro_M);
+            b[1][v] = repro_round(b[1][v], fabs(b[1][v]), ksn[v], repro_M);
+            b[2][v] = repro_round(b[2][v], tp[v], ksn[v], repro_M);
+            b[3][v] = repro_round(b[3][v], tp[v], ksn[v], repro_M);
+            b[4][v] = repro_round(b[4][v], tp[v], ksn[v], repro_M);
+            b[5][v] = repro_round(b[5][v], te[v], ksn[v], repro_M);
+        }
+    }
     bool any = false;
 #pragma unroll
     for (int ch = 0; ch < kBufChannels; ++ch)
@@ -833,11 +849,6 @@ extern "C" int pm_fold_ghosts(pm_ctx *c) {
         else k_fold_ghosts<1, kBufChannels><<<blocks, 256, 0, c->stream>>>(P, c->buf, n_edge, n_z, n_y);
     }
     int rc = check_launch(c, "k_fold_ghosts");
-    if (rc == PM_OK && c->repro) {      // Appendix A: round the folded sums (error scales and counts were folded with them)
-        if (P.nx % 2 == 0) k_repro_round<2><<<(unsigned)((P.N / 2 + 255) / 256), 256, 0, c->stream>>>(P, c->buf, c->repro_M, P.N / 2);
-        else k_repro_round<1><<<(unsigned)((P.N + 255) / 256), 256, 0, c->stream>>>(P, c->buf, c->repro_M, P.N);
-        rc = check_launch(c, "k_repro_round");
-    }
     tick(c, PM_K_FOLD, 1);
     if (rc != PM_OK) return rc;
     c->stage = ST_FOLDED;
@@ -852,13 +863,17 @@ static void launch_apply(pm_ctx *c, const DevState &U) {
     const unsigned n_items = (unsigned)(P.N / VEC);
     const unsigned blocks = (n_items + kApplyThreads - 1) / kApplyThreads;
     const bool tl = P.tl_num > 0.0;
+#define PM_APPLY(LAM_, TL_, REPRO_, lamptr)                                                                                   \
+    k_apply_limited<VEC, LAM_, TL_, REPRO_><<<blocks, kApplyThreads, 0, c->stream>>>(P, U, c->buf, c->ret, c->ret_tr, lamptr, \
+                                                                                     c->repro_M, n_items, ipr)
     if (c->lam) {
-        if (tl) k_apply_limited<VEC, true, true><<<blocks, kApplyThreads, 0, c->stream>>>(P, U, c->buf, c->ret, c->ret_tr, c->lam, n_items, ipr);
-        else k_apply_limited<VEC, true, false><<<blocks, kApplyThreads, 0, c->stream>>>(P, U, c->buf, c->ret, c->ret_tr, c->lam, n_items, ipr);
+        if (c->repro) { if (tl) PM_APPLY(true, true, true, c->lam); else PM_APPLY(true, false, true, c->lam); }
+        else { if (tl) PM_APPLY(true, true, false, c->lam); else PM_APPLY(true, false, false, c->lam); }
     } else {
-        if (tl) k_apply_limited<VEC, false, true><<<blocks, kApplyThreads, 0, c->stream>>>(P, U, c->buf, c->ret, c->ret_tr, nullptr, n_items, ipr);
-        else k_apply_limited<VEC, false, false><<<blocks, kApplyThreads, 0, c->stream>>>(P, U, c->buf, c->ret, c->ret_tr, nullptr, n_items, ipr);
+        if (c->repro) { if (tl) PM_APPLY(false, true, true, nullptr); else PM_APPLY(false, false, true, nullptr); }
+        else { if (tl) PM_APPLY(false, true, false, nullptr); else PM_APPLY(false, false, false, nullptr); }
     }
+#undef PM_APPLY
 }
 
 extern "C" int pm_apply_limited(pm_ctx *c, pm_state *st) {
@@ -1021,6 +1036,17 @@ extern "C" int pm_debug_return_mesh(pm_ctx *c, int word, const double **dev_ptr)
     if (!c || !dev_ptr || word < 0 || word >= kRetWords || !c->ret) return PM_EINVAL;
     *dev_ptr = c->ret + word;          // record of cell q at 4 q: stride kRetWords between cells
     return PM_OK;
+}
+
+extern "C" int pm_debug_round_buffers(pm_ctx *c) {
+    if (!c) return PM_EINVAL;
+    if (!c->repro) PM_FAIL(c, PM_EINVAL, "pm_debug_round_buffers needs PM_FLAG_REPRODUCIBLE");
+    if (!c->buffer_valid) PM_FAIL(c, PM_EORDER, "pm_debug_round_buffers: fold first");
+    PM_CUDA(c, cudaSetDevice(c->device));
+    const DevP &P = c->P;
+    if (P.nx % 2 == 0) k_repro_round<2><<<(unsigned)((P.N / 2 + 255) / 256), 256, 0, c->stream>>>(P, c->buf, c->repro_M, P.N / 2);
+    else k_repro_round<1><<<(unsigned)((P.N + 255) / 256), 256, 0, c->stream>>>(P, c->buf, c->repro_M, P.N);
+    return check_launch(c, "k_repro_round");
 }
 
 extern "C" int pm_debug_lambda(pm_ctx *c, const double **dev_ptr) {

@@ -24,7 +24,7 @@ KERNEL_GROUPS = ("bin", "zero", "sinks", "sne", "fold", "apply", "return")
 STATUS_NAMES = {0: "PM_OK", -1: "PM_EINVAL", -2: "PM_ENOMEM", -3: "PM_ECUDA", -4: "PM_EORDER", -5: "PM_EDOMAIN"}
 
 EXPORTS = ["pm_create", "pm_deposit", "pm_fold_ghosts", "pm_apply_limited", "pm_return_to_particles", "pm_check",
-           "pm_step_host", "pm_destroy", "pm_last_error", "pm_launch_count", "pm_kernel_times", "pm_probe_red_f64", "pm_set_repro_margin", "pm_create_sinks", "pm_debug_buffer",
+           "pm_step_host", "pm_destroy", "pm_last_error", "pm_launch_count", "pm_kernel_times", "pm_probe_red_f64", "pm_set_repro_margin", "pm_create_sinks", "pm_debug_round_buffers", "pm_debug_buffer",
            "pm_debug_return_mesh", "pm_debug_lambda", "pm_debug_sink_scalars", "pm_debug_sn_scalars",
            "pm_debug_stencil"]
 
@@ -106,6 +106,7 @@ def lib():
         L.pm_create_sinks.argtypes = [vp, C.POINTER(PmState), C.c_int64] + [vp] * 7 + [i64p]
         L.pm_kernel_times.argtypes = [vp, C.POINTER(C.c_float), C.c_int32]
         L.pm_probe_red_f64.argtypes = [vp, C.c_int64, C.c_int32, C.POINTER(C.c_double)]
+        L.pm_debug_round_buffers.argtypes = [vp]
         L.pm_debug_buffer.argtypes = [vp, C.c_int, C.POINTER(vp), i64p, i64p, i32p]
         L.pm_debug_return_mesh.argtypes = [vp, C.c_int, C.POINTER(vp)]
         L.pm_debug_lambda.argtypes = [vp, C.POINTER(vp)]
@@ -318,6 +319,9 @@ class Context:
         return int(self.L.pm_launch_count(self.h))
 
     # ---- test-only views ------------------------------------------------------------------------
+    def pm_debug_round_buffers(self):
+        self._chk(self.L.pm_debug_round_buffers(self.h), "pm_debug_round_buffers")
+
     def debug_buffer(self, channel: int):
         """Returns (ghosted tensor (nz+2g, ny+2g, pitch), owned view (nz, ny, nx), g)."""
         ptr = C.c_void_p()

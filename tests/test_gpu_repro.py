@@ -23,13 +23,18 @@ def _permuted(w, seed):
     return w2, pk, pn
 
 
-def _run(w, flags, steps=1):
+def _run(w, flags, steps=1, view_buffers=True):
+    """view_buffers: round the folded buffers in place (pm_debug_round_buffers) at step 0 and copy them out.  In the product
+    path the apply pass rounds the sums as it reads them and the buffers stay unrounded; the rounding is idempotent, so
+    both ways must leave the same state (checked below), and every later step runs the product path only."""
     g = parity.GpuRun(w, flags=FLAGS | flags)
     bufs = None
     for it in range(steps):
         g.ctx.pm_deposit(g.state, g.sinks, g.sne, w.dt)
         g.ctx.pm_fold_ghosts()
-        if it == 0:
+        if it == 0 and view_buffers:
+            if flags & pm.PM_FLAG_REPRODUCIBLE:
+                g.ctx.pm_debug_round_buffers()
             bufs = [g.owned_buffer(ch).copy() for ch in range(6)]
         g.ctx.pm_apply_limited(g.state)
         g.ctx.pm_return_to_particles(g.sinks)
@@ -52,6 +57,11 @@ def test_particle_order_does_not_change_a_bit(flags, n):
         assert np.array_equal(fa, fb)
     assert np.array_equal(ga.sinks.m.cpu().numpy()[pk], gb.sinks.m.cpu().numpy())
     assert np.array_equal(ga.sinks.vx.cpu().numpy()[pk], gb.sinks.vx.cpu().numpy())
+    # the product path alone (rounding inside the apply pass, buffers never rounded in place) gives the same bits
+    gc, _ = _run(w2, pm.PM_FLAG_REPRODUCIBLE | flags, steps=2, view_buffers=False)
+    for fa, fc in zip(ga.state_np(), gc.state_np()):
+        assert np.array_equal(fa, fc)
+    assert np.array_equal(gb.sinks.m.cpu().numpy(), gc.sinks.m.cpu().numpy())
 
 
 def test_without_the_flag_the_order_shows():
@@ -107,19 +117,24 @@ def test_margin_setter_and_errors():
 
 
 def test_full_size_reproducible_step_twice_identical():
-    """Config 5 (512^3, 10^6 particles) in the launch configuration bench.py --reproducible times: two independent runs of the
-    same step (different atomic order, as always) leave bit-identical buffers and state."""
+    """Config 5 (512^3, 10^6 particles) in the launch configuration bench.py --reproducible times: independent runs of the
+    same step (different atomic order, as always) give bit-identical rounded buffers and a bit-identical state (momentum,
+    internal energy, sink masses).  Runs 0 and 1 round the buffers in place to look at them; run 2 is the product path
+    alone (rounding inside the apply pass)."""
     w = inputs.make(5)
     dev = torch.device("cuda:0")
     outs = []
-    for rep in range(2):
+    for rep in range(3):
         ctx = pm.Context(w.params, device="cuda:0", flags=pm.PM_FLAG_REPRODUCIBLE)
         st = pm.DeviceState.from_host(w.state, dev)
         sk = pm.DeviceSinks.from_host(w.sinks, dev)
         sn = pm.DeviceSNe.from_host(w.sne, dev)
         ctx.pm_deposit(st, sk, sn, w.dt)
         ctx.pm_fold_ghosts()
-        sums = [ctx.debug_buffer(ch)[1].clone() for ch in (0, 2, 5)]
+        sums = None
+        if rep < 2:
+            ctx.pm_debug_round_buffers()
+            sums = [ctx.debug_buffer(ch)[1].clone() for ch in (0, 2, 5)]
         ctx.pm_apply_limited(st)
         ctx.pm_return_to_particles(sk)
         ctx.pm_check()
@@ -128,4 +143,5 @@ def test_full_size_reproducible_step_twice_identical():
         del st, sk, sn
     for a, b in zip(outs[0][0], outs[1][0]):
         assert torch.equal(a, b)
-    assert torch.equal(outs[0][1], outs[1][1]) and torch.equal(outs[0][2], outs[1][2]) and torch.equal(outs[0][3], outs[1][3])
+    for rep in (1, 2):
+        assert torch.equal(outs[0][1], outs[rep][1]) and torch.equal(outs[0][2], outs[rep][2]) and torch.equal(outs[0][3], outs[rep][3])
