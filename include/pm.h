@@ -78,7 +78,7 @@ enum {
     PM_FLAG_DEBUG_LAMBDA = 2,    /* keep the Eq. 21 lambda of every cell (pm_debug_lambda) */
     PM_FLAG_GENERIC_KERNELS = 4, /* always use the generic (any radius, any n_sub) deposit / return kernels */
     PM_FLAG_TIMING = 8,          /* bracket every kernel with CUDA events on the ctx's stream (pm_kernel_times) */
-    PM_FLAG_REPRODUCIBLE = 16    /* Appendix A (L586-615): four more buffer channels (error scales, contribution counts); the apply
+    PM_FLAG_REPRODUCIBLE = 16    /* Appendix A (L586-615): three more buffer channels (two error scales, contribution counts); the apply
                                   * pass rounds the folded sums as it reads them: the step no longer depends on the order of
                                   * the atomic additions, except with probability ~2^-M per cell */
 };

@@ -238,7 +238,7 @@ __global__ void __launch_bounds__(128) k_deposit_sinks(const DevP P, const DevSt
             }
             double *dst = buf0 + ghost_index(P, i, j, k);
             atomicAdd(dst, -amt);                                     // R1: signed change
-            if (REPRO) atomicAdd(dst + kChKsink * P.Nb, 1.0);         // Appendix A: contribution count
+            if (REPRO) atomicAdd(dst + kChK * P.Nb, kSinkUnit);         // Appendix A: contribution count
         }
     }
     if (lane == 0) {
@@ -311,7 +311,7 @@ __global__ void __launch_bounds__(kSnWarps * 32) k_deposit_sne(const DevP P, con
         if (REPRO) {                                 // Appendix A: error scales and the contribution count (dst is channel 1)
             atomicAdd(dst + (kChTp - 1) * P.Nb, (fabs(d[1]) + fabs(d[2])) + fabs(d[3]));
             atomicAdd(dst + (kChTe - 1) * P.Nb, fabs(d[4]));
-            atomicAdd(dst + (kChKsn - 1) * P.Nb, 1.0);
+            atomicAdd(dst + (kChK - 1) * P.Nb, 1.0);
         }
     }
     if (dbg && lane == 0) {
@@ -450,8 +450,9 @@ __global__ void __launch_bounds__(256) k_repro_round(const DevP P, double *__res
     const int j = (int)(row % P.ny), k = (int)(row / P.ny);
     double *b = buf + ghost_index(P, i, j, k);
     double ksn[W], ksk[W];
-    ldv<W>(b + (long long)kChKsn * P.Nb, ksn);
-    ldv<W>(b + (long long)kChKsink * P.Nb, ksk);
+    ldv<W>(b + (long long)kChK * P.Nb, ksn);
+#pragma unroll
+    for (int e = 0; e < W; ++e) repro_counts(ksn[e], ksn[e], ksk[e]);
     bool any_sn = false, any_sk = false;
 #pragma unroll
     for (int e = 0; e < W; ++e) { any_sn |= ksn[e] > 1.0; any_sk |= ksk[e] > 1.0; }
@@ -500,8 +501,9 @@ __global__ void __launch_bounds__(kApplyThreads, 6) k_apply_limited(const DevP P
     for (int ch = 0; ch < kBufChannels; ++ch) ldv<VEC>(buf + (long long)ch * P.Nb + gq, b[ch]);
     if (REPRO) {   // Appendix A: round the folded sums here, where they are read anyway (rounding never turns a non-zero sum into zero)
         double ksn[VEC], ksk[VEC], tp[VEC], te[VEC];
-        ldv<VEC>(buf + (long long)kChKsn * P.Nb + gq, ksn);
-        ldv<VEC>(buf + (long long)kChKsink * P.Nb + gq, ksk);
+        ldv<VEC>(buf + (long long)kChK * P.Nb + gq, ksn);
+#pragma unroll
+        for (int v = 0; v < VEC; ++v) repro_counts(ksn[v], ksn[v], ksk[v]);
         ldv<VEC>(buf + (long long)kChTp * P.Nb + gq, tp);
         ldv<VEC>(buf + (long long)kChTe * P.Nb + gq, te);
 #pragma unroll

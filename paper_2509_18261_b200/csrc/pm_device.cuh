@@ -13,12 +13,12 @@ namespace pm {
 
 constexpr int kBufChannels = 6;      // 0: accretion d rho (signed, R1/R29); 1..5: SN d rho, d p (3), d E
 constexpr int kRetWords = 4;         // eta, v_old (3)
-// Appendix A mode (PM_FLAG_REPRODUCIBLE) adds four channels behind the six: error scales and contribution counts
+// Appendix A mode (PM_FLAG_REPRODUCIBLE) adds three channels behind the six: two error scales and the contribution counts
 constexpr int kChTp = 6;             // sum_s (|dp_x| + |dp_y| + |dp_z|) of the SN terms
 constexpr int kChTe = 7;             // sum_s |dE| of the SN terms
-constexpr int kChKsn = 8;            // number of SNe that contributed (as a double)
-constexpr int kChKsink = 9;          // number of sinks that contributed
-constexpr int kReproChannels = 10;
+constexpr int kChK = 8;              // contribution counts in one word: SNe + 2^20 * sinks (exact in a double; < 2^20 SNe per cell)
+constexpr double kSinkUnit = 1048576.0;
+constexpr int kReproChannels = 9;
 constexpr int kSbLog2 = 2;           // a super-block is (2^kSbLog2)^3 tiles of 8^3 cells (1..6 measured: no difference)
 constexpr double kFourPi = 12.566370614359172953850573533118;
 
@@ -332,6 +332,12 @@ __device__ __forceinline__ double repro_round(double x, double T, double k, int 
     if (nb > 52) nb = 52;
     const unsigned long long u = (unsigned long long)__double_as_longlong(x) & ~((1ull << nb) - 1ull);
     return __longlong_as_double((long long)u);
+}
+
+// split the packed count word: k_sn = low part, k_sink = multiples of 2^20
+__device__ __forceinline__ void repro_counts(double k, double &ksn, double &ksk) {
+    ksk = floor(k * (1.0 / kSinkUnit));
+    ksn = k - ksk * kSinkUnit;
 }
 
 }  // namespace pm

@@ -156,7 +156,7 @@ __global__ void __launch_bounds__(kFastSinkWarps * 32, kFastSinkMinBlocks) k_dep
             ret_tr[q] = -CUDART_INF;                    // invalidate last step's entry; the apply pass rewrites it where mass is removed
         }
         atomicAdd(dst, -amt);                           // R1: signed
-        if (REPRO) atomicAdd(dst + kChKsink * P.Nb, 1.0);   // Appendix A: contribution count (same-sign terms: T = |sum|)
+        if (REPRO) atomicAdd(dst + kChK * P.Nb, kSinkUnit);   // Appendix A: contribution count (same-sign terms: T = |sum|)
     }
     if (lane == 0) {
         scal[s] = sc.mdot; scal[S.n + s] = sc.r_acc; scal[2 * S.n + s] = wsum;

@@ -240,7 +240,7 @@ __device__ __forceinline__ void sn_deposit_one(const DevP &P, const DevState &U,
         if (REPRO) {                                 // Appendix A: error scales and the contribution count (dst is channel 1)
             atomicAdd(dst + (kChTp - 1) * P.Nb, (fabs(dpx) + fabs(dpy)) + fabs(dpz));
             atomicAdd(dst + (kChTe - 1) * P.Nb, fabs(de));
-            atomicAdd(dst + (kChKsn - 1) * P.Nb, 1.0);
+            atomicAdd(dst + (kChK - 1) * P.Nb, 1.0);
         }
     }
     if (dbg && lane == 0) {
