@@ -51,6 +51,7 @@ struct pm_ctx {
     double dt;
     long long launches;
     // host-step staging
+    cudaStream_t copy_stream; cudaEvent_t ev_inputs, ev_etot;   // pm_step_host: E uploads on its own stream under the deposit
     double *stg_state;  long long stg_state_cap;
     double *stg_sinks;  long long stg_sinks_cap;
     double *stg_sne;    long long stg_sne_cap;
@@ -721,6 +722,7 @@ extern "C" int pm_destroy(pm_ctx *c) {
     for (double *p : ptrs) if (p) cudaFree(p);
     if (c->timing)
         for (int k = 0; k < PM_NUM_KERNELS; ++k) { cudaEventDestroy(c->ev[k][0]); cudaEventDestroy(c->ev[k][1]); }
+    if (c->copy_stream) { cudaStreamDestroy(c->copy_stream); cudaEventDestroy(c->ev_inputs); cudaEventDestroy(c->ev_etot); }
     if (c->bin_mem) cudaFree(c->bin_mem);
     if (c->create_mem) cudaFree(c->create_mem);
     if (c->err_flag) cudaFree(c->err_flag);
@@ -987,7 +989,14 @@ extern "C" int pm_step_host(pm_ctx *c, pm_state *hs, pm_sinks *hk, const pm_sne 
     if ((rc = grow(c, &c->stg_sne, &c->stg_sne_cap, 8 * nn)) != PM_OK) return rc;
     cudaStream_t s = c->stream;
     double *hst[6] = { hs->rho, hs->mx, hs->my, hs->mz, hs->etot, hs->eint };
-    for (int f = 0; f < 6; ++f) PM_CUDA(c, cudaMemcpyAsync(c->stg_state + f * N, hst[f], N * 8, cudaMemcpyHostToDevice, s));
+    if (!c->copy_stream) {
+        PM_CUDA(c, cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
+        PM_CUDA(c, cudaEventCreateWithFlags(&c->ev_inputs, cudaEventDisableTiming));
+        PM_CUDA(c, cudaEventCreateWithFlags(&c->ev_etot, cudaEventDisableTiming));
+    }
+    // everything the deposit reads first (it never reads E); E follows on the copy stream, under the deposit kernels
+    for (int f = 0; f < 6; ++f)
+        if (f != 4) PM_CUDA(c, cudaMemcpyAsync(c->stg_state + f * N, hst[f], N * 8, cudaMemcpyHostToDevice, s));
     pm_state ds = { c->stg_state, c->stg_state + N, c->stg_state + 2 * N, c->stg_state + 3 * N, c->stg_state + 4 * N, c->stg_state + 5 * N };
     pm_sinks dk; std::memset(&dk, 0, sizeof(dk));
     pm_sne dn; std::memset(&dn, 0, sizeof(dn));
@@ -1011,8 +1020,13 @@ extern "C" int pm_step_host(pm_ctx *c, pm_state *hs, pm_sinks *hk, const pm_sne 
         dn.n = nn; dn.x = b; dn.y = b + nn; dn.z = b + 2 * nn; dn.vx = b + 3 * nn; dn.vy = b + 4 * nn; dn.vz = b + 5 * nn;
         dn.e_sn = b + 6 * nn; dn.m_ej = b + 7 * nn;
     }
+    PM_CUDA(c, cudaEventRecord(c->ev_inputs, s));
+    PM_CUDA(c, cudaStreamWaitEvent(c->copy_stream, c->ev_inputs, 0));
+    PM_CUDA(c, cudaMemcpyAsync(c->stg_state + 4 * N, hst[4], N * 8, cudaMemcpyHostToDevice, c->copy_stream));
+    PM_CUDA(c, cudaEventRecord(c->ev_etot, c->copy_stream));
     if ((rc = pm_deposit(c, &ds, nk > 0 ? &dk : nullptr, nn > 0 ? &dn : nullptr, dt)) != PM_OK) return rc;
     if ((rc = pm_fold_ghosts(c)) != PM_OK) return rc;
+    PM_CUDA(c, cudaStreamWaitEvent(s, c->ev_etot, 0));          // the apply pass is the first reader of E
     if ((rc = pm_apply_limited(c, &ds)) != PM_OK) return rc;
     if ((rc = pm_return_to_particles(c, nk > 0 ? &dk : nullptr)) != PM_OK) return rc;
     for (int f = 0; f < 6; ++f) PM_CUDA(c, cudaMemcpyAsync(hst[f], c->stg_state + f * N, N * 8, cudaMemcpyDeviceToHost, s));
