@@ -25,6 +25,7 @@ constexpr int kSnB = 7, kSnCells = 343, kSnNs = 4;
 // Box cell (a, b, c) = (x, y, z offsets in 0..6) packed as a | b << 3 | c << 6 (< 448).
 struct __align__(16) SnWarpSmem {
     double d2[3][kSnB * kSnNs];     // squared sub-sample offsets per axis
+    double thr[kSnB * kSnNs];       // per x sub-sample: the largest s >= 0 with fl(s + dx^2) <= r_K^2 (-1: none)
     double dmin[3][8], dmax[3][8];  // per-cell min / max of them
     double dc[3][8];                // cell-centre offsets from the particle per axis
     int off[3][8];                  // wrapped owned-index contribution per axis (x: i, y: j*nx, z: k*nx*ny)
@@ -37,6 +38,24 @@ __device__ __forceinline__ unsigned lanemask_lt() {
     unsigned m;
     asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m));
     return m;
+}
+
+// The largest double s >= 0 that passes the sub-sample test  fl(s + x) <= R  (x >= 0), or -1 when not even s = 0 passes.
+// fl(s + x) is monotone in s, so the test is  s <= sn_threshold(x)  EXACTLY: the estimate R - x + h (h = half the gap
+// above R, the rounding boundary) is walked to the boundary with the test itself, which makes the result independent
+// of how good the estimate was.
+__device__ __forceinline__ double sn_threshold(const double x, const double R) {
+    if (!(x <= R)) return -1.0;
+    const double h = 0.5 * (__longlong_as_double(__double_as_longlong(R) + 1) - R);
+    const double hi = R - x, lo = (R - hi) - x;          // R - x = hi + lo exactly (R >= x >= 0)
+    double t = hi + (lo + h);
+    for (int it = 0; it < 64 && !((t + x) <= R); ++it) t = __longlong_as_double(__double_as_longlong(t) - 1);
+    for (int it = 0; it < 64; ++it) {
+        const double u = __longlong_as_double(__double_as_longlong(t) + 1);
+        if (!((u + x) <= R)) break;
+        t = u;
+    }
+    return t;
 }
 
 __device__ __forceinline__ double pick3(int ax, double a, double b, double c) { return ax == 0 ? a : (ax == 1 ? b : c); }
@@ -86,6 +105,7 @@ __device__ __forceinline__ void sn_deposit_one(const DevP &P, const DevState &U,
         sm.dmin[ax][c] = fmin(fmin(v0, v1), fmin(v2, v3));
         sm.dmax[ax][c] = fmax(fmax(v0, v1), fmax(v2, v3));
     }
+    if (lane < kSnB * kSnNs) sm.thr[lane] = sn_threshold(sm.d2[0][lane], P.rk2_sn);
     __syncwarp();
     // ---- phase 1: classify by ROWS (49 rows of 7 cells; this lane owns rows `lane` and `lane + 32`): two fp64 compares per
     // cell give bit masks of the full and of the boundary cells; the boundary cells go to a list (any order)
@@ -130,7 +150,8 @@ __device__ __forceinline__ void sn_deposit_one(const DevP &P, const DevState &U,
     for (int idx = lane; idx < nb; idx += 32) {
         const int pc = sm.list[idx];
         const int a = pc & 7, b = (pc >> 3) & 7, cc = pc >> 6;
-        const double x0 = sm.d2[0][4 * a], x1 = sm.d2[0][4 * a + 1], x2 = sm.d2[0][4 * a + 2], x3 = sm.d2[0][4 * a + 3];
+        // (dz^2 + dy^2) + dx^2 <= r_K^2 in its exact threshold form: one add and four compares per (z, y) pair
+        const double t0 = sm.thr[4 * a], t1 = sm.thr[4 * a + 1], t2 = sm.thr[4 * a + 2], t3 = sm.thr[4 * a + 3];
         double yv[4], zv[4];
 #pragma unroll
         for (int q = 0; q < 4; ++q) { yv[q] = sm.d2[1][4 * b + q]; zv[q] = sm.d2[2][4 * cc + q]; }
@@ -140,7 +161,7 @@ __device__ __forceinline__ void sn_deposit_one(const DevP &P, const DevState &U,
 #pragma unroll
             for (int qy = 0; qy < 4; ++qy) {
                 const double sy = zv[qz] + yv[qy];
-                cnt += ((sy + x0) <= rk2) + ((sy + x1) <= rk2) + ((sy + x2) <= rk2) + ((sy + x3) <= rk2);
+                cnt += (sy <= t0) + (sy <= t1) + (sy <= t2) + (sy <= t3);
             }
         sm.cnt[pc] = (unsigned char)cnt;
     }

@@ -396,3 +396,23 @@ def test_generic_and_fast_kernels_agree_bitwise_on_integers():
     assert np.array_equal(outs[0][0], outs[1][0])
     assert np.array_equal(outs[0][1], outs[1][1])
     assert np.allclose(outs[0][2], outs[1][2], rtol=1e-13, atol=0)     # V_snr = (sum of omega counts) V / 64
+
+
+def test_sn_subsamples_exactly_on_the_kernel_radius():
+    """Supernovae an odd multiple of dx/8 off a cell corner: every sub-sample offset is a multiple of dx/4, 30 of them lie
+    exactly ON r_K = 3 dx and many more within a few ulp of the rounding boundary of the test (L203).  The specialised
+    kernel's threshold form of the test must give the oracle's counts: V_snr bit for bit, buffers within tolerance."""
+    w = inputs.scaled_mixed(24, 64, seed_index=5)
+    assert w.params["dx"] == 1.0 and w.params["rk_sn"] == 3.0 and w.params["sn_nsub"] == 4
+    rng = np.random.default_rng(11)
+    eighths = np.array([0.125, 0.375, 0.625, 0.875])
+    for f in ("x", "y", "z"):
+        getattr(w.sne, f)[:] = rng.integers(0, 24, size=w.sne.n) + rng.choice(eighths, size=w.sne.n)
+    # a few more a hair off the exact positions: sums that straddle the rounding boundary of r_K^2
+    k = w.sne.n // 2
+    w.sne.x[:k] = np.nextafter(w.sne.x[:k], np.where(rng.random(k) < 0.5, -np.inf, np.inf))
+    g, o, _ = parity.run_and_compare(w, steps=1)
+    v_gpu = g.ctx.debug_sn_scalars().cpu().numpy()[1]
+    assert np.array_equal(v_gpu, o.sn_diag["v_snr"]), "V_snr = (sum of omega counts) V / 64 must match bit for bit"
+    exact = w.sne.x == np.round(w.sne.x * 8) / 8
+    assert np.all(v_gpu[exact] == 7153.0 / 64.0)

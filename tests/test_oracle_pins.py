@@ -638,3 +638,21 @@ def test_return_matches_list_form():
         dm = po.return_from_list(o.eta, cells, a, 1.0)
         assert dm == pytest.approx(o.sink_diag["dm"][s], rel=1e-14)
         assert w.sinks.m[s] == pytest.approx(sk0.m[s] + dm, rel=1e-15)
+
+
+@pytest.mark.parametrize("off", [(0.125, 0.125, 0.125), (0.625, 0.375, 0.875)])
+def test_sn_omega_subsamples_exactly_on_the_radius(off):
+    """A supernova an odd multiple of dx/8 off a cell corner sees every sub-cell centre (n_sub = 4) at a multiple of
+    dx/4: with r_K = 3 dx the test of L203 is m1^2 + m2^2 + m3^2 <= 144 on the integer lattice, every operand exact
+    in binary, and the sub-samples ON the radius (30 of them) count as inside.  The sum of the omega counts is the
+    number of lattice points in the closed ball of radius 12, counted here by plain integer enumeration."""
+    n = 12
+    p = inputs.default_params(n)
+    assert p["dx"] == 1.0 and p["rk_sn"] == 3.0 and p["sn_nsub"] == 4
+    pos = (5.0 + off[0], 6.0 + off[1], 4.0 + off[2])
+    counts, _ = po.sn_omega_box(p, *pos)
+    r = range(-12, 13)
+    inside = sum(1 for a in r for b in r for c in r if a * a + b * b + c * c <= 144)
+    on_radius = sum(1 for a in r for b in r for c in r if a * a + b * b + c * c == 144)
+    assert on_radius == 30
+    assert int(counts.sum()) == inside
