@@ -819,7 +819,7 @@ extern "C" int pm_deposit(pm_ctx *c, const pm_state *st, const pm_sinks *sk, con
         const unsigned blocks = (unsigned)((nn + kSnWarps - 1) / kSnWarps);
         const size_t smem = kSnWarps * sn_table_bytes(2 * P.gn + 1, P.nsub);
         tick(c, PM_K_SNE, 0);
-        if (P.gn == 3 && P.nsub == 4 && !c->force_generic)
+        if (P.gn == 3 && P.nsub == 4 && !c->force_generic && 7 * P.pk < (1ll << 31))   // box offsets are 32-bit there
             (c->repro ? k_deposit_sne_g3n4<true> : k_deposit_sne_g3n4<false>)<<<(unsigned)((nn + kFastSnWarps - 1) / kFastSnWarps), kFastSnWarps * 32, 0, c->stream>>>(P, U, S, c->buf, dbg ? c->dbg_sn : nullptr, c->err_flag, perm + nk);
         else
             (c->repro ? k_deposit_sne<true> : k_deposit_sne<false>)<<<blocks, kSnWarps * 32, smem, c->stream>>>(P, U, S, c->buf, dbg ? c->dbg_sn : nullptr, c->err_flag, perm + nk);

@@ -29,7 +29,6 @@ struct __align__(16) SnWarpSmem {
     double dmin[3][8], dmax[3][8];  // per-cell min / max of them
     double dc[3][8];                // cell-centre offsets from the particle per axis
     int off[3][8];                  // wrapped owned-index contribution per axis (x: i, y: j*nx, z: k*nx*ny)
-    int goff[2][8];                 // ghosted-index contribution of y and z
     unsigned short list[352];       // boundary-cell list, then active-cell list (packed codes)
     unsigned char cnt[448];         // omega counts (0..64) by packed code
 };
@@ -96,7 +95,6 @@ __device__ __forceinline__ void sn_deposit_one(const DevP &P, const DevState &U,
         sm.dc[ax][c] = cell_centre(x0, u, P.dx) - ps;
         const int wq = wrap1(u, n);
         sm.off[ax][c] = ax == 0 ? wq : (ax == 1 ? wq * P.nx : wq * P.nx * P.ny);
-        if (ax > 0) sm.goff[ax - 1][c] = (int)((u + P.g) * (ax == 1 ? P.pj : P.pk));
     }
     __syncwarp();
     if (lane < 21) {
@@ -200,6 +198,11 @@ __device__ __forceinline__ void sn_deposit_one(const DevP &P, const DevState &U,
     const double vsx = S.vx[s], vsy = S.vy[s], vsz = S.vz[s], e_sn = S.e_sn[s], m_ej = S.m_ej[s];
     const double v64 = P.V * (1.0 / 64.0);
     double m_gas = 0.0, px = 0.0, py = 0.0, pz = 0.0, v_snr = 0.0;
+    // owned index of a box cell: plain strides when the box does not cross the periodic seam (warp-uniform), else the
+    // wrapped per-axis tables
+    const bool inner = ih >= 3 && ih + 3 < P.nx && jh >= 3 && jh + 3 < P.ny && kh >= 3 && kh + 3 < P.nz;
+    const int nxny = P.nx * P.ny;
+    const int qb = ((kh - 3) * P.ny + (jh - 3)) * P.nx + (ih - 3);
     // batches of kSnGatherBatch list entries per lane: all their loads are in flight together (the gather is latency-bound)
 #pragma unroll 1
     for (int base = lane; base < na; base += 32 * kSnGatherBatch) {
@@ -211,7 +214,7 @@ __device__ __forceinline__ void sn_deposit_one(const DevP &P, const DevState &U,
             const bool on = idx < na;
             const int e = on ? sm.list[idx] : 0;
             const int a = e & 7, b = (e >> 3) & 7, cc = (e >> 6) & 7;
-            q[u] = on ? sm.off[2][cc] + sm.off[1][b] + sm.off[0][a] : 0;
+            q[u] = !on ? 0 : (inner ? qb + cc * nxny + b * P.nx + a : sm.off[2][cc] + sm.off[1][b] + sm.off[0][a]);
             wv[u] = on ? (double)((e >> 9) + 1) * v64 : 0.0;              // omega V; omega = count / 64 is exact
         }
         double rho[kSnGatherBatch], mx[kSnGatherBatch], my[kSnGatherBatch], mz[kSnGatherBatch];
@@ -233,13 +236,14 @@ __device__ __forceinline__ void sn_deposit_one(const DevP &P, const DevState &U,
     const double k_rho = m_ej * inv_vsnr;                 // d rho = omega M_ej / V_snr
     const double k_e = (e_sn + sc.e_kin) * inv_vsnr;     // (E_sn + E_kin) / V_snr per unit omega
     const double k_p = sc.p_rad * inv_vsnr;
-    double *const sbuf = buf + P.Nb + (ih - 3 + P.gx);
+    double *const sbuf = buf + P.Nb + ((long long)(kh - 3 + P.g) * P.pk + (long long)(jh - 3 + P.g) * P.pj + (ih - 3 + P.gx));
+    const int pj = (int)P.pj, pk = (int)P.pk;
 #pragma unroll 1
     for (int idx = lane; idx < na; idx += 32) {
         const int e = sm.list[idx];
         const int a = e & 7, b = (e >> 3) & 7, cc = (e >> 6) & 7;
         const double omega = (double)((e >> 9) + 1) * (1.0 / 64.0);
-        const int q = sm.off[2][cc] + sm.off[1][b] + sm.off[0][a];
+        const int q = inner ? qb + cc * nxny + b * P.nx + a : sm.off[2][cc] + sm.off[1][b] + sm.off[0][a];
         const double rho = U.rho[q], mx = U.mx[q], my = U.my[q], mz = U.mz[q];
         const double ddx = sm.dc[0][a], ddy = sm.dc[1][b], ddz = sm.dc[2][cc];
         const double r2 = dist2(ddx, ddy, ddz);
@@ -247,7 +251,7 @@ __device__ __forceinline__ void sn_deposit_one(const DevP &P, const DevState &U,
         const double drho = omega * k_rho;
         const double pscale = (k_p * omega) * ir;
         const double prx = pscale * ddx, pry = pscale * ddy, prz = pscale * ddz;
-        double *dst = sbuf + (sm.goff[1][cc] + sm.goff[0][b] + a);
+        double *dst = sbuf + (cc * pk + b * pj + a);              // ghosted layout: no wrap, plain strides
         // omega rho (v_COM - v) = omega (rho v_COM - m): no division by rho
         const double dpx = fma(omega, fma(rho, sc.vcx, -mx), fma(drho, sc.vcx, prx));
         const double dpy = fma(omega, fma(rho, sc.vcy, -my), fma(drho, sc.vcy, pry));
