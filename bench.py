@@ -290,6 +290,40 @@ def run_ours(args, rank, world, local_rank):
                      "hbm_footprint_5GB_5ch": ctx.pm_probe_red_f64(5 << 30, 5), "unit": "1e9 fp64 RED lanes/s",
                      "pattern": "rows of 7 consecutive doubles, 5 planes (pm_probe_red_f64)"}
 
+    # ---- row (f)3, not part of the step: PM gravity (Steps 1, 2, 5; L95, L107) for the same number of particles --------
+    gravity = None
+    if rank == 0 and world == 1 and not args.reproducible and args.config is None:
+        gw = inputs.gravity_workload(n, npart)
+        gpos = [torch.from_numpy(a).to(dev) for a in (gw.x, gw.y, gw.z)]
+        gvel = [torch.from_numpy(a).to(dev) for a in (gw.vx, gw.vy, gw.vz)]
+        gm = torch.from_numpy(gw.m).to(dev)
+        gmesh = [torch.from_numpy(a).to(dev) for a in gw.g]
+        rho_tot = torch.empty_like(st.rho)
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+        samples = []
+        for rep in range(6):                                         # ctx launches on torch's current stream
+            ev[0].record()
+            ctx.pm_gravity_deposit(st.rho, gpos[0], gpos[1], gpos[2], gm, rho_tot)
+            ev[1].record()
+            ctx.pm_gravity_kick(gmesh[0], gmesh[1], gmesh[2], gpos[0], gpos[1], gpos[2], v=gvel, dt=0.5 * gw.dt)
+            ev[2].record()
+            ctx.pm_drift(gpos[0], gpos[1], gpos[2], gvel[0], gvel[1], gvel[2], gw.dt)
+            ev[3].record()
+            torch.cuda.synchronize(dev)
+            if rep >= 2:
+                samples.append([ev[i].elapsed_time(ev[i + 1]) for i in range(3)])
+        ctx.pm_check()
+        gms = [float(np.median([s_[i] for s_ in samples])) for i in range(3)]
+        gbytes = [8.0 * Nb + 24.0 * N + 16.0 * (Nb - N) + 160.0 * npart, 264.0 * npart, 72.0 * npart]
+        peak_g, _ = measured_peak()
+        gravity = {"particles": npart, "workload": gw.name,
+                   "timing": "torch CUDA events on the launching stream, median of 4 after 2 warm-up rounds; meshes (GBs) larger than L2"}
+        for name, ms_, b_ in zip(("deposit", "kick", "drift"), gms, gbytes):
+            gravity[name] = {"ms": ms_, "algorithmic_bytes": b_, "achieved_gbs": b_ / (ms_ * 1e-3) / 1e9,
+                             "frac_of_measured_peak": b_ / (ms_ * 1e-3) / 1e9 / peak_g}
+        gravity["particles_per_s_kdk_half"] = npart / (sum(gms) * 1e-3)
+        del gpos, gvel, gm, gmesh, rho_tot
+
     # ---- e2e through pm_step_host with pinned host buffers --------------------------------------
     e2e_steps = max(1, min(args.steps, args.e2e_steps))
     hst = inputs.State(*(torch.from_numpy(f).pin_memory() for f in w.state.fields()))
@@ -353,6 +387,8 @@ def run_ours(args, rank, world, local_rank):
         }
         if creation:
             line["sink_creation"] = creation
+        if gravity:
+            line["gravity"] = gravity
         if red_probe:
             n_red = 5.0 * 183.0 * w.sne.n     # ~183 cells with omega > 0 per SN (SURVEY.md 8 probe), 5 channels
             red_probe["sn_deposit_achieved"] = n_red / (kernel_ms["sne"] * 1e-3) / 1e9 if kernel_ms["sne"] > 0 else None

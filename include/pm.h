@@ -14,6 +14,8 @@
  *                          U := U + eta dU^sum, in place on the caller's conserved state.
  *   pm_return_to_particles Step 4, Eq. 5 (L79-87): u_s := u_s - sum_ijk eta_ijk dU^s_ijk V_ijk for every sink
  *                          (supernova particles skip this step, L201).
+ *   pm_gravity_deposit / pm_gravity_kick / pm_drift   PM gravity for the particles' own motion (L95, L107): Steps 1, 2, 5
+ *                          with the cloud-in-cell kernel, interpolation back with the same kernel, kick-drift-kick.
  *
  * All pointers inside pm_state / pm_sinks / pm_sne are DEVICE pointers (cudaMalloc'ed by the caller, e.g. torch
  * allocations) unless a function says "host".  Every array is fp64, contiguous.  Mesh fields hold nx*ny*nz values,
@@ -134,6 +136,39 @@ int pm_set_repro_margin(pm_ctx *ctx, int32_t M);
  * (call again with larger arrays).  Synchronises. */
 int pm_create_sinks(pm_ctx *ctx, pm_state *state, int64_t max_new, double *x, double *y, double *z, double *vx, double *vy,
                     double *vz, double *m, int64_t *n_new);
+
+/* ---- PM gravity: Steps 1, 2 and 5 only (L95: "no limiting ... interactions do not modify particle
+ * properties, only mesh properties"; L107: sinks and star particles move under "a standard PM gravity method, which we
+ * implement using steps 1, 2, and 5", kick-drift-kick).  The Poisson solve between pm_gravity_deposit and pm_gravity_kick is
+ * the host code's (multigrid, L427) and is not part of this library: the acceleration mesh is an input.
+ * Kernel W: cloud-in-cell (R40).  Per axis s = (x - x0)/dx - 1/2, i0 = floor(s), f = s - i0; cells i0, i0 + 1 get 1 - f, f;
+ * W_ijk = (W_z W_y) W_x; r_K = dx, so one ghost layer contains it (L59).  All pointers DEVICE, fp64, contiguous; particle
+ * arrays hold n values, mesh arrays nx*ny*nz (x fastest, no ghosts).  Particles must lie in [x0, x0 + n dx) (else
+ * PM_EDOMAIN at the next pm_check).  Asynchronous on the ctx's stream. */
+
+/* rho_tot := rho_gas + sum_s m_s W(x_ijk - x_s) / V (L51: "depositing particle mass into the gas density field for the
+ * purposes of computing the gravitational potential").  Step 1: buffer channel 0 is zeroed and receives the eight fp64
+ * atomic additions of every particle, ghost layer included; Step 2: pm_fold_ghosts on that channel; Step 5: the sum is
+ * written to rho_tot (eta = 1).  rho_gas may be NULL (particles only) and may alias rho_tot.  n may be 0.  Uses the ctx's
+ * buffer mesh: not allowed between pm_deposit and pm_apply_limited (PM_EORDER); afterwards the retained accretion buffer of
+ * L108 is gone, so call it before the step's pm_deposit as the paper's sequence does (L107-109), or pm_create_sinks first. */
+int pm_gravity_deposit(pm_ctx *ctx, const double *rho_gas, int64_t n, const double *x, const double *y, const double *z,
+                       const double *m, double *rho_tot);
+
+/* Mesh -> particle interpolation with the same W (L27), fused with a kick (L107): a_s = sum_ijk W(x_ijk - x_s) g_ijk over
+ * the particle's eight cells (periodic; summed in the order k, j, i, low cell first), then v_s += a_s dt (dt = half the
+ * step for each of the two kicks).  gx, gy, gz: acceleration meshes.  vx, vy, vz: all NULL = interpolate only.  ax, ay, az:
+ * optional outputs of a_s, all NULL = not stored.  At least one of the two groups must be given. */
+int pm_gravity_kick(pm_ctx *ctx, const double *gx, const double *gy, const double *gz, int64_t n, const double *x,
+                    const double *y, const double *z, double *vx, double *vy, double *vz, double dt, double *ax, double *ay,
+                    double *az);
+
+/* Drift: x_s += v_s dt, brought back into the periodic box by whole box lengths (R41: a result that rounds onto the upper
+ * face is put on the lower face).  Positions are modified in place -- the one call that moves particles; not allowed
+ * between pm_apply_limited and pm_return_to_particles (PM_EORDER).  A non-finite result, or one more than 1e6 box lengths
+ * away, raises PM_EDOMAIN at the next pm_check and is stored unwrapped. */
+int pm_drift(pm_ctx *ctx, int64_t n, double *x, double *y, double *z, const double *vx, const double *vy, const double *vz,
+             double dt);
 
 /* Synchronise the ctx's stream and report PM_ECUDA / PM_EDOMAIN raised by earlier asynchronous work. */
 int pm_check(pm_ctx *ctx);

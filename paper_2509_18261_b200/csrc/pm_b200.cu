@@ -7,9 +7,12 @@
 //   k_fold_ghosts      a6  gather fold: every owned cell within g of a face sums its <= 7 ghost images, fixed order
 //   k_apply_limited    a7  fused limiter + apply, 128-bit loads/stores, untouched cells skip the state traffic
 //   k_return_sinks     a8  one warp per sink: sum eta a V (1, v_old) with a shuffle reduction
+//   k_grav_deposit / k_grav_apply / k_grav_kick / k_drift   (f)3  PM gravity: cloud-in-cell deposit (Steps 1, 2, 5),
+//                      interpolation + half kick, drift (pm_gravity.cuh)
 #include "pm_device.cuh"
 #include "pm_fast.cuh"
 #include "pm_create.cuh"
+#include "pm_gravity.cuh"
 #include "../../include/pm.h"
 
 #include <cmath>
@@ -964,6 +967,80 @@ extern "C" int pm_create_sinks(pm_ctx *c, pm_state *st, int64_t max_new, double 
     }
     *n_new = found;
     return PM_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// (f)3: PM gravity (L95, L107): Steps 1, 2, 5 with the cloud-in-cell kernel, interpolation + kick, drift
+// ---------------------------------------------------------------------------------------------------------------
+static int fold_channel0(pm_ctx *c) {
+    const DevP &P = c->P;
+    const long long g2 = 2 * P.g;
+    const int W = (P.g % 2 == 0 && P.nx % 2 == 0) ? 2 : 1;
+    const long long n_z = g2 * P.ny * P.nx / W;
+    const long long n_y = (long long)(P.nz - g2) * g2 * P.nx / W;
+    const long long n_x = (long long)(P.nz - g2) * (P.ny - g2) * g2 / W;
+    const long long n_edge = n_z + n_y + n_x;
+    const unsigned blocks = (unsigned)((n_edge + 255) / 256);
+    if (W == 2) k_fold_ghosts<2, 1><<<blocks, 256, 0, c->stream>>>(P, c->buf, n_edge, n_z, n_y);
+    else k_fold_ghosts<1, 1><<<blocks, 256, 0, c->stream>>>(P, c->buf, n_edge, n_z, n_y);
+    return check_launch(c, "k_fold_ghosts<1 channel>");
+}
+
+extern "C" int pm_gravity_deposit(pm_ctx *c, const double *rho_gas, int64_t n, const double *x, const double *y, const double *z,
+                                  const double *m, double *rho_tot) {
+    if (!c) return PM_EINVAL;
+    if (n < 0 || !rho_tot) PM_FAIL(c, PM_EINVAL, "pm_gravity_deposit: null output or negative particle count");
+    if (n > 0 && !(x && y && z && m)) PM_FAIL(c, PM_EINVAL, "pm_gravity_deposit: null particle array");
+    if (c->stage == ST_DEPOSITED || c->stage == ST_FOLDED)
+        PM_FAIL(c, PM_EORDER, "pm_gravity_deposit: the buffer mesh is in use (finish the exchange step first)");
+    PM_CUDA(c, cudaSetDevice(c->device));
+    const DevP &P = c->P;
+    c->buffer_valid = false;      // channel 0 no longer holds the accretion rates of the last exchange step
+    c->stage = ST_IDLE;
+    int rc;
+    PM_CUDA(c, cudaMemsetAsync(c->buf, 0, (size_t)P.Nb * sizeof(double), c->stream));     // Step 1: "initialized to zero" (L59)
+    if (n > 0) {
+        k_grav_deposit<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(P, x, y, z, m, n, c->buf, c->err_flag);
+        if ((rc = check_launch(c, "k_grav_deposit")) != PM_OK) return rc;
+    }
+    if ((rc = fold_channel0(c)) != PM_OK) return rc;                                       // Step 2
+    const bool vec = P.nx % 2 == 0 && aligned16(rho_tot) && (!rho_gas || aligned16(rho_gas));
+    const long long work = vec ? P.N / 2 : P.N;
+    long long blocks = (work + 255) / 256;
+    const long long cap = (long long)c->sm_count * 32;
+    if (blocks > cap) blocks = cap;
+    if (vec) k_grav_apply<2><<<(unsigned)blocks, 256, 0, c->stream>>>(P, rho_gas, c->buf, rho_tot);   // Step 5
+    else k_grav_apply<1><<<(unsigned)blocks, 256, 0, c->stream>>>(P, rho_gas, c->buf, rho_tot);
+    return check_launch(c, "k_grav_apply");
+}
+
+extern "C" int pm_gravity_kick(pm_ctx *c, const double *gx, const double *gy, const double *gz, int64_t n, const double *x,
+                               const double *y, const double *z, double *vx, double *vy, double *vz, double dt, double *ax,
+                               double *ay, double *az) {
+    if (!c) return PM_EINVAL;
+    if (n < 0 || !(gx && gy && gz)) PM_FAIL(c, PM_EINVAL, "pm_gravity_kick: null acceleration mesh or negative particle count");
+    if (n == 0) return PM_OK;
+    if (!(x && y && z)) PM_FAIL(c, PM_EINVAL, "pm_gravity_kick: null position array");
+    const bool has_v = vx || vy || vz, has_a = ax || ay || az;
+    if (has_v && !(vx && vy && vz)) PM_FAIL(c, PM_EINVAL, "pm_gravity_kick: give all of vx, vy, vz or none");
+    if (has_a && !(ax && ay && az)) PM_FAIL(c, PM_EINVAL, "pm_gravity_kick: give all of ax, ay, az or none");
+    if (!has_v && !has_a) PM_FAIL(c, PM_EINVAL, "pm_gravity_kick: nothing to write (no velocities, no acceleration output)");
+    PM_CUDA(c, cudaSetDevice(c->device));
+    k_grav_kick<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(c->P, gx, gy, gz, n, x, y, z, vx, vy, vz, dt, ax, ay, az, c->err_flag);
+    return check_launch(c, "k_grav_kick");
+}
+
+extern "C" int pm_drift(pm_ctx *c, int64_t n, double *x, double *y, double *z, const double *vx, const double *vy, const double *vz,
+                        double dt) {
+    if (!c) return PM_EINVAL;
+    if (n < 0) PM_FAIL(c, PM_EINVAL, "pm_drift: negative particle count");
+    if (n == 0) return PM_OK;
+    if (!(x && y && z && vx && vy && vz)) PM_FAIL(c, PM_EINVAL, "pm_drift: null particle array");
+    if (c->stage == ST_APPLIED)
+        PM_FAIL(c, PM_EORDER, "pm_drift: pm_return_to_particles needs the positions of the preceding pm_deposit; call it first");
+    PM_CUDA(c, cudaSetDevice(c->device));
+    k_drift<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(c->P, n, x, y, z, vx, vy, vz, dt, c->err_flag);
+    return check_launch(c, "k_drift");
 }
 
 extern "C" int pm_check(pm_ctx *c) {

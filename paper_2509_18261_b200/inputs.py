@@ -263,6 +263,51 @@ def scaled_mixed(n: int, n_particles: int, seed_index: int = 5, n_clusters: int 
                   f"config5_shape_{n}_{n_particles}")
 
 
+@dataclass
+class GravityWorkload:
+    """Inputs of the PM-gravity calls: collisionless particles, the gas density they are deposited
+    onto, and an acceleration mesh standing in for the host code's Poisson solve (out of scope, L427)."""
+    name: str
+    params: dict
+    rho_gas: np.ndarray          # (nz, ny, nx)
+    x: np.ndarray
+    y: np.ndarray
+    z: np.ndarray
+    vx: np.ndarray
+    vy: np.ndarray
+    vz: np.ndarray
+    m: np.ndarray
+    g: tuple                     # (gx, gy, gz), each (nz, ny, nx)
+    dt: float
+
+
+def gravity_workload(n: int, n_particles: int, seed_index: int = 6, n_clusters: int | None = None,
+                     shape: tuple | None = None, dx: float = 1.0, x0=(0.0, 0.0, 0.0)) -> GravityWorkload:
+    """Config-5-shaped particle set for the gravity path: positions half uniform, half in Gaussian clusters (sigma = 6 dx),
+    masses U(1, 100), velocities N(0, 0.05), lognormal gas (sigma_ln = 1.5), acceleration mesh N(0, 0.01) per component.
+    shape = (nx, ny, nz) for a non-cubic box (positions are drawn in the cube of side min(shape))."""
+    g_rho, g_vel, g_cen, g_pos, g_pm = _streams(seed_index)
+    nx, ny, nz = shape if shape is not None else (n, n, n)
+    p = default_params(n)
+    p.update(nx=nx, ny=ny, nz=nz, dx=dx, x0=tuple(x0))
+    if dx != 1.0:                      # kernel radii of the exchange step in cells, not length units (ghost width 4)
+        p.update(rk_sink=3.5 * dx, rk_sn=2.5 * dx)
+    if n_clusters is None:
+        n_clusters = max(1, int(round(200 * (n / 512.0) ** 3)))
+    rho = np.exp(1.5 * g_rho.standard_normal((nz, ny, nx)) - 0.5 * 1.5 * 1.5)
+    acc = tuple(0.01 * g_vel.standard_normal((nz, ny, nx)) for _ in range(3))
+    pos = _clustered_positions(g_cen, g_pos, n_particles, min(nx, ny, nz), n_clusters, 6.0, 0.5)
+    m = g_pm.uniform(1.0, 100.0, size=n_particles)
+    vel = 0.05 * g_pm.standard_normal((n_particles, 3))
+    xs = [np.ascontiguousarray(x0[c] + pos[:, c] * dx) for c in range(3)]
+    # x0 + pos dx can round onto the upper face; such a particle is put on the lower face
+    for c, nn in enumerate((nx, ny, nz)):
+        xs[c][xs[c] >= x0[c] + nn * dx] = x0[c]
+    return GravityWorkload(f"gravity_{nx}x{ny}x{nz}_{n_particles}", p, rho, xs[0], xs[1], xs[2],
+                           np.ascontiguousarray(vel[:, 0]), np.ascontiguousarray(vel[:, 1]), np.ascontiguousarray(vel[:, 2]),
+                           m, acc, dt=0.5)
+
+
 CONFIGS = {
     1: config1_tiny_sink,
     2: config2_bondi,

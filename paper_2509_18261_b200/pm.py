@@ -24,7 +24,7 @@ KERNEL_GROUPS = ("bin", "zero", "sinks", "sne", "fold", "apply", "return")
 STATUS_NAMES = {0: "PM_OK", -1: "PM_EINVAL", -2: "PM_ENOMEM", -3: "PM_ECUDA", -4: "PM_EORDER", -5: "PM_EDOMAIN"}
 
 EXPORTS = ["pm_create", "pm_deposit", "pm_fold_ghosts", "pm_apply_limited", "pm_return_to_particles", "pm_check",
-           "pm_step_host", "pm_destroy", "pm_last_error", "pm_launch_count", "pm_kernel_times", "pm_probe_red_f64", "pm_set_repro_margin", "pm_create_sinks", "pm_debug_round_buffers", "pm_debug_buffer",
+           "pm_step_host", "pm_destroy", "pm_last_error", "pm_launch_count", "pm_kernel_times", "pm_probe_red_f64", "pm_set_repro_margin", "pm_create_sinks", "pm_gravity_deposit", "pm_gravity_kick", "pm_drift", "pm_debug_round_buffers", "pm_debug_buffer",
            "pm_debug_return_mesh", "pm_debug_lambda", "pm_debug_sink_scalars", "pm_debug_sn_scalars",
            "pm_debug_stencil"]
 
@@ -104,6 +104,9 @@ def lib():
         L.pm_launch_count.restype = C.c_int64
         L.pm_set_repro_margin.argtypes = [vp, C.c_int32]
         L.pm_create_sinks.argtypes = [vp, C.POINTER(PmState), C.c_int64] + [vp] * 7 + [i64p]
+        L.pm_gravity_deposit.argtypes = [vp, vp, C.c_int64, vp, vp, vp, vp, vp]
+        L.pm_gravity_kick.argtypes = [vp] + [vp] * 3 + [C.c_int64] + [vp] * 6 + [C.c_double] + [vp] * 3
+        L.pm_drift.argtypes = [vp, C.c_int64] + [vp] * 6 + [C.c_double]
         L.pm_kernel_times.argtypes = [vp, C.POINTER(C.c_float), C.c_int32]
         L.pm_probe_red_f64.argtypes = [vp, C.c_int64, C.c_int32, C.POINTER(C.c_double)]
         L.pm_debug_round_buffers.argtypes = [vp]
@@ -139,6 +142,14 @@ def _ptr(t):
         return None
     assert t.dtype == torch.float64 and t.is_contiguous(), "fp64 contiguous tensors only"
     return t.data_ptr()
+
+
+def _dptr(t):
+    """Device pointer of a contiguous fp64 CUDA tensor (None -> NULL)."""
+    if t is None:
+        return None
+    assert t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()
+    return C.c_void_p(t.data_ptr())
 
 
 def _from_ptr(ptr: int, n: int, device, dtype=torch.float64):
@@ -300,6 +311,26 @@ class Context:
                                          C.byref(n)), "pm_create_sinks")
         k = n.value if n.value <= max_new else 0
         return int(n.value), {key: v[:k] for key, v in out.items()}
+
+    # ---- PM gravity (Steps 1, 2, 5; L95, L107) ---------------------------------------------------
+    def pm_gravity_deposit(self, rho_gas, x, y, z, m, rho_tot):
+        """rho_tot := rho_gas + CIC deposit of the particle masses (device tensors; rho_gas may be None)."""
+        n = int(x.numel())
+        self._chk(self.L.pm_gravity_deposit(self.h, _dptr(rho_gas), n, _dptr(x), _dptr(y), _dptr(z), _dptr(m), _dptr(rho_tot)),
+                  "pm_gravity_deposit")
+
+    def pm_gravity_kick(self, gx, gy, gz, x, y, z, v=None, dt: float = 0.0, a=None):
+        """a_s = CIC interpolation of (gx, gy, gz); v += a dt when v = (vx, vy, vz) is given; a = (ax, ay, az) optional outputs."""
+        n = int(x.numel())
+        vv = v if v is not None else (None, None, None)
+        aa = a if a is not None else (None, None, None)
+        self._chk(self.L.pm_gravity_kick(self.h, _dptr(gx), _dptr(gy), _dptr(gz), n, _dptr(x), _dptr(y), _dptr(z),
+                                         _dptr(vv[0]), _dptr(vv[1]), _dptr(vv[2]), float(dt), _dptr(aa[0]), _dptr(aa[1]), _dptr(aa[2])),
+                  "pm_gravity_kick")
+
+    def pm_drift(self, x, y, z, vx, vy, vz, dt: float):
+        n = int(x.numel())
+        self._chk(self.L.pm_drift(self.h, n, _dptr(x), _dptr(y), _dptr(z), _dptr(vx), _dptr(vy), _dptr(vz), float(dt)), "pm_drift")
 
     def pm_set_repro_margin(self, M: int):
         self._chk(self.L.pm_set_repro_margin(self.h, int(M)), "pm_set_repro_margin")
