@@ -55,8 +55,8 @@ __global__ void __launch_bounds__(256) k_grav_deposit(const DevP P, const double
 // Step 5 (Eq. 6 with eta = 1, L95): rho_tot = rho_gas + folded buffer, owned cells only.  VEC = 2 uses 128-bit accesses
 // (nx even; the ghosted row origin gx is even by construction).  rho_gas == nullptr: particles only.
 template <int VEC>
-__global__ void __launch_bounds__(256) k_grav_apply(const DevP P, const double *__restrict__ rho_gas, const double *__restrict__ buf,
-                                                    double *__restrict__ rho_tot) {
+__global__ void __launch_bounds__(256) k_grav_apply(const DevP P, const double *rho_gas, const double *__restrict__ buf,
+                                                    double *rho_tot) {   // rho_gas may alias rho_tot: no __restrict__ on the two
     const long long nv = P.N / VEC;
     const int nxv = P.nx / VEC;
     for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < nv; t += (long long)gridDim.x * blockDim.x) {

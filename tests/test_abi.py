@@ -60,6 +60,9 @@ def test_argument_validation_without_gpu(built):
     assert L.pm_create(C.byref(p), 0, None, C.byref(h)) == pm.PM_EINVAL
     assert L.pm_fold_ghosts(None) == pm.PM_EINVAL
     assert L.pm_destroy(None) == pm.PM_EINVAL
+    assert L.pm_gravity_deposit(None, None, 0, None, None, None, None, None) == pm.PM_EINVAL
+    assert L.pm_gravity_kick(None, None, None, None, 0, None, None, None, None, None, None, 0.0, None, None, None) == pm.PM_EINVAL
+    assert L.pm_drift(None, 0, None, None, None, None, None, None, 0.0) == pm.PM_EINVAL
 
 
 @pytest.mark.skipif(torch.cuda.is_available(), reason="checks the no-GPU failure mode")
