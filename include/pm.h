@@ -144,7 +144,12 @@ int pm_create_sinks(pm_ctx *ctx, pm_state *state, int64_t max_new, double *x, do
  * Kernel W: cloud-in-cell (R40).  Per axis s = (x - x0)/dx - 1/2, i0 = floor(s), f = s - i0; cells i0, i0 + 1 get 1 - f, f;
  * W_ijk = (W_z W_y) W_x; r_K = dx, so one ghost layer contains it (L59).  All pointers DEVICE, fp64, contiguous; particle
  * arrays hold n values, mesh arrays nx*ny*nz (x fastest, no ghosts).  Particles must lie in [x0, x0 + n dx) (else
- * PM_EDOMAIN at the next pm_check).  Asynchronous on the ctx's stream. */
+ * PM_EDOMAIN at the next pm_check).  Asynchronous on the ctx's stream.
+ * Order of work: from 65536 particles on, both kernels take the particles in the a1 bin order (a counting sort of the
+ * host tiles on the device, no comparison sort; the particle arrays themselves are never permuted), which keeps the mesh
+ * sectors of neighbouring particles together in DRAM pages and L2.  The order is cached in the ctx between a
+ * pm_gravity_deposit and the pm_gravity_kick on the same x pointer and n, and dropped by pm_drift and pm_deposit.  Results
+ * do not depend on it except through the order of the deposit's atomic additions. */
 
 /* rho_tot := rho_gas + sum_s m_s W(x_ijk - x_s) / V (L51: "depositing particle mass into the gas density field for the
  * purposes of computing the gravitational potential").  Step 1: buffer channel 0 is zeroed and receives the eight fp64

@@ -63,6 +63,7 @@ struct pm_ctx {
     int nch;            // buffer channels allocated: 6, or 10 with PM_FLAG_REPRODUCIBLE
     bool repro; int repro_M;
     int *create_mem; long long create_cap;   // sink creation scratch: [0] = count, [1 ..] = list
+    const double *gperm_x; long long gperm_n; bool gperm_valid;   // gravity: perm in bin_mem orders the n particles at gperm_x by host tile
     bool buffer_valid;  // a deposit + fold has filled the buffer mesh (sink creation reads its accretion channel)
     bool timing;        // PM_FLAG_TIMING
     cudaEvent_t ev[PM_NUM_KERNELS][2];
@@ -765,6 +766,7 @@ extern "C" int pm_deposit(pm_ctx *c, const pm_state *st, const pm_sinks *sk, con
     if (dbg && (rc = grow(c, &c->dbg_sn, &c->cap_dbg_sn, 9 * nn)) != PM_OK) return rc;
 
     for (int k = 0; k < PM_NUM_KERNELS; ++k) c->ev_used[k] = false;
+    c->gperm_valid = false;      // the bins below reuse bin_mem
     const long long np = nk + nn;
     int *keys = nullptr, *perm = nullptr, *counts = nullptr;
     if (np > 0) {   // a1: bin particles by host tile
@@ -986,6 +988,45 @@ static int fold_channel0(pm_ctx *c) {
     return check_launch(c, "k_fold_ghosts<1 channel>");
 }
 
+// Particles in a1 bin order for the gravity kernels (a counting sort by host tile, no comparison sort): *perm_out lists the
+// particle indices tile by tile, or is NULL for small sets (order does not matter below the L2 size).  The permutation only
+// decides which thread takes which particle; results do not depend on it (interpolation) or only through the order of the
+// atomic additions (deposit).
+constexpr long long kGravSortMin = 1 << 16;
+static int grav_order(pm_ctx *c, const double *x, const double *y, const double *z, long long n, const int **perm_out) {
+    *perm_out = nullptr;
+    if (n < kGravSortMin) return PM_OK;
+    if (n >= (1ll << 31)) PM_FAIL(c, PM_EINVAL, "too many particles");
+    const DevP &P = c->P;
+    const int nkeys = 2 * P.ntile + 1;
+    const int nscan = (nkeys + kScanChunk - 1) / kScanChunk;
+    if (c->gperm_valid && c->gperm_x == x && c->gperm_n == n) { *perm_out = c->bin_mem + n; return PM_OK; }
+    c->gperm_valid = false;
+    const long long need = 2 * n + nkeys + nscan;
+    if (need > c->bin_cap) {
+        if (c->bin_mem) { PM_CUDA(c, cudaFree(c->bin_mem)); c->bin_mem = nullptr; c->bin_cap = 0; }
+        const long long cap = need + need / 4;
+        cudaError_t e = cudaMalloc(&c->bin_mem, (size_t)cap * sizeof(int));
+        if (e != cudaSuccess) { c->bin_mem = nullptr; PM_FAIL(c, PM_ENOMEM, "cudaMalloc of bins failed: %s", cudaGetErrorString(e)); }
+        c->bin_cap = cap;
+    }
+    int *keys = c->bin_mem, *perm = keys + n, *counts = perm + n, *sums = counts + nkeys;
+    int rc;
+    PM_CUDA(c, cudaMemsetAsync(counts, 0, (size_t)nkeys * sizeof(int), c->stream));
+    const unsigned blocks = (unsigned)((n + 255) / 256);
+    k_bin_count<<<blocks, 256, 0, c->stream>>>(P, x, y, z, n, nullptr, nullptr, nullptr, 0, keys, counts);
+    if ((rc = check_launch(c, "k_bin_count")) != PM_OK) return rc;
+    k_bin_scan_local<<<nscan, 256, 0, c->stream>>>(counts, nkeys, sums);
+    if ((rc = check_launch(c, "k_bin_scan_local")) != PM_OK) return rc;
+    k_bin_scan_sums<<<1, 1024, 0, c->stream>>>(sums, nscan);
+    if ((rc = check_launch(c, "k_bin_scan_sums")) != PM_OK) return rc;
+    k_bin_fill<<<blocks, 256, 0, c->stream>>>(keys, counts, sums, perm, n, n);
+    if ((rc = check_launch(c, "k_bin_fill")) != PM_OK) return rc;
+    c->gperm_x = x; c->gperm_n = n; c->gperm_valid = true;
+    *perm_out = perm;
+    return PM_OK;
+}
+
 extern "C" int pm_gravity_deposit(pm_ctx *c, const double *rho_gas, int64_t n, const double *x, const double *y, const double *z,
                                   const double *m, double *rho_tot) {
     if (!c) return PM_EINVAL;
@@ -1000,7 +1041,9 @@ extern "C" int pm_gravity_deposit(pm_ctx *c, const double *rho_gas, int64_t n, c
     int rc;
     PM_CUDA(c, cudaMemsetAsync(c->buf, 0, (size_t)P.Nb * sizeof(double), c->stream));     // Step 1: "initialized to zero" (L59)
     if (n > 0) {
-        k_grav_deposit<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(P, x, y, z, m, n, c->buf, c->err_flag);
+        const int *perm;
+        if ((rc = grav_order(c, x, y, z, n, &perm)) != PM_OK) return rc;
+        k_grav_deposit<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(P, x, y, z, m, n, perm, c->buf, c->err_flag);
         if ((rc = check_launch(c, "k_grav_deposit")) != PM_OK) return rc;
     }
     if ((rc = fold_channel0(c)) != PM_OK) return rc;                                       // Step 2
@@ -1026,7 +1069,10 @@ extern "C" int pm_gravity_kick(pm_ctx *c, const double *gx, const double *gy, co
     if (has_a && !(ax && ay && az)) PM_FAIL(c, PM_EINVAL, "pm_gravity_kick: give all of ax, ay, az or none");
     if (!has_v && !has_a) PM_FAIL(c, PM_EINVAL, "pm_gravity_kick: nothing to write (no velocities, no acceleration output)");
     PM_CUDA(c, cudaSetDevice(c->device));
-    k_grav_kick<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(c->P, gx, gy, gz, n, x, y, z, vx, vy, vz, dt, ax, ay, az, c->err_flag);
+    const int *perm;
+    int rc;
+    if ((rc = grav_order(c, x, y, z, n, &perm)) != PM_OK) return rc;
+    k_grav_kick<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(c->P, gx, gy, gz, n, x, y, z, vx, vy, vz, dt, ax, ay, az, perm, c->err_flag);
     return check_launch(c, "k_grav_kick");
 }
 
@@ -1039,6 +1085,7 @@ extern "C" int pm_drift(pm_ctx *c, int64_t n, double *x, double *y, double *z, c
     if (c->stage == ST_APPLIED)
         PM_FAIL(c, PM_EORDER, "pm_drift: pm_return_to_particles needs the positions of the preceding pm_deposit; call it first");
     PM_CUDA(c, cudaSetDevice(c->device));
+    c->gperm_valid = false;      // positions change: the cached order is stale (still a valid permutation, but not reused)
     k_drift<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(c->P, n, x, y, z, vx, vy, vz, dt, c->err_flag);
     return check_launch(c, "k_drift");
 }

@@ -24,9 +24,11 @@ __device__ __forceinline__ void cic_axis(double x, double x0, double inv_dx, int
 // particle: the two x-neighbours of a row are adjacent in memory (one 32-byte sector three times out of four).
 __global__ void __launch_bounds__(256) k_grav_deposit(const DevP P, const double *__restrict__ px, const double *__restrict__ py,
                                                       const double *__restrict__ pz, const double *__restrict__ pm_,
-                                                      long long n, double *__restrict__ buf, int *__restrict__ err_flag) {
-    const long long s = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (s >= n) return;
+                                                      long long n, const int *__restrict__ perm, double *__restrict__ buf,
+                                                      int *__restrict__ err_flag) {
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= n) return;
+    const long long s = perm ? perm[t] : t;      // particles taken in a1 bin order (DRAM page / L2 sector locality)
     const double x = px[s], y = py[s], z = pz[s], m = pm_[s];
     int i0, j0, k0;
     double wx[2], wy[2], wz[2];
@@ -84,9 +86,11 @@ __global__ void __launch_bounds__(256) k_grav_kick(const DevP P, const double *_
                                                    const double *__restrict__ py, const double *__restrict__ pz,
                                                    double *__restrict__ vx, double *__restrict__ vy, double *__restrict__ vz,
                                                    double dt, double *__restrict__ ax, double *__restrict__ ay,
-                                                   double *__restrict__ az, int *__restrict__ err_flag) {
-    const long long s = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (s >= n) return;
+                                                   double *__restrict__ az, const int *__restrict__ perm,
+                                                   int *__restrict__ err_flag) {
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= n) return;
+    const long long s = perm ? perm[t] : t;
     const double x = px[s], y = py[s], z = pz[s];
     int i0, j0, k0;
     double wx[2], wy[2], wz[2];

@@ -255,3 +255,44 @@ def test_full_size_sampled_and_invariants():
         ref = go.gravity_interpolate(p, w.g[c], w.x[pick], w.y[pick], w.z[pick])
         assert np.array_equal(a[c].cpu().numpy()[pick], ref)
     ctx.close()
+
+
+def test_bin_ordered_path_above_the_sort_threshold():
+    """n >= 65536 particles: the library takes the particles in a1 bin order (a cached permutation shared by the deposit and
+    the kick, invalidated by pm_drift).  Same checks as the small cases, then a drift and a second deposit + kick, which must
+    follow the NEW positions (a stale order would still be a valid permutation; a stale index would not be)."""
+    w = inputs.gravity_workload(64, 100_000, seed_index=11)
+    check_deposit(w)
+    check_kick_and_drift(w)
+    p = w.params
+    ctx = pm.Context(p, device=DEV)
+    x, y, z, m = dev(w.x), dev(w.y), dev(w.z), dev(w.m)
+    v = [dev(w.vx), dev(w.vy), dev(w.vz)]
+    gx, gy, gz = (dev(a) for a in w.g)
+    rho = torch.empty((64, 64, 64), dtype=torch.float64, device=DEV)
+    ctx.pm_gravity_deposit(None, x, y, z, m, rho)                  # builds and caches the order
+    ctx.pm_drift(x, y, z, v[0], v[1], v[2], 37.0)                  # invalidates it
+    ctx.pm_gravity_deposit(None, x, y, z, m, rho)
+    a = [torch.empty_like(x) for _ in range(3)]
+    ctx.pm_gravity_kick(gx, gy, gz, x, y, z, a=a)                  # reuses the order of the second deposit
+    ctx.pm_check()
+    pos = [go.drift(q, vv, 37.0, 0.0, 64, 1.0) for q, vv in zip((w.x, w.y, w.z), (w.vx, w.vy, w.vz))]
+    for c, q in enumerate((x, y, z)):
+        assert np.array_equal(q.cpu().numpy(), pos[c])
+    ref = go.gravity_deposit(p, None, pos[0], pos[1], pos[2], w.m)
+    got = rho.cpu().numpy()
+    assert np.array_equal(got != 0, ref != 0)
+    assert np.all(np.abs(got - ref) <= 1e-12 * np.abs(ref) + 1e-300)
+    for c in range(3):
+        assert np.array_equal(a[c].cpu().numpy(), go.gravity_interpolate(p, w.g[c], *pos))
+    # an exchange step in between reuses the bin memory: the gravity order must be rebuilt, not reused
+    wk = inputs.scaled_mixed(64, 2000)
+    st = pm.DeviceState.from_host(wk.state, torch.device(DEV))
+    sk = pm.DeviceSinks.from_host(wk.sinks, torch.device(DEV))
+    sn = pm.DeviceSNe.from_host(wk.sne, torch.device(DEV))
+    ctx.step(st, sk, sn, wk.dt)
+    ctx.pm_gravity_kick(gx, gy, gz, x, y, z, a=a)
+    ctx.pm_check()
+    for c in range(3):
+        assert np.array_equal(a[c].cpu().numpy(), go.gravity_interpolate(p, w.g[c], *pos))
+    ctx.close()
