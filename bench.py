@@ -322,6 +322,18 @@ def run_ours(args, rank, world, local_rank):
             gravity[name] = {"ms": ms_, "algorithmic_bytes": b_, "achieved_gbs": b_ / (ms_ * 1e-3) / 1e9,
                              "frac_of_measured_peak": b_ / (ms_ * 1e-3) / 1e9 / peak_g}
         gravity["particles_per_s_kdk_half"] = npart / (sum(gms) * 1e-3)
+        if not args.no_cpu_baseline:       # the gravity oracle as it stands, on a 128^3 block with the same particles per cell
+            from oracle import pm_gravity_oracle as go
+            ow = inputs.gravity_workload(128, max(npart // 64, 1))
+            t0 = time.perf_counter()
+            go.gravity_deposit(ow.params, ow.rho_gas, ow.x, ow.y, ow.z, ow.m)
+            oa = [go.gravity_interpolate(ow.params, ow.g[c], ow.x, ow.y, ow.z) for c in range(3)]
+            ov = [go.kick(v_, a_, 0.5 * ow.dt) for v_, a_ in zip((ow.vx, ow.vy, ow.vz), oa)]
+            for c, q in enumerate((ow.x, ow.y, ow.z)):
+                go.drift(q, ov[c], ow.dt, 0.0, 128, 1.0)
+            osec = time.perf_counter() - t0
+            gravity["cpu_baseline"] = {"value": ow.x.size / osec, "unit": "particles/s (one KDK half: deposit + kick + drift)", "cores": 1,
+                                       "kind": "oracle", "sample": f"128^3 block, {ow.x.size} particles (same particles per cell), {osec:.3f} s"}
         del gpos, gvel, gm, gmesh, rho_tot
 
     # ---- e2e through pm_step_host with pinned host buffers --------------------------------------
