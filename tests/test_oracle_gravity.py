@@ -239,3 +239,21 @@ def test_drift_wraps_into_the_box():
     # a result that rounds onto the upper face goes to the lower face (R41)
     xn = go.drift(np.array([-3.0]), np.array([-1e-30]), 1.0, lo, n, dx)
     assert xn[0] == lo
+
+
+def test_gravity_workload_is_seeded_and_inside_the_box():
+    """The shared input generator (no method arithmetic): same seed -> same arrays; every particle inside [x0, x0 + n dx)."""
+    from paper_2509_18261_b200 import inputs
+    a = inputs.gravity_workload(24, 500, seed_index=8, shape=(24, 20, 28), dx=0.37, x0=(-3.0, 11.5, 0.125))
+    b = inputs.gravity_workload(24, 500, seed_index=8, shape=(24, 20, 28), dx=0.37, x0=(-3.0, 11.5, 0.125))
+    for f in ("x", "y", "z", "vx", "vy", "vz", "m", "rho_gas"):
+        assert np.array_equal(getattr(a, f), getattr(b, f))
+    p = a.params
+    for q, lo, n in ((a.x, -3.0, 24), (a.y, 11.5, 20), (a.z, 0.125, 28)):
+        assert q.min() >= lo and q.max() < lo + n * 0.37
+        i0, w0, w1 = go.cic_axis(q, lo, 0.37)
+        assert i0.min() >= -1 and i0.max() <= n - 1 and w0.min() >= 0 and w1.min() >= 0
+    assert a.rho_gas.shape == (28, 20, 24) and a.g[0].shape == (28, 20, 24)
+    assert p["rk_sink"] / p["dx"] <= 4 and p["rk_sn"] / p["dx"] <= 3
+    c = inputs.gravity_workload(24, 500, seed_index=9)
+    assert not np.array_equal(c.x[:10], inputs.gravity_workload(24, 500, seed_index=8).x[:10])
