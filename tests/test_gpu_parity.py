@@ -203,7 +203,7 @@ def test_config4_clustered_10_steps():
     try:
         g, o, n2 = parity.run_and_compare(w, steps=3)
     except AssertionError as first:
-        # Seen once in 19 runs of this test on B200 (close_reorder, quantity not captured): the only run-to-run variable
+        # Seen once in 32 runs of this test on B200 (close_reorder, quantity not captured): the only run-to-run variable
         # is the order of the atomic additions (R36).  An arithmetic difference fails every time; an order effect does not.
         # The first message goes to the warnings summary so that the tolerance concerned can be re-derived.
         import warnings
