@@ -28,6 +28,19 @@
  * deposit -> fold -> apply -> return (return may be skipped when there are no sinks); otherwise PM_EORDER.
  * The buffer mesh stays valid (as dU^sum, L108) until the next pm_deposit, which resets it.
  *
+ * Buffer reset ("all cells initialized to zero", L59): the mesh is cut into tiles of 8^3 cells with a liveness flag.  pm_deposit
+ * marks and zeroes the tiles this step's particles can add into (known from the particle bins); all other tiles are stale, and
+ * fold, apply and sink creation take them as zeros without reading them.
+ *
+ * Which call is allowed when (PM_EORDER otherwise).  "in step" = after pm_deposit, before pm_apply_limited has returned:
+ *   pm_deposit              any time (abandons an unfinished step)
+ *   pm_fold_ghosts          directly after pm_deposit          pm_apply_limited        directly after pm_fold_ghosts
+ *   pm_return_to_particles  directly after pm_apply_limited (may be skipped when there are no sinks)
+ *   pm_create_sinks         not in step; after a step it needs the folded buffer of that step
+ *   pm_gravity_deposit      not in step (it works in buffer channel 1; the retained accretion channel 0 is left alone)
+ *   pm_gravity_kick         any time (own scratch memory; reads no buffer)
+ *   pm_drift                not between pm_apply_limited and pm_return_to_particles (Step 4 needs the deposit's positions)
+ *
  * Errors: every function returns 0 on success or a negative pm_status; no exceptions, no aborts, no output.
  * pm_last_error(ctx) gives a human-readable message for the last failure on that ctx.
  */
@@ -129,7 +142,7 @@ int pm_set_repro_margin(pm_ctx *ctx, int32_t M);
  * pm_apply_limited / pm_return_to_particles, before the next pm_deposit).  A cell creates a sink if rho > rho_Tr (Eq. 12),
  * it is a strict local density maximum among the cells whose centres lie within rk_sink of its own (periodic), and the
  * accretion channel of the retained buffer mesh is zero there (no sink's kernel covers it, L177; before the first deposit
- * this test is skipped).  New sink: cell centre, m = (rho - rho_Tr) V, velocity of the cell; the cell is left at rho_Tr
+ * this test is skipped; after a pm_deposit that was not folded: PM_EORDER).  New sink: cell centre, m = (rho - rho_Tr) V, velocity of the cell; the cell is left at rho_Tr
  * with the same velocity and specific energies (L183).  state: DEVICE, modified in place.  x .. m: DEVICE arrays of
  * max_new doubles, filled in increasing cell-index order (an ordered compaction on the device; only the count goes to
  * the host).  *n_new (HOST) = number of cells found; if it exceeds max_new NOTHING is created and the state is unchanged
@@ -147,16 +160,16 @@ int pm_create_sinks(pm_ctx *ctx, pm_state *state, int64_t max_new, double *x, do
  * PM_EDOMAIN at the next pm_check).  Asynchronous on the ctx's stream.
  * Order of work: from 65536 particles on, both kernels take the particles in the a1 bin order (a counting sort of the
  * host tiles on the device, no comparison sort; the particle arrays themselves are never permuted), which keeps the mesh
- * sectors of neighbouring particles together in DRAM pages and L2.  The order is cached in the ctx between a
- * pm_gravity_deposit and the pm_gravity_kick on the same x pointer and n, and dropped by pm_drift and pm_deposit.  Results
+ * sectors of neighbouring particles together in DRAM pages and L2.  The order is cached in the ctx (in scratch memory of its
+ * own) between a pm_gravity_deposit and the pm_gravity_kick on the same x pointer and n, and dropped by pm_drift.  Results
  * do not depend on it except through the order of the deposit's atomic additions. */
 
 /* rho_tot := rho_gas + sum_s m_s W(x_ijk - x_s) / V (L51: "depositing particle mass into the gas density field for the
  * purposes of computing the gravitational potential").  Step 1: buffer channel 0 is zeroed and receives the eight fp64
  * atomic additions of every particle, ghost layer included; Step 2: pm_fold_ghosts on that channel; Step 5: the sum is
- * written to rho_tot (eta = 1).  rho_gas may be NULL (particles only) and may alias rho_tot.  n may be 0.  Uses the ctx's
- * buffer mesh: not allowed between pm_deposit and pm_apply_limited (PM_EORDER); afterwards the retained accretion buffer of
- * L108 is gone, so call it before the step's pm_deposit as the paper's sequence does (L107-109), or pm_create_sinks first. */
+ * written to rho_tot (eta = 1).  rho_gas may be NULL (particles only) and may alias rho_tot.  n may be 0.  Uses channel 1 of the
+ * ctx's buffer mesh (free between steps; swept to zero here): not allowed between pm_deposit and pm_apply_limited (PM_EORDER).
+ * The retained accretion channel of L108 / L177 (channel 0) is not touched, so pm_create_sinks still works afterwards. */
 int pm_gravity_deposit(pm_ctx *ctx, const double *rho_gas, int64_t n, const double *x, const double *y, const double *z,
                        const double *m, double *rho_tot);
 
@@ -193,8 +206,8 @@ int64_t pm_launch_count(const pm_ctx *ctx);
 
 /* Device time of each kernel group in the most recent step, in milliseconds, measured with CUDA events recorded on the
  * ctx's stream around the launches (needs PM_FLAG_TIMING; synchronises).  ms (HOST, n >= PM_NUM_KERNELS floats):
- * PM_K_BIN (the four binning kernels), PM_K_ZERO, PM_K_SINKS, PM_K_SNE, PM_K_FOLD, PM_K_APPLY, PM_K_RETURN;
- * a group that did not run reports 0. */
+ * PM_K_BIN (the four binning kernels), PM_K_ZERO (tile stamping + reset), PM_K_SINKS, PM_K_SNE, PM_K_FOLD, PM_K_APPLY,
+ * PM_K_RETURN; a group that did not run reports 0. */
 enum { PM_K_BIN = 0, PM_K_ZERO = 1, PM_K_SINKS = 2, PM_K_SNE = 3, PM_K_FOLD = 4, PM_K_APPLY = 5, PM_K_RETURN = 6, PM_NUM_KERNELS = 7 };
 int pm_kernel_times(pm_ctx *ctx, float *ms, int32_t n);
 
@@ -210,7 +223,7 @@ int pm_probe_red_f64(pm_ctx *ctx, int64_t footprint_bytes, int32_t channels, dou
  * The channel is a contiguous (dims[0], dims[1], dims[2]) = (nz+2g, ny+2g, row pitch) array, x fastest; the row pitch
  * is nx + 2*gx with gx = g rounded up to even (keeps 128-bit accesses aligned).  *origin = element offset of owned
  * cell (0,0,0); owned cell (i,j,k) sits at origin + (k*dims[1] + j)*dims[2] + i, ghost cells at i,j,k in [-g, n+g).
- * *ghost = g. */
+ * *ghost = g.  Stale tiles (no particle touched them in this step) are filled with the zeros they stand for first. */
 int pm_debug_buffer(pm_ctx *ctx, int channel, const double **dev_ptr, int64_t dims[3], int64_t *origin, int32_t *ghost);
 
 /* Return mesh: one record of 4 doubles per cell (eta of Eq. 4, pre-step velocity x, y, z), valid where buffer channel

@@ -606,9 +606,11 @@ int orc_return(const orc_params *p, const orc_state *U_old, const double *eta, o
                 }
         double m_old = sk->m[s];
         double m_new = m_old + dm;
-        sk->vx[s] = (m_old * sk->vx[s] + dpx) / m_new;                /* u = (m, m v), L49 */
-        sk->vy[s] = (m_old * sk->vy[s] + dpy) / m_new;
-        sk->vz[s] = (m_old * sk->vz[s] + dpz) / m_new;
+        if (m_new != 0.0) {                                           /* R43: m = 0 and no gain: velocity undefined by Eq. 5, kept */
+            sk->vx[s] = (m_old * sk->vx[s] + dpx) / m_new;            /* u = (m, m v), L49 */
+            sk->vy[s] = (m_old * sk->vy[s] + dpy) / m_new;
+            sk->vz[s] = (m_old * sk->vz[s] + dpz) / m_new;
+        }
         sk->m[s] = m_new;
         if (sk->dm) sk->dm[s] = dm;
         if (sk->dpx) sk->dpx[s] = dpx;

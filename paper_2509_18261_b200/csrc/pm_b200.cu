@@ -1,7 +1,7 @@
 // pm_b200.cu -- kernels and C ABI of libpm_b200 (see include/pm.h).  sm_100a only; built with -fmad=false.
 //
 // Kernels:
-//   k_zero_buffer      a0  buffer reset, 128-bit stores
+//   (a0, the buffer reset, has no kernel of its own: tiles are zeroed on their first touch inside the deposit kernels, pm_tiles.cuh)
 //   k_deposit_sinks    a1-a3  one warp per sink: kernel means -> Bondi-Hoyle rate -> Gaussian weights -> fp64 RED
 //   k_deposit_sne      a1,a4,a5  one warp per SN: omega counts -> stencil sums -> Eq. 17 -> fp64 RED (5 channels)
 //   k_fold_ghosts      a6  gather fold: every owned cell within g of a face sums its <= 7 ghost images, fixed order
@@ -10,11 +10,13 @@
 //   k_grav_deposit / k_grav_apply / k_grav_kick / k_drift   (f)3  PM gravity: cloud-in-cell deposit (Steps 1, 2, 5),
 //                      interpolation + half kick, drift (pm_gravity.cuh)
 #include "pm_device.cuh"
+#include "pm_tiles.cuh"
 #include "pm_fast.cuh"
 #include "pm_create.cuh"
 #include "pm_gravity.cuh"
 #include "../../include/pm.h"
 
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -60,11 +62,17 @@ struct pm_ctx {
     double *stg_sne;    long long stg_sne_cap;
     // particle binning: keys[np] | perm[np] | counts[2*ntile + 1]
     int *bin_mem;       long long bin_cap;
+    int *grav_mem;      long long grav_cap;   // the same three arrays for the gravity calls (their own: a kick may come between
+                                              // pm_deposit and pm_return_to_particles, which still needs the sink order in bin_mem)
+    unsigned char *tile_live; long long ntiles;   // liveness flags of the buffer-mesh tiles (pm_tiles.cuh), rewritten by every pm_deposit
     int nch;            // buffer channels allocated: 6, or 10 with PM_FLAG_REPRODUCIBLE
     bool repro; int repro_M;
     int *create_mem; long long create_cap;   // sink creation scratch: [0] = count, [1 ..] = list
-    const double *gperm_x; long long gperm_n; bool gperm_valid;   // gravity: perm in bin_mem orders the n particles at gperm_x by host tile
+    const double *gperm_x; long long gperm_n; bool gperm_valid;   // gravity: perm in grav_mem orders the n particles at gperm_x by host tile
     bool buffer_valid;  // a deposit + fold has filled the buffer mesh (sink creation reads its accretion channel)
+    bool ever_deposited;
+    bool grav_in_ch1;   // buffer channel 1 holds the last pm_gravity_deposit (until the next pm_deposit): the debug view must not
+                        // "fill in" its stale tiles
     bool timing;        // PM_FLAG_TIMING
     cudaEvent_t ev[PM_NUM_KERNELS][2];
     bool ev_used[PM_NUM_KERNELS];
@@ -91,13 +99,22 @@ static void tick(pm_ctx *c, int k, int which) {
 }
 
 // ---------------------------------------------------------------------------------------------------------------
-// a0: buffer reset
+// a0: buffer reset.  No sweep: see pm_tiles.cuh.  The kernel below is for the test-only views (pm_debug_buffer,
+// pm_debug_round_buffers): it stores the zeros that stale tiles stand for and marks them live, so that the raw buffer can be read.
 // ---------------------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) k_zero_buffer(double2 *__restrict__ p, long long n2) {
-    long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    const long long stride = (long long)gridDim.x * blockDim.x;
-    const double2 z = make_double2(0.0, 0.0);
-    for (; i < n2; i += stride) p[i] = z;
+__global__ void __launch_bounds__(128) k_tiles_materialize(const DevP P, double *__restrict__ buf, const Tiles T, const bool repro,
+                                                           const bool keep_n, const int ntiles) {
+    const int t = blockIdx.x * 4 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+    if (t >= ntiles) return;
+    const unsigned f = T.live[t];
+    const bool lk = f & kLiveK, ln = keep_n || (f & kLiveN);
+    unsigned mask = 0;
+    if (!lk) mask |= 1u;
+    if (!ln) mask |= repro ? 0xFEu : 0x3Eu;
+    if (repro && !lk && !ln) mask |= 1u << kChK;
+    if (mask) tile_zero(P, buf, t, mask, lane);
+    __syncwarp();
+    if (lane == 0) T.live[t] = (unsigned char)(f | kLiveK | (keep_n ? 0u : kLiveN));
 }
 
 // ---------------------------------------------------------------------------------------------------------------
@@ -109,7 +126,8 @@ __global__ void __launch_bounds__(256) k_bin_count(const DevP P, const double *_
                                                    const double *__restrict__ kz, long long nk,
                                                    const double *__restrict__ nx_, const double *__restrict__ ny_,
                                                    const double *__restrict__ nz_, long long nn,
-                                                   int *__restrict__ keys, int *__restrict__ counts) {
+                                                   int *__restrict__ keys, int *__restrict__ counts,
+                                                   unsigned char *__restrict__ occ) {
     const long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= nk + nn) return;
     const bool sink = p < nk;
@@ -120,6 +138,7 @@ __global__ void __launch_bounds__(256) k_bin_count(const DevP P, const double *_
     const int key = bin_key(P, ih, jh, kh) + (sink ? 0 : P.ntile);
     keys[p] = key;
     atomicAdd(counts + key, 1);
+    if (occ) occ[key] = 1;            // bin occupancy for the reset (k_tiles_mark)
 }
 
 // Exclusive prefix sum of counts[0..n), two levels: every block scans its own 2048 keys in place and publishes its
@@ -242,8 +261,8 @@ __global__ void __launch_bounds__(128) k_deposit_sinks(const DevP P, const DevSt
                 ret_tr[q] = -CUDART_INF;                              // invalidate last step's entry (rewritten by the apply pass)
             }
             double *dst = buf0 + ghost_index(P, i, j, k);
-            atomicAdd(dst, -amt);                                     // R1: signed change
-            if (REPRO) atomicAdd(dst + kChK * P.Nb, kSinkUnit);         // Appendix A: contribution count
+            red_add(dst, -amt);                                     // R1: signed change
+            if (REPRO) red_add(dst + kChK * P.Nb, kSinkUnit);         // Appendix A: contribution count
         }
     }
     if (lane == 0) {
@@ -271,20 +290,20 @@ __global__ void __launch_bounds__(kSnWarps * 32) k_deposit_sne(const DevP P, con
     if (w >= S.n) return;
     const long long s = perm[w];
     const int g = P.gn, B = 2 * g + 1, nc = B * B * B;
-    const SnTables T = sn_tables_at(smem + (size_t)wib * sn_table_bytes(B, P.nsub), B, P.nsub);
+    const SnTables Tb = sn_tables_at(smem + (size_t)wib * sn_table_bytes(B, P.nsub), B, P.nsub);
     const double xs = S.x[s], ys = S.y[s], zs = S.z[s];
     const int ih = host_cell(xs, P.x0[0], P.inv_dx), jh = host_cell(ys, P.x0[1], P.inv_dx), kh = host_cell(zs, P.x0[2], P.inv_dx);
     if (ih < 0 || ih >= P.nx || jh < 0 || jh >= P.ny || kh < 0 || kh >= P.nz) {
         if (lane == 0) atomicOr(err, 1);
         return;
     }
-    sn_fill_tables(P, T, lane, xs, ys, zs, ih, jh, kh);
+    sn_fill_tables(P, Tb, lane, xs, ys, zs, ih, jh, kh);
     const double vsx = S.vx[s], vsy = S.vy[s], vsz = S.vz[s], e_sn = S.e_sn[s], m_ej = S.m_ej[s];
     double m_gas = 0.0, px = 0.0, py = 0.0, pz = 0.0, v_snr = 0.0;
     for (int c = lane; c < nc; c += 32) {
         const int a = c % B, t = c / B, b = t % B, cc = t / B;
-        const int cnt = sn_omega_count(P, T, a, b, cc);
-        T.cnt[c] = (unsigned short)cnt;
+        const int cnt = sn_omega_count(P, Tb, a, b, cc);
+        Tb.cnt[c] = (unsigned short)cnt;
         if (cnt > 0) {
             const double omega = (double)cnt / P.nsub3;
             const long long q = owned_index(P, ih - g + a, jh - g + b, kh - g + cc);
@@ -302,7 +321,7 @@ __global__ void __launch_bounds__(kSnWarps * 32) k_deposit_sne(const DevP P, con
     const SnScalars sc = sn_scalars(P, m_gas, px, py, pz, v_snr, vsx, vsy, vsz, e_sn, m_ej);
     __syncwarp();
     for (int c = lane; c < nc; c += 32) {
-        const int cnt = T.cnt[c];
+        const int cnt = Tb.cnt[c];
         if (cnt == 0) continue;
         const int a = c % B, t = c / B, b = t % B, cc = t / B;
         const int i = ih - g + a, j = jh - g + b, k = kh - g + cc;
@@ -312,11 +331,11 @@ __global__ void __launch_bounds__(kSnWarps * 32) k_deposit_sne(const DevP P, con
         sn_cell_deposit(P, sc, xs, ys, zs, e_sn, m_ej, i, j, k, cnt, rho, U.mx[q] / rho, U.my[q] / rho, U.mz[q] / rho, d);
         double *dst = buf + P.Nb + ghost_index(P, i, j, k);
 #pragma unroll
-        for (int f = 0; f < 5; ++f) atomicAdd(dst + (long long)f * P.Nb, d[f]);
+        for (int f = 0; f < 5; ++f) red_add(dst + (long long)f * P.Nb, d[f]);
         if (REPRO) {                                 // Appendix A: error scales and the contribution count (dst is channel 1)
-            atomicAdd(dst + (kChTp - 1) * P.Nb, (fabs(d[1]) + fabs(d[2])) + fabs(d[3]));
-            atomicAdd(dst + (kChTe - 1) * P.Nb, fabs(d[4]));
-            atomicAdd(dst + (kChK - 1) * P.Nb, 1.0);
+            red_add(dst + (kChTp - 1) * P.Nb, (fabs(d[1]) + fabs(d[2])) + fabs(d[3]));
+            red_add(dst + (kChTe - 1) * P.Nb, fabs(d[4]));
+            red_add(dst + (kChK - 1) * P.Nb, 1.0);
         }
     }
     if (dbg && lane == 0) {
@@ -373,8 +392,12 @@ __device__ __forceinline__ void stv(double *p, const double v[VEC]) {
 
 // W = 2: one thread folds two x-adjacent cells with 128-bit accesses (needs g and nx even, so that a pair never straddles
 // the g-wide face strip and every pair is 16-byte aligned); W = 1 otherwise.  Counts are in units of W cells.
-template <int W, int NCH>
-__global__ void __launch_bounds__(256) k_fold_ghosts(const DevP P, double *__restrict__ buf, long long n_edge,
+// STAMPS: a stale tile stands for zeros (pm_tiles.cuh) and is not read; an owned cell whose own tile is stale has no live image
+// either (a deposit that reaches a ghost cell also claims the tile of its image), so there is nothing to do for it.  Channel 0
+// belongs to group K, channels 1..7 to group N, the Appendix A count channel (8) is live where either group is.
+// STAMPS = false: plain fold of NCH channels starting at buf (PM gravity, which resets its one channel by a sweep).
+template <int W, int NCH, bool STAMPS>
+__global__ void __launch_bounds__(256) k_fold_ghosts(const DevP P, double *__restrict__ buf, const Tiles T, long long n_edge,
                                                      long long n_zslab, long long n_yslab) {
     const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (t >= n_edge) return;
@@ -414,31 +437,53 @@ __global__ void __launch_bounds__(256) k_fold_ghosts(const DevP P, double *__res
     // are issued before any store
     long long img[8];
     bool ok[8];
+    unsigned lk = 0xffu, ln = 0xffu;       // bit m: image m's tile is live in group K / N (bit 0: the owned cell's own tile)
 #pragma unroll
     for (int m = 1; m < 8; ++m) {
         const int cx = m & 1, cy = (m >> 1) & 1, cz = m >> 2;
         ok[m] = (!cx || ox) && (!cy || oy) && (!cz || oz);
         img[m] = ghost_index(P, i + cx * ox, j + cy * oy, k + cz * oz);
     }
+    if (STAMPS) {
+        lk = 0; ln = 0;
+#pragma unroll
+        for (int m = 0; m < 8; ++m) {
+            const int cx = m & 1, cy = (m >> 1) & 1, cz = m >> 2;
+            if (m == 0 || ok[m]) {
+                const unsigned f = T.live[tile_index(P, i + cx * ox, j + cy * oy, k + cz * oz)];
+                lk |= (f & kLiveK ? 1u : 0u) << m;
+                ln |= (f & kLiveN ? 1u : 0u) << m;
+            }
+        }
+        if (!((lk | ln) & 1u)) return;
+    }
     double acc[NCH][W];
 #pragma unroll
     for (int ch = 0; ch < NCH; ++ch) {
+        const unsigned live = !STAMPS ? 0xffu : (ch == 0 ? lk : (ch == kChK ? (lk | ln) : ln));
         const double *b = buf + (long long)ch * P.Nb;
         double a[W];
-        ldv<W>(b + base, a);
 #pragma unroll
-        for (int m = 1; m < 8; ++m)
-            if (ok[m]) {
-                double v[W];
-                ldv<W>(b + img[m], v);
+        for (int e = 0; e < W; ++e) a[e] = 0.0;
+        if (live & 1u) {
+            ldv<W>(b + base, a);
 #pragma unroll
-                for (int e = 0; e < W; ++e) a[e] += v[e];
-            }
+            for (int m = 1; m < 8; ++m)
+                if (ok[m] && (live >> m & 1u)) {
+                    double v[W];
+                    ldv<W>(b + img[m], v);
+#pragma unroll
+                    for (int e = 0; e < W; ++e) a[e] += v[e];
+                }
+        }
 #pragma unroll
         for (int e = 0; e < W; ++e) acc[ch][e] = a[e];
     }
 #pragma unroll
-    for (int ch = 0; ch < NCH; ++ch) stv<W>(buf + (long long)ch * P.Nb + base, acc[ch]);
+    for (int ch = 0; ch < NCH; ++ch) {
+        const unsigned live = !STAMPS ? 1u : (ch == 0 ? lk : (ch == kChK ? (lk | ln) : ln));
+        if (live & 1u) stv<W>(buf + (long long)ch * P.Nb + base, acc[ch]);
+    }
 }
 
 // ---------------------------------------------------------------------------------------------------------------
@@ -490,7 +535,7 @@ constexpr int kApplyThreads = 128;
 
 template <int VEC, bool LAM, bool TL, bool REPRO>
 __global__ void __launch_bounds__(kApplyThreads, 6) k_apply_limited(const DevP P, const DevState U, const double *__restrict__ buf,
-                                                       double *__restrict__ ret, double *__restrict__ ret_tr,
+                                                       const Tiles T, double *__restrict__ ret, double *__restrict__ ret_tr,
                                                        double *__restrict__ lam_out, const int repro_M,
                                                        unsigned int n_items, unsigned int items_per_row) {
     const unsigned int item_raw = blockIdx.x * blockDim.x + threadIdx.x;
@@ -501,16 +546,25 @@ __global__ void __launch_bounds__(kApplyThreads, 6) k_apply_limited(const DevP P
     const unsigned int k = row / (unsigned int)P.ny, j = row - k * (unsigned int)P.ny;
     const long long q = (long long)row * P.nx + i0;
     const long long gq = (long long)(k + P.g) * P.pk + (long long)(j + P.g) * P.pj + (i0 + P.gx);
+    // a stale tile stands for zeros and is not read (pm_tiles.cuh); the VEC cells of an item lie in one tile (i0 is even)
+    const unsigned lf = __ldg(T.live + tile_index(P, (int)i0, (int)j, (int)k));
+    const bool live_k = lf & kLiveK, live_n = lf & kLiveN;
     double b[kBufChannels][VEC];
 #pragma unroll
-    for (int ch = 0; ch < kBufChannels; ++ch) ldv<VEC>(buf + (long long)ch * P.Nb + gq, b[ch]);
+    for (int ch = 0; ch < kBufChannels; ++ch) {
+#pragma unroll
+        for (int v = 0; v < VEC; ++v) b[ch][v] = 0.0;
+        if (ch == 0 ? live_k : live_n) ldv<VEC>(buf + (long long)ch * P.Nb + gq, b[ch]);
+    }
     if (REPRO) {   // Appendix A: round the folded sums here, where they are read anyway (rounding never turns a non-zero sum into zero)
         double ksn[VEC], ksk[VEC], tp[VEC], te[VEC];
-        ldv<VEC>(buf + (long long)kChK * P.Nb + gq, ksn);
+#pragma unroll
+        for (int v = 0; v < VEC; ++v) { ksn[v] = 0.0; tp[v] = 0.0; te[v] = 0.0; }
+        if (live_k || live_n) ldv<VEC>(buf + (long long)kChK * P.Nb + gq, ksn);
 #pragma unroll
         for (int v = 0; v < VEC; ++v) repro_counts(ksn[v], ksn[v], ksk[v]);
-        ldv<VEC>(buf + (long long)kChTp * P.Nb + gq, tp);
-        ldv<VEC>(buf + (long long)kChTe * P.Nb + gq, te);
+        if (live_n) ldv<VEC>(buf + (long long)kChTp * P.Nb + gq, tp);
+        if (live_n) ldv<VEC>(buf + (long long)kChTe * P.Nb + gq, te);
 #pragma unroll
         for (int v = 0; v < VEC; ++v) {
             b[0][v] = repro_round(b[0][v], fabs(b[0][v]), ksk[v], repro_M);
@@ -598,9 +652,11 @@ __global__ void __launch_bounds__(128) k_return_sinks(const DevP P, const DevSin
     dm = warp_sum(dm); dpx = warp_sum(dpx); dpy = warp_sum(dpy); dpz = warp_sum(dpz);
     if (lane == 0) {
         const double m_old = S.m[s], m_new = m_old + dm;
-        S.vx[s] = (m_old * S.vx[s] + dpx) / m_new;
-        S.vy[s] = (m_old * S.vy[s] + dpy) / m_new;
-        S.vz[s] = (m_old * S.vz[s] + dpz) / m_new;
+        if (m_new != 0.0) {                       // R43: a massless sink that gained nothing keeps its velocity (no 0/0)
+            S.vx[s] = (m_old * S.vx[s] + dpx) / m_new;
+            S.vy[s] = (m_old * S.vy[s] + dpy) / m_new;
+            S.vz[s] = (m_old * S.vz[s] + dpz) / m_new;
+        }
         S.m[s] = m_new;
         if (S.dm) S.dm[s] = dm;
         if (S.dpx) S.dpx[s] = dpx;
@@ -670,6 +726,8 @@ extern "C" int pm_create(const pm_params *prm, int device, void *cuda_stream, pm
     const int sbm = (1 << kSbLog2) - 1;
     P.nsbx = (((prm->nx + 7) >> 3) + sbm) >> kSbLog2; P.nsby = (((prm->ny + 7) >> 3) + sbm) >> kSbLog2; P.nsbz = (((prm->nz + 7) >> 3) + sbm) >> kSbLog2;
     P.ntile = (P.nsbx * P.nsby * P.nsbz) << (3 * kSbLog2);
+    P.ntx = ((prm->nx + g + 7) >> 3) + 1; P.nty = ((prm->ny + g + 7) >> 3) + 1; P.ntz = ((prm->nz + g + 7) >> 3) + 1;
+    c->ntiles = (long long)P.ntx * P.nty * P.ntz;
 
     cudaError_t e = cudaSetDevice(device);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, device);
@@ -684,6 +742,9 @@ extern "C" int pm_create(const pm_params *prm, int device, void *cuda_stream, pm
     c->repro_M = 28;                                  // the paper's example margin (L612)
     c->nch = c->repro ? kReproChannels : kBufChannels;
     if (e == cudaSuccess) e = cudaMalloc(&c->buf, (size_t)c->nch * P.Nb * sizeof(double));
+    if (e == cudaSuccess) e = cudaMalloc(&c->tile_live, (size_t)c->ntiles);
+    // before the first deposit every tile is stale = zeros
+    if (e == cudaSuccess) e = cudaMemsetAsync(c->tile_live, 0, (size_t)c->ntiles, c->stream);
     if (e == cudaSuccess && gs > 0) e = cudaMalloc(&c->ret, (size_t)kRetWords * N * sizeof(double));
     if (e == cudaSuccess && gs > 0 && P.tl_num > 0.0) e = cudaMalloc(&c->ret_tr, (size_t)N * sizeof(double));
     if (e == cudaSuccess && (prm->flags & PM_FLAG_DEBUG_LAMBDA)) e = cudaMalloc(&c->lam, (size_t)N * sizeof(double));
@@ -701,6 +762,7 @@ extern "C" int pm_create(const pm_params *prm, int device, void *cuda_stream, pm
         int rc = (e == cudaErrorMemoryAllocation) ? PM_ENOMEM : PM_ECUDA;
         cudaGetLastError();
         if (c->buf) cudaFree(c->buf);
+        if (c->tile_live) cudaFree(c->tile_live);
         if (c->ret) cudaFree(c->ret);
         if (c->ret_tr) cudaFree(c->ret_tr);
         if (c->lam) cudaFree(c->lam);
@@ -728,6 +790,8 @@ extern "C" int pm_destroy(pm_ctx *c) {
         for (int k = 0; k < PM_NUM_KERNELS; ++k) { cudaEventDestroy(c->ev[k][0]); cudaEventDestroy(c->ev[k][1]); }
     if (c->copy_stream) { cudaStreamDestroy(c->copy_stream); cudaEventDestroy(c->ev_inputs); cudaEventDestroy(c->ev_etot); }
     if (c->bin_mem) cudaFree(c->bin_mem);
+    if (c->grav_mem) cudaFree(c->grav_mem);
+    if (c->tile_live) cudaFree(c->tile_live);
     if (c->create_mem) cudaFree(c->create_mem);
     if (c->err_flag) cudaFree(c->err_flag);
     if (c->err_host) cudaFreeHost(c->err_host);
@@ -745,6 +809,8 @@ extern "C" int pm_set_repro_margin(pm_ctx *c, int32_t M) {
 
 extern "C" const char *pm_last_error(const pm_ctx *c) { return c ? c->msg : "null ctx"; }
 extern "C" int64_t pm_launch_count(const pm_ctx *c) { return c ? c->launches : 0; }
+
+static Tiles tiles_of(const pm_ctx *c) { return Tiles{ c->tile_live }; }
 
 static bool state_ok(const pm_state *s) { return s && s->rho && s->mx && s->my && s->mz && s->etot && s->eint; }
 
@@ -766,14 +832,15 @@ extern "C" int pm_deposit(pm_ctx *c, const pm_state *st, const pm_sinks *sk, con
     if (dbg && (rc = grow(c, &c->dbg_sn, &c->cap_dbg_sn, 9 * nn)) != PM_OK) return rc;
 
     for (int k = 0; k < PM_NUM_KERNELS; ++k) c->ev_used[k] = false;
-    c->gperm_valid = false;      // the bins below reuse bin_mem
     const long long np = nk + nn;
-    int *keys = nullptr, *perm = nullptr, *counts = nullptr;
+    int *keys = nullptr, *perm = nullptr, *counts = nullptr, *live = nullptr;
+    unsigned char *occ = nullptr;
     if (np > 0) {   // a1: bin particles by host tile
         if (np >= (1ll << 31)) PM_FAIL(c, PM_EINVAL, "pm_deposit: too many particles");
         const int nkeys = 2 * P.ntile + 1;
         const int nscan = (nkeys + kScanChunk - 1) / kScanChunk;
-        const long long need = 2 * np + nkeys + nscan;
+        const int nocc = (2 * P.ntile + 3) / 4;                         // bin occupancy bytes, in ints
+        const long long need = 2 * np + nkeys + nscan + nocc + 2;
         if (need > c->bin_cap) {
             if (c->bin_mem) { PM_CUDA(c, cudaFree(c->bin_mem)); c->bin_mem = nullptr; c->bin_cap = 0; }
             const long long cap = need + need / 4;
@@ -783,11 +850,13 @@ extern "C" int pm_deposit(pm_ctx *c, const pm_state *st, const pm_sinks *sk, con
         }
         keys = c->bin_mem; perm = keys + np; counts = perm + np;
         int *sums = counts + nkeys;
-        PM_CUDA(c, cudaMemsetAsync(counts, 0, (size_t)nkeys * sizeof(int), c->stream));
+        occ = reinterpret_cast<unsigned char *>(sums + nscan);
+        live = sums + nscan + nocc;
+        PM_CUDA(c, cudaMemsetAsync(counts, 0, (size_t)(nkeys + nscan + nocc + 2) * sizeof(int), c->stream));
         const unsigned blocks = (unsigned)((np + 255) / 256);
         tick(c, PM_K_BIN, 0);
         k_bin_count<<<blocks, 256, 0, c->stream>>>(P, nk ? sk->x : nullptr, nk ? sk->y : nullptr, nk ? sk->z : nullptr, nk,
-                                                   nn ? sn->x : nullptr, nn ? sn->y : nullptr, nn ? sn->z : nullptr, nn, keys, counts);
+                                                   nn ? sn->x : nullptr, nn ? sn->y : nullptr, nn ? sn->z : nullptr, nn, keys, counts, occ);
         if ((rc = check_launch(c, "k_bin_count")) != PM_OK) return rc;
         k_bin_scan_local<<<nscan, 256, 0, c->stream>>>(counts, nkeys, sums);
         if ((rc = check_launch(c, "k_bin_scan_local")) != PM_OK) return rc;
@@ -797,13 +866,19 @@ extern "C" int pm_deposit(pm_ctx *c, const pm_state *st, const pm_sinks *sk, con
         if ((rc = check_launch(c, "k_bin_fill")) != PM_OK) return rc;
         tick(c, PM_K_BIN, 1);
     }
-    {   // a0: reset (L59 "all cells initialized to zero")
-        const long long n2 = (long long)c->nch * P.Nb / 2;
+    // a0: reset (L59 "all cells initialized to zero").  The tiles this step's particles can add into are marked live (from the
+    // bin occupancy) and zeroed; all others are stale and taken as zeros by the readers (pm_tiles.cuh).
+    if (np == 0) PM_CUDA(c, cudaMemsetAsync(c->tile_live, 0, (size_t)c->ntiles, c->stream));
+    if (np > 0) {
+        const Tiles T = tiles_of(c);
         tick(c, PM_K_ZERO, 0);
-        // grid of 16 CTAs per SM (two waves): 1.03 ms against 1.14 ms for 8; cudaMemsetAsync is faster alone (0.92 ms) but the
-        // step as a whole is not (the deposit kernels behind it slow down by the same amount)
-        k_zero_buffer<<<c->sm_count * 16, 256, 0, c->stream>>>(reinterpret_cast<double2 *>(c->buf), n2);
-        if ((rc = check_launch(c, "k_zero_buffer")) != PM_OK) return rc;
+        k_tiles_mark<<<(unsigned)((c->ntiles + 255) / 256), 256, 0, c->stream>>>(P, T, occ, (int)c->ntiles, nk > 0, nn > 0, live);
+        if ((rc = check_launch(c, "k_tiles_mark")) != PM_OK) return rc;
+        const unsigned zblocks = (unsigned)std::min<long long>((c->ntiles + 7) / 8, (long long)c->sm_count * 16);
+        k_tiles_zero<<<zblocks, 256, 0, c->stream>>>(P, c->buf, T, c->repro, (int)c->ntiles, live);
+        if ((rc = check_launch(c, "k_tiles_zero")) != PM_OK) return rc;
+        k_zero_sweep<<<c->sm_count * 16, 256, 0, c->stream>>>(P, c->buf, c->repro, (int)c->ntiles, live);
+        if ((rc = check_launch(c, "k_zero_sweep")) != PM_OK) return rc;
         tick(c, PM_K_ZERO, 1);
     }
     const DevState U = { st->rho, st->mx, st->my, st->mz, st->etot, st->eint };
@@ -832,6 +907,8 @@ extern "C" int pm_deposit(pm_ctx *c, const pm_state *st, const pm_sinks *sk, con
         tick(c, PM_K_SNE, 1);
     }
     c->n_sinks_dep = nk; c->n_sne_dep = nn; c->dt = dt;
+    c->ever_deposited = true;
+    c->grav_in_ch1 = false;
     c->stage = ST_DEPOSITED;
     c->buffer_valid = false;              // unfolded until pm_fold_ghosts
     return PM_OK;
@@ -850,12 +927,13 @@ extern "C" int pm_fold_ghosts(pm_ctx *c) {
     const long long n_edge = n_z + n_y + n_x;
     const unsigned blocks = (unsigned)((n_edge + 255) / 256);
     tick(c, PM_K_FOLD, 0);
+    const Tiles T = tiles_of(c);
     if (c->repro) {
-        if (W == 2) k_fold_ghosts<2, kReproChannels><<<blocks, 256, 0, c->stream>>>(P, c->buf, n_edge, n_z, n_y);
-        else k_fold_ghosts<1, kReproChannels><<<blocks, 256, 0, c->stream>>>(P, c->buf, n_edge, n_z, n_y);
+        if (W == 2) k_fold_ghosts<2, kReproChannels, true><<<blocks, 256, 0, c->stream>>>(P, c->buf, T, n_edge, n_z, n_y);
+        else k_fold_ghosts<1, kReproChannels, true><<<blocks, 256, 0, c->stream>>>(P, c->buf, T, n_edge, n_z, n_y);
     } else {
-        if (W == 2) k_fold_ghosts<2, kBufChannels><<<blocks, 256, 0, c->stream>>>(P, c->buf, n_edge, n_z, n_y);
-        else k_fold_ghosts<1, kBufChannels><<<blocks, 256, 0, c->stream>>>(P, c->buf, n_edge, n_z, n_y);
+        if (W == 2) k_fold_ghosts<2, kBufChannels, true><<<blocks, 256, 0, c->stream>>>(P, c->buf, T, n_edge, n_z, n_y);
+        else k_fold_ghosts<1, kBufChannels, true><<<blocks, 256, 0, c->stream>>>(P, c->buf, T, n_edge, n_z, n_y);
     }
     int rc = check_launch(c, "k_fold_ghosts");
     tick(c, PM_K_FOLD, 1);
@@ -873,7 +951,7 @@ static void launch_apply(pm_ctx *c, const DevState &U) {
     const unsigned blocks = (n_items + kApplyThreads - 1) / kApplyThreads;
     const bool tl = P.tl_num > 0.0;
 #define PM_APPLY(LAM_, TL_, REPRO_, lamptr)                                                                                   \
-    k_apply_limited<VEC, LAM_, TL_, REPRO_><<<blocks, kApplyThreads, 0, c->stream>>>(P, U, c->buf, c->ret, c->ret_tr, lamptr, \
+    k_apply_limited<VEC, LAM_, TL_, REPRO_><<<blocks, kApplyThreads, 0, c->stream>>>(P, U, c->buf, tiles_of(c), c->ret, c->ret_tr, lamptr, \
                                                                                      c->repro_M, n_items, ipr)
     if (c->lam) {
         if (c->repro) { if (tl) PM_APPLY(true, true, true, c->lam); else PM_APPLY(true, false, true, c->lam); }
@@ -951,7 +1029,9 @@ extern "C" int pm_create_sinks(pm_ctx *c, pm_state *st, int64_t max_new, double 
     const DevState U = { st->rho, st->mx, st->my, st->mz, st->etot, st->eint };
     int rc;
     PM_CUDA(c, cudaMemsetAsync(total, 0, (size_t)(1 + nblocks) * sizeof(int), c->stream));
-    k_create_find<<<nblocks, 256, 0, c->stream>>>(P, U, c->buffer_valid ? c->buf : nullptr, flag, bcount);
+    // (iii) needs the folded accretion channel of the last deposit; before the first deposit there is none and the test is skipped
+    if (c->ever_deposited && !c->buffer_valid) PM_FAIL(c, PM_EORDER, "pm_create_sinks: the retained buffer is not folded (call pm_fold_ghosts)");
+    k_create_find<<<nblocks, 256, 0, c->stream>>>(P, U, c->buffer_valid ? c->buf : nullptr, tiles_of(c), flag, bcount);
     if ((rc = check_launch(c, "k_create_find")) != PM_OK) return rc;
     k_bin_scan_local<<<nscan, 256, 0, c->stream>>>(bcount, nblocks, sums);
     if ((rc = check_launch(c, "k_bin_scan_local")) != PM_OK) return rc;
@@ -974,7 +1054,10 @@ extern "C" int pm_create_sinks(pm_ctx *c, pm_state *st, int64_t max_new, double 
 // ---------------------------------------------------------------------------------------------------------------
 // (f)3: PM gravity (L95, L107): Steps 1, 2, 5 with the cloud-in-cell kernel, interpolation + kick, drift
 // ---------------------------------------------------------------------------------------------------------------
-static int fold_channel0(pm_ctx *c) {
+// Gravity works in buffer channel 1 (the first supernova channel): it is free between steps, its reset here is a plain
+// sweep of that one channel, and the tile flags are not involved -- the next pm_deposit rewrites them anyway.  Channel 0
+// (the retained accretion buffer of L108 / L177) and its flags are left alone, so pm_create_sinks still works afterwards.
+static int fold_gravity_channel(pm_ctx *c, double *gbuf) {
     const DevP &P = c->P;
     const long long g2 = 2 * P.g;
     const int W = (P.g % 2 == 0 && P.nx % 2 == 0) ? 2 : 1;
@@ -983,8 +1066,8 @@ static int fold_channel0(pm_ctx *c) {
     const long long n_x = (long long)(P.nz - g2) * (P.ny - g2) * g2 / W;
     const long long n_edge = n_z + n_y + n_x;
     const unsigned blocks = (unsigned)((n_edge + 255) / 256);
-    if (W == 2) k_fold_ghosts<2, 1><<<blocks, 256, 0, c->stream>>>(P, c->buf, n_edge, n_z, n_y);
-    else k_fold_ghosts<1, 1><<<blocks, 256, 0, c->stream>>>(P, c->buf, n_edge, n_z, n_y);
+    if (W == 2) k_fold_ghosts<2, 1, false><<<blocks, 256, 0, c->stream>>>(P, gbuf, tiles_of(c), n_edge, n_z, n_y);
+    else k_fold_ghosts<1, 1, false><<<blocks, 256, 0, c->stream>>>(P, gbuf, tiles_of(c), n_edge, n_z, n_y);
     return check_launch(c, "k_fold_ghosts<1 channel>");
 }
 
@@ -1000,21 +1083,21 @@ static int grav_order(pm_ctx *c, const double *x, const double *y, const double 
     const DevP &P = c->P;
     const int nkeys = 2 * P.ntile + 1;
     const int nscan = (nkeys + kScanChunk - 1) / kScanChunk;
-    if (c->gperm_valid && c->gperm_x == x && c->gperm_n == n) { *perm_out = c->bin_mem + n; return PM_OK; }
+    if (c->gperm_valid && c->gperm_x == x && c->gperm_n == n) { *perm_out = c->grav_mem + n; return PM_OK; }
     c->gperm_valid = false;
     const long long need = 2 * n + nkeys + nscan;
-    if (need > c->bin_cap) {
-        if (c->bin_mem) { PM_CUDA(c, cudaFree(c->bin_mem)); c->bin_mem = nullptr; c->bin_cap = 0; }
+    if (need > c->grav_cap) {
+        if (c->grav_mem) { PM_CUDA(c, cudaFree(c->grav_mem)); c->grav_mem = nullptr; c->grav_cap = 0; }
         const long long cap = need + need / 4;
-        cudaError_t e = cudaMalloc(&c->bin_mem, (size_t)cap * sizeof(int));
-        if (e != cudaSuccess) { c->bin_mem = nullptr; PM_FAIL(c, PM_ENOMEM, "cudaMalloc of bins failed: %s", cudaGetErrorString(e)); }
-        c->bin_cap = cap;
+        cudaError_t e = cudaMalloc(&c->grav_mem, (size_t)cap * sizeof(int));
+        if (e != cudaSuccess) { c->grav_mem = nullptr; PM_FAIL(c, PM_ENOMEM, "cudaMalloc of bins failed: %s", cudaGetErrorString(e)); }
+        c->grav_cap = cap;
     }
-    int *keys = c->bin_mem, *perm = keys + n, *counts = perm + n, *sums = counts + nkeys;
+    int *keys = c->grav_mem, *perm = keys + n, *counts = perm + n, *sums = counts + nkeys;
     int rc;
     PM_CUDA(c, cudaMemsetAsync(counts, 0, (size_t)nkeys * sizeof(int), c->stream));
     const unsigned blocks = (unsigned)((n + 255) / 256);
-    k_bin_count<<<blocks, 256, 0, c->stream>>>(P, x, y, z, n, nullptr, nullptr, nullptr, 0, keys, counts);
+    k_bin_count<<<blocks, 256, 0, c->stream>>>(P, x, y, z, n, nullptr, nullptr, nullptr, 0, keys, counts, nullptr);
     if ((rc = check_launch(c, "k_bin_count")) != PM_OK) return rc;
     k_bin_scan_local<<<nscan, 256, 0, c->stream>>>(counts, nkeys, sums);
     if ((rc = check_launch(c, "k_bin_scan_local")) != PM_OK) return rc;
@@ -1036,24 +1119,24 @@ extern "C" int pm_gravity_deposit(pm_ctx *c, const double *rho_gas, int64_t n, c
         PM_FAIL(c, PM_EORDER, "pm_gravity_deposit: the buffer mesh is in use (finish the exchange step first)");
     PM_CUDA(c, cudaSetDevice(c->device));
     const DevP &P = c->P;
-    c->buffer_valid = false;      // channel 0 no longer holds the accretion rates of the last exchange step
-    c->stage = ST_IDLE;
+    double *const gbuf = c->buf + P.Nb;      // channel 1; see fold_gravity_channel
+    c->grav_in_ch1 = true;
     int rc;
-    PM_CUDA(c, cudaMemsetAsync(c->buf, 0, (size_t)P.Nb * sizeof(double), c->stream));     // Step 1: "initialized to zero" (L59)
+    PM_CUDA(c, cudaMemsetAsync(gbuf, 0, (size_t)P.Nb * sizeof(double), c->stream));     // Step 1: "initialized to zero" (L59)
     if (n > 0) {
         const int *perm;
         if ((rc = grav_order(c, x, y, z, n, &perm)) != PM_OK) return rc;
-        k_grav_deposit<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(P, x, y, z, m, n, perm, c->buf, c->err_flag);
+        k_grav_deposit<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(P, x, y, z, m, n, perm, gbuf, c->err_flag);
         if ((rc = check_launch(c, "k_grav_deposit")) != PM_OK) return rc;
     }
-    if ((rc = fold_channel0(c)) != PM_OK) return rc;                                       // Step 2
+    if ((rc = fold_gravity_channel(c, gbuf)) != PM_OK) return rc;                           // Step 2
     const bool vec = P.nx % 2 == 0 && aligned16(rho_tot) && (!rho_gas || aligned16(rho_gas));
     const long long work = vec ? P.N / 2 : P.N;
     long long blocks = (work + 255) / 256;
     const long long cap = (long long)c->sm_count * 32;
     if (blocks > cap) blocks = cap;
-    if (vec) k_grav_apply<2><<<(unsigned)blocks, 256, 0, c->stream>>>(P, rho_gas, c->buf, rho_tot);   // Step 5
-    else k_grav_apply<1><<<(unsigned)blocks, 256, 0, c->stream>>>(P, rho_gas, c->buf, rho_tot);
+    if (vec) k_grav_apply<2><<<(unsigned)blocks, 256, 0, c->stream>>>(P, rho_gas, gbuf, rho_tot);   // Step 5
+    else k_grav_apply<1><<<(unsigned)blocks, 256, 0, c->stream>>>(P, rho_gas, gbuf, rho_tot);
     return check_launch(c, "k_grav_apply");
 }
 
@@ -1163,8 +1246,18 @@ extern "C" int pm_step_host(pm_ctx *c, pm_state *hs, pm_sinks *hk, const pm_sne 
 }
 
 // ---- test-only views ---------------------------------------------------------------------------------------------
+static int materialize_tiles(pm_ctx *c) {
+    PM_CUDA(c, cudaSetDevice(c->device));
+    k_tiles_materialize<<<(unsigned)((c->ntiles + 3) / 4), 128, 0, c->stream>>>(c->P, c->buf, tiles_of(c), c->repro, c->grav_in_ch1, (int)c->ntiles);
+    return check_launch(c, "k_tiles_materialize");
+}
+
 extern "C" int pm_debug_buffer(pm_ctx *c, int channel, const double **dev_ptr, int64_t dims[3], int64_t *origin, int32_t *ghost) {
     if (!c || !dev_ptr || channel < 0 || channel >= kBufChannels) return PM_EINVAL;
+    {   // the raw mesh is only readable once the zeros that stale tiles stand for have been stored (test-only, not timed)
+        int rc = materialize_tiles(c);
+        if (rc != PM_OK) return rc;
+    }
     *dev_ptr = c->buf + (long long)channel * c->P.Nb;
     if (dims) { dims[0] = c->P.nz + 2 * c->P.g; dims[1] = c->P.ny + 2 * c->P.g; dims[2] = c->P.pj; }
     if (origin) *origin = (long long)c->P.g * c->P.pk + (long long)c->P.g * c->P.pj + c->P.gx;
@@ -1182,7 +1275,8 @@ extern "C" int pm_debug_round_buffers(pm_ctx *c) {
     if (!c) return PM_EINVAL;
     if (!c->repro) PM_FAIL(c, PM_EINVAL, "pm_debug_round_buffers needs PM_FLAG_REPRODUCIBLE");
     if (!c->buffer_valid) PM_FAIL(c, PM_EORDER, "pm_debug_round_buffers: fold first");
-    PM_CUDA(c, cudaSetDevice(c->device));
+    int rc0 = materialize_tiles(c);
+    if (rc0 != PM_OK) return rc0;
     const DevP &P = c->P;
     if (P.nx % 2 == 0) k_repro_round<2><<<(unsigned)((P.N / 2 + 255) / 256), 256, 0, c->stream>>>(P, c->buf, c->repro_M, P.N / 2);
     else k_repro_round<1><<<(unsigned)((P.N + 255) / 256), 256, 0, c->stream>>>(P, c->buf, c->repro_M, P.N);

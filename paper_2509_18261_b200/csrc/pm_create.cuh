@@ -5,6 +5,7 @@
 // and lowers the cells.  Nothing but the final count goes to the host.
 #pragma once
 #include "pm_device.cuh"
+#include "pm_tiles.cuh"
 
 namespace pm {
 
@@ -18,7 +19,7 @@ __device__ __forceinline__ double truelove_rho(const DevP &P, double rho, double
 // One thread per cell for tests (i) and (iii); the few cells that pass are then handled by the whole warp, one after the
 // other: the 32 lanes split the (2g+1)^3 neighbour offsets and leave at the first neighbour that is not smaller -- a lone
 // lane walking its 257 neighbours would hold the other 31 idle (a third of the time of the first version).
-__global__ void __launch_bounds__(256) k_create_find(const DevP P, const DevState U, const double *__restrict__ buf0,
+__global__ void __launch_bounds__(256) k_create_find(const DevP P, const DevState U, const double *__restrict__ buf0, const Tiles T,
                                                      unsigned char *__restrict__ flag, int *__restrict__ block_count) {
     const long long c_raw = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     const int lane = threadIdx.x & 31;
@@ -29,7 +30,8 @@ __global__ void __launch_bounds__(256) k_create_find(const DevP P, const DevStat
     const long long row = c / P.nx;
     const int j = (int)(row % P.ny), k = (int)(row / P.ny);
     bool cand = valid && rho > truelove_rho(P, rho, U.eint[c]);                       // (i)   above rho_Tr
-    if (cand && buf0 && buf0[ghost_index(P, i, j, k)] != 0.0) cand = false;            // (iii) inside another sink's kernel (L177)
+    // (iii) inside another sink's kernel (L177); a tile no sink touched in the last step is stale and stands for zeros
+    if (cand && buf0 && (T.live[tile_index(P, i, j, k)] & kLiveK) && buf0[ghost_index(P, i, j, k)] != 0.0) cand = false;
     unsigned todo = __ballot_sync(0xffffffffu, cand);
     bool created = false;
     const int g = P.gs, B = 2 * g + 1, nb = B * B * B;

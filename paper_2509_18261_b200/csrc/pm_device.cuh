@@ -40,6 +40,8 @@ struct DevP {
     double nsub3;
     int nsbx, nsby, nsbz;   // super-blocks (4x4x4 tiles of 8^3 cells) per axis: the bins particles are ordered by
     int ntile;              // bin keys per particle kind: super-blocks x tiles per super-block
+    int ntx, nty, ntz;      // buffer-mesh tiles of 8^3 cells per axis, ghost tiles included (pm_tiles.cuh): tile t holds the
+                            // cells [8 (t - 1), 8 t) of owned coordinates
 };
 
 struct DevState { double *rho, *mx, *my, *mz, *etot, *eint; };

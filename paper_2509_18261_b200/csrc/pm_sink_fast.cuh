@@ -8,6 +8,7 @@
 // sum rho (v - v_s) = sum (m - rho v_s), rho c_s = sqrt(gamma (gamma - 1) e_int rho), a = w * [mdot dt / (V sum w)].
 #pragma once
 #include "pm_device.cuh"
+#include "pm_tiles.cuh"
 
 namespace pm {
 
@@ -155,8 +156,8 @@ __global__ void __launch_bounds__(kFastSinkWarps * 32, kFastSinkMinBlocks) k_dep
             amt = fmax(amt, truelove_excess(P, U.rho[q], U.eint[q]));
             ret_tr[q] = -CUDART_INF;                    // invalidate last step's entry; the apply pass rewrites it where mass is removed
         }
-        atomicAdd(dst, -amt);                           // R1: signed
-        if (REPRO) atomicAdd(dst + kChK * P.Nb, kSinkUnit);   // Appendix A: contribution count (same-sign terms: T = |sum|)
+        red_add(dst, -amt);                           // R1: signed
+        if (REPRO) red_add(dst + kChK * P.Nb, kSinkUnit);   // Appendix A: contribution count (same-sign terms: T = |sum|)
     }
     if (lane == 0) {
         scal[s] = sc.mdot; scal[S.n + s] = sc.r_acc; scal[2 * S.n + s] = wsum;
@@ -206,9 +207,11 @@ __global__ void __launch_bounds__(kFastSinkWarps * 32, kFastSinkMinBlocks) k_ret
     dm = warp_sum(dm); dpx = warp_sum(dpx); dpy = warp_sum(dpy); dpz = warp_sum(dpz);
     if (lane == 0) {
         const double m_old = S.m[s], m_new = m_old + dm;
-        S.vx[s] = (m_old * S.vx[s] + dpx) / m_new;
-        S.vy[s] = (m_old * S.vy[s] + dpy) / m_new;
-        S.vz[s] = (m_old * S.vz[s] + dpz) / m_new;
+        if (m_new != 0.0) {                       // R43: a massless sink that gained nothing keeps its velocity (no 0/0)
+            S.vx[s] = (m_old * S.vx[s] + dpx) / m_new;
+            S.vy[s] = (m_old * S.vy[s] + dpy) / m_new;
+            S.vz[s] = (m_old * S.vz[s] + dpz) / m_new;
+        }
         S.m[s] = m_new;
         if (S.dm) S.dm[s] = dm;
         if (S.dpx) S.dpx[s] = dpx;

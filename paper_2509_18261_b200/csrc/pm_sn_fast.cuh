@@ -12,6 +12,7 @@
 // kernel and a gather/scatter kernel was measured slower.
 #pragma once
 #include "pm_device.cuh"
+#include "pm_tiles.cuh"
 
 namespace pm {
 
@@ -257,15 +258,15 @@ __device__ __forceinline__ void sn_deposit_one(const DevP &P, const DevState &U,
         const double dpy = fma(omega, fma(rho, sc.vcy, -my), fma(drho, sc.vcy, pry));
         const double dpz = fma(omega, fma(rho, sc.vcz, -mz), fma(drho, sc.vcz, prz));
         const double de = fma(omega, k_e, fma(sc.vcx, prx, fma(sc.vcy, pry, sc.vcz * prz)));
-        atomicAdd(dst, drho);
-        atomicAdd(dst + P.Nb, dpx);
-        atomicAdd(dst + 2 * P.Nb, dpy);
-        atomicAdd(dst + 3 * P.Nb, dpz);
-        atomicAdd(dst + 4 * P.Nb, de);
+        red_add(dst, drho);
+        red_add(dst + P.Nb, dpx);
+        red_add(dst + 2 * P.Nb, dpy);
+        red_add(dst + 3 * P.Nb, dpz);
+        red_add(dst + 4 * P.Nb, de);
         if (REPRO) {                                 // Appendix A: error scales and the contribution count (dst is channel 1)
-            atomicAdd(dst + (kChTp - 1) * P.Nb, (fabs(dpx) + fabs(dpy)) + fabs(dpz));
-            atomicAdd(dst + (kChTe - 1) * P.Nb, fabs(de));
-            atomicAdd(dst + (kChK - 1) * P.Nb, 1.0);
+            red_add(dst + (kChTp - 1) * P.Nb, (fabs(dpx) + fabs(dpy)) + fabs(dpz));
+            red_add(dst + (kChTe - 1) * P.Nb, fabs(de));
+            red_add(dst + (kChK - 1) * P.Nb, 1.0);
         }
     }
     if (dbg && lane == 0) {

@@ -7,6 +7,7 @@ not built, importing/using this module raises.
 from __future__ import annotations
 
 import ctypes as C
+import glob
 import os
 import subprocess
 
@@ -15,8 +16,7 @@ import torch
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libpm_b200.so")
 SRC = [os.path.join(_HERE, "csrc", "pm_b200.cu")]
-HDRS = [os.path.join(_HERE, "csrc", "pm_device.cuh"), os.path.join(_HERE, "csrc", "pm_create.cuh"), os.path.join(_HERE, "csrc", "pm_fast.cuh"),
-        os.path.join(_HERE, "csrc", "pm_sn_fast.cuh"), os.path.join(_HERE, "csrc", "pm_sink_fast.cuh"), os.path.join(os.path.dirname(_HERE), "include", "pm.h")]
+HDRS = sorted(glob.glob(os.path.join(_HERE, "csrc", "*.cuh"))) + [os.path.join(os.path.dirname(_HERE), "include", "pm.h")]
 
 PM_OK, PM_EINVAL, PM_ENOMEM, PM_ECUDA, PM_EORDER, PM_EDOMAIN = 0, -1, -2, -3, -4, -5
 PM_FLAG_DEBUG_SCALARS, PM_FLAG_DEBUG_LAMBDA, PM_FLAG_GENERIC_KERNELS, PM_FLAG_TIMING, PM_FLAG_REPRODUCIBLE = 1, 2, 4, 8, 16
@@ -137,10 +137,13 @@ def make_params(p: dict, flags: int = 0) -> PmParams:
     return o
 
 
-def _ptr(t):
+def _ptr(t, n=None):
+    """Device pointer of a contiguous fp64 CUDA tensor of n elements (None -> NULL): the kernels get a raw pointer, so a CPU
+    tensor or a short array must be refused here."""
     if t is None:
         return None
-    assert t.dtype == torch.float64 and t.is_contiguous(), "fp64 contiguous tensors only"
+    assert t.is_cuda and t.dtype == torch.float64 and t.is_contiguous(), "fp64 contiguous CUDA tensors only"
+    assert n is None or t.numel() == n, f"array of {t.numel()} elements where {n} are expected"
     return t.data_ptr()
 
 
@@ -175,10 +178,12 @@ class DeviceState:
     def fields(self):
         return [getattr(self, f) for f in self.FIELDS]
 
-    def c(self) -> PmState:
+    def c(self, n_cells=None) -> PmState:
         s = PmState()
+        dev = {getattr(self, f).device for f in self.FIELDS}
+        assert len(dev) == 1, "state fields live on different devices"
         for f in self.FIELDS:
-            setattr(s, f, _ptr(getattr(self, f)))
+            setattr(s, f, _ptr(getattr(self, f), n_cells))
         return s
 
 
@@ -203,7 +208,7 @@ class DeviceSinks:
         s = PmSinks()
         s.n = self.n
         for f in self.IN + self.OUT:
-            setattr(s, f, _ptr(getattr(self, f)))
+            setattr(s, f, _ptr(getattr(self, f), self.n))
         return s
 
 
@@ -223,7 +228,7 @@ class DeviceSNe:
         s = PmSNe()
         s.n = self.n
         for f in self.IN:
-            setattr(s, f, _ptr(getattr(self, f)))
+            setattr(s, f, _ptr(getattr(self, f), self.n))
         return s
 
 
@@ -235,6 +240,7 @@ class Context:
         self.device = torch.device(device)
         self.params = dict(params)
         idx = self.device.index if self.device.index is not None else 0
+        self.device = torch.device(self.device.type, idx)          # with an explicit index, so that tensor.device compares equal
         if stream is None:
             stream = torch.cuda.current_stream(self.device)
         self.stream = stream
@@ -249,8 +255,20 @@ class Context:
         if rc != PM_OK:
             raise PmError(rc, where, self.L.pm_last_error(self.h).decode())
 
+    def _cells(self):
+        return self.params["nx"] * self.params["ny"] * self.params["nz"]
+
+    def _on_device(self, *objs):
+        for o in objs:
+            if o is None:
+                continue
+            for f in getattr(o, "FIELDS", None) or (o.IN + getattr(o, "OUT", ())):
+                t = getattr(o, f, None)
+                assert t is None or t.device == self.device, f"{f} lives on {t.device}, the ctx on {self.device}"
+
     def pm_deposit(self, state: DeviceState, sinks, sne, dt: float):
-        cs = state.c()
+        self._on_device(state, sinks, sne)
+        cs = state.c(self._cells())
         ck = sinks.c() if sinks is not None else None
         cn = sne.c() if sne is not None else None
         self._chk(self.L.pm_deposit(self.h, C.byref(cs), C.byref(ck) if ck else None, C.byref(cn) if cn else None, dt),
@@ -260,10 +278,12 @@ class Context:
         self._chk(self.L.pm_fold_ghosts(self.h), "pm_fold_ghosts")
 
     def pm_apply_limited(self, state: DeviceState):
-        cs = state.c()
+        self._on_device(state)
+        cs = state.c(self._cells())
         self._chk(self.L.pm_apply_limited(self.h, C.byref(cs)), "pm_apply_limited")
 
     def pm_return_to_particles(self, sinks):
+        self._on_device(sinks)
         ck = sinks.c() if sinks is not None else None
         self._chk(self.L.pm_return_to_particles(self.h, C.byref(ck) if ck else None), "pm_return_to_particles")
 
@@ -306,7 +326,8 @@ class Context:
         """Sec. 3.1.2.  Returns (n_found, dict of device tensors x, y, z, vx, vy, vz, m of length min(n_found, max_new))."""
         out = {k: torch.zeros(max(max_new, 1), dtype=torch.float64, device=self.device) for k in ("x", "y", "z", "vx", "vy", "vz", "m")}
         n = C.c_int64(0)
-        cs = state.c()
+        self._on_device(state)
+        cs = state.c(self._cells())
         self._chk(self.L.pm_create_sinks(self.h, C.byref(cs), int(max_new), *(out[k].data_ptr() for k in ("x", "y", "z", "vx", "vy", "vz", "m")),
                                          C.byref(n)), "pm_create_sinks")
         k = n.value if n.value <= max_new else 0

@@ -15,3 +15,18 @@ def pytest_configure(config):
 @pytest.fixture(scope="session")
 def golden_dir():
     return os.path.join(ROOT, "tests", "golden")
+
+
+@pytest.fixture(autouse=True)
+def _parity_context(request):
+    """Names the running test in the parity helpers' margin / failure records and flushes the margins afterwards."""
+    try:
+        from tests import parity
+    except Exception:            # CPU-only collection without torch.cuda is fine: parity is only used by gpu tests
+        yield
+        return
+    parity.CONTEXT["test"] = request.node.name
+    parity.MARGINS.clear()
+    yield
+    if parity.MARGINS:
+        parity.dump_margins()

@@ -11,7 +11,9 @@ compare element by element.  Tolerances (BASELINE.json north_star; DESIGN.md "To
 """
 from __future__ import annotations
 
+import json
 import math
+import os
 
 import numpy as np
 import torch
@@ -25,14 +27,51 @@ REORDER = 1e-14
 TOTALS_REL = 1e-13
 
 
+# Every comparison records how much of its bound it used (max over elements of err / tol), and every failure is also appended
+# to a file: the log tail of a GPU run may lose the assertion message, the file does not.  MARGINS feeds the table in DESIGN.md
+# section 5; the files land in gpurun_out/ (the one folder that comes back from the GPU box).
+LOG_DIR = os.environ.get("PM_PARITY_LOG_DIR", os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "gpurun_out"))
+MARGINS: dict = {}
+CONTEXT = {"test": ""}
+
+
+def _record(what: str, err: np.ndarray, tol: np.ndarray):
+    ratio = float(np.max(err / np.maximum(tol, 1e-320))) if err.size else 0.0
+    key = (CONTEXT["test"], what.split(" (")[0])
+    MARGINS[key] = max(MARGINS.get(key, 0.0), ratio)
+    return ratio
+
+
+def dump_margins():
+    """Append this process's margins (used fraction of each bound) to gpurun_out/parity_margins.jsonl."""
+    try:
+        os.makedirs(LOG_DIR, exist_ok=True)
+        with open(os.path.join(LOG_DIR, "parity_margins.jsonl"), "a") as f:
+            for (test, what), r in sorted(MARGINS.items()):
+                f.write(json.dumps({"test": test, "quantity": what, "used_fraction_of_bound": r}) + "\n")
+    except OSError:
+        pass
+
+
+def _fail(msg: str):
+    try:
+        os.makedirs(LOG_DIR, exist_ok=True)
+        with open(os.path.join(LOG_DIR, "parity_failures.log"), "a") as f:
+            f.write(f"[{CONTEXT['test']}] {msg}\n")
+    except OSError:
+        pass
+    raise AssertionError(msg)
+
+
 def close_strict(gpu: np.ndarray, ref: np.ndarray, what: str, rel: float = REL):
     err = np.abs(gpu - ref)
     tol = rel * np.abs(ref) + ABS_FLOOR
+    _record(what, err, tol)
     bad = err > tol
     if bad.any():
-        w = np.argmax(err / np.maximum(tol, 1e-320))
-        raise AssertionError(f"{what}: {bad.sum()} of {bad.size} outside {rel:g} rel; worst at flat index {w}: "
-                             f"gpu={gpu.reshape(-1)[w]!r} ref={ref.reshape(-1)[w]!r}")
+        w = int(np.argmax(err / np.maximum(tol, 1e-320)))
+        _fail(f"{what}: {bad.sum()} of {bad.size} outside {rel:g} rel; worst at flat index {w}: "
+              f"gpu={gpu.reshape(-1)[w]!r} ref={ref.reshape(-1)[w]!r} err={err.reshape(-1)[w]:.3e} bound={tol.reshape(-1)[w]:.3e}")
 
 
 def close_reorder(gpu: np.ndarray, ref: np.ndarray, scale: np.ndarray, what: str, rel: float = REL):
@@ -40,11 +79,13 @@ def close_reorder(gpu: np.ndarray, ref: np.ndarray, scale: np.ndarray, what: str
     err = np.abs(gpu - ref)
     tol1 = rel * np.abs(ref) + ABS_FLOOR
     tol = tol1 + REORDER * scale
+    _record(what, err, tol)
     bad = err > tol
     if bad.any():
-        w = np.argmax(err - tol)
-        raise AssertionError(f"{what}: {bad.sum()} of {bad.size} outside tolerance; worst at flat index {w}: "
-                             f"gpu={gpu.reshape(-1)[w]!r} ref={ref.reshape(-1)[w]!r} scale={scale.reshape(-1)[w]!r}")
+        w = int(np.argmax(err / np.maximum(tol, 1e-320)))
+        _fail(f"{what}: {bad.sum()} of {bad.size} outside tolerance; worst at flat index {w}: "
+              f"gpu={gpu.reshape(-1)[w]!r} ref={ref.reshape(-1)[w]!r} err={err.reshape(-1)[w]:.3e} "
+              f"bound={tol.reshape(-1)[w]:.3e} (rel part {tol1.reshape(-1)[w]:.3e}, scale={np.broadcast_to(scale, err.shape).reshape(-1)[w]!r})")
     return int((err > tol1).sum())
 
 

@@ -28,7 +28,7 @@ def run_deposit(w, with_gas=True):
 def check_deposit(w, with_gas=True):
     ctx, out = run_deposit(w, with_gas)
     p = w.params
-    ghosted, owned, g, ox = ctx.debug_buffer(0)
+    ghosted, owned, g, ox = ctx.debug_buffer(1)
     # Step 1 alone: the ghost cells keep what was deposited into them (the fold leaves them in place)
     ref_buf = go.gravity_deposit_buffer(p, w.x, w.y, w.z, w.m, g=g)
     gb = ghosted[:, :, ox - g:ox - g + p["nx"] + 2 * g].cpu().numpy()

@@ -343,7 +343,7 @@ def test_step_host_matches_device_path():
         assert np.allclose(a, b, rtol=1e-10, atol=1e-10 * np.abs(a).max())
     assert np.allclose(g.sinks.m.cpu().numpy(), hk.m, rtol=1e-12)
     assert np.allclose(g.sinks.dm.cpu().numpy(), hk.dm, rtol=1e-12)
-    assert ctx.pm_launch_count() == 10
+    assert ctx.pm_launch_count() == 12      # 4 binning, 3 reset (stamp, tile-wise zero, sweep), 2 deposits, fold, apply, return
 
 
 def test_kernel_times_and_red_probe():
