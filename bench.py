@@ -99,9 +99,9 @@ def measured_peak():
 
 def ncu_traffic(kernel: str):
     """DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) from the committed ncu --set full capture,
-    profiles/r01_ncu_traffic.csv (made by the command in profiles/r01_ncu_full.md); None if not recorded."""
+    profiles/r02_ncu_traffic.csv (made by the command in profiles/r02_ncu_full.md); None if not recorded."""
     try:
-        with open(os.path.join(ROOT, "profiles", "r01_ncu_traffic.csv")) as f:
+        with open(os.path.join(ROOT, "profiles", "r02_ncu_traffic.csv")) as f:
             for ln in f.read().splitlines()[1:]:
                 k, v = ln.split(",")
                 if k == kernel:
@@ -113,32 +113,39 @@ def ncu_traffic(kernel: str):
 
 # ---------------------------------------------------------------------------------------------
 def time_oracle(n: int, steps: int):
-    """The oracle, as it stands, single-threaded, on a config-5-shaped n^3 block with the same particles per cell."""
+    """The oracle, as it stands, single-threaded: on config 5 itself (n = 512) or on a config-5-shaped n^3 block with the same
+    particles per cell (the bounded sample of the default run)."""
     from oracle import pm_oracle as po
     from paper_2509_18261_b200 import inputs
     npart = int(round(1_000_000 * (n / 512.0) ** 3))
-    w = inputs.scaled_mixed(n, npart, seed_index=5)
+    w = inputs.make(5) if n == 512 else inputs.scaled_mixed(n, npart, seed_index=5)
     o = po.Oracle(w.params, w.state, w.sinks, w.sne, keep_abs=False)
     t0 = time.perf_counter()
     for _ in range(steps):
         o.step(w.dt)
     dt = (time.perf_counter() - t0) / steps
+    what = "config 5 itself (512^3, 10^6 particles)" if n == 512 else f"config-5-shaped {n}^3 block, {npart} particles (same particles per cell)"
     return {"value": n ** 3 / dt / 1e6, "unit": UNIT, "cores": 1, "kind": "oracle",
-            "sample": f"config-5-shaped {n}^3 block, {npart} particles (same particles per cell), {steps} step(s), "
-                      f"{dt:.2f} s per step, particles/s = {npart / dt:.3e}",
-            "seconds_per_step": dt, "particles_per_s": npart / dt}
+            "sample": f"{what}, {steps} step(s), {dt:.2f} s per step, particles/s = {npart / dt:.3e}; single thread "
+                      f"of {os.cpu_count()} host cores (the oracle is a plain sequential program)",
+            "seconds_per_step": dt, "particles_per_s": npart / dt, "steps": steps, "host_cores": os.cpu_count(),
+            "workload": "config5_large_512" if n == 512 else f"config5_shape_{n}_{npart} (bounded sample of config5_large_512)"}
 
 
 def run_reference(args, rank, world):
+    """--impl reference: the oracle as it stands on the host cores.  Every step is a bounded sample of the workload (a
+    config-5-shaped 256^3 block, ~11 s per step) unless --cpu-baseline-full asks for config 5 itself (~90 s per step); the
+    line reports the steps it really ran."""
     if rank != 0:
         return
+    n = 512 if args.cpu_baseline_full else ORACLE_SAMPLE_N
     steps = max(1, min(args.steps, 2))
-    r = time_oracle(ORACLE_SAMPLE_N, steps)
+    r = time_oracle(n, steps)
     line = {"impl": "reference", "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": args.gpus,
-            "steps": args.steps, "warmup": args.warmup, "ms_per_step": r["seconds_per_step"] * 1e3,
+            "steps": steps, "steps_requested": args.steps, "warmup": 0, "ms_per_step": r["seconds_per_step"] * 1e3,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": "config5_large_512 (oracle timed on a bounded sample)", "sample": r["sample"]},
-            "cpu_baseline": {k: r[k] for k in ("value", "unit", "cores", "kind", "sample")},
+            "config": {"workload": r["workload"], "sample": r["sample"]},
+            "cpu_baseline": {k: r[k] for k in ("value", "unit", "cores", "kind", "sample", "host_cores")},
             "e2e": {"value": r["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line), flush=True)
@@ -161,18 +168,153 @@ def whole_job_value(cells_per_rank: int, steps: int, world: int, total_ms: float
     return world * cells_per_rank * steps / (total_ms * 1e-3) / 1e6
 
 
-def algorithmic_bytes(N, Nb, nk, nn, t4, ts4, tn4, nch=6):
-    """Bytes each kernel group must move per step (SURVEY.md 8(d) per-cell figures times
-    the fraction of 32-byte sectors (4 cells) that hold a touched cell -- the smallest unit HBM moves)."""
+def algorithmic_bytes(N, Nb, nk, nn, t, ts, tn, fk=1.0, fn=1.0, nch=6):
+    """Bytes each kernel group must move per step: SURVEY.md 8(d)'s per-cell figures, each touched CELL counted once.
+    t, ts, tn = fraction of the owned cells touched by any particle / by a sink / by a supernova; fk, fn = fraction of the
+    buffer-mesh tiles that are live in channel group K (accretion) / N (supernovae) -- stale tiles are neither reset nor
+    read (pm_tiles.cuh); with every tile live and every cell touched the figures are 8(d)'s dense ones.
+    8(d) books "buffer reset + deposit write-back (accumulate in cache, write once)" as ONE row, 8 C_b N_b: it is the
+    `zero` entry here (the reset kernels write the live tiles once); the deposit kernels are left with their gather reads
+    and the particle records, as in 8(d).  Call it with sector (4-cell) fractions for the bytes DRAM moves at its smallest
+    granularity (reported as sector_bytes)."""
+    ck, cn = (2, 8) if nch > 6 else (1, 5)                            # Appendix A mode: + count channel, + two error scales
+    buf_live = ck * fk + cn * fn                                       # live buffer words per buffer cell
     return {
         "bin": 8.0 * 3 * (nk + nn) + 4.0 * 3 * (nk + nn),            # positions read, keys + perm written and read
-        "zero": 8.0 * nch * Nb,                                      # store only (9 channels in Appendix A mode)
-        "sinks": 8.0 * 5 * ts4 * N + 8.0 * (1 + (nch > 6)) * ts4 * N + 8.0 * 10 * nk,   # gather 5 fields, write back 1 (2) channels once
-        "sne": 8.0 * 4 * tn4 * N + 8.0 * (5 + 3 * (nch > 6)) * tn4 * N + 8.0 * 8 * nn,  # gather 4 fields, write back 5 (8) channels once
-        "fold": 3 * 8.0 * nch * (Nb - N),   # read ghosts, RMW owned images 
-        "apply": N * (8.0 * nch + 96.0 * t4 + 32.0 * ts4),                # 6 (9) buffer words; 6 + 6 state words and 4 return words where touched
-        "return": 8.0 * 4 * ts4 * N + 8.0 * 12 * nk,
+        "zero": 8.0 * buf_live * Nb,                                   # a0 + the write-back of a3/a5: each live buffer word written once
+        "sinks": 8.0 * 5 * ts * N + 8.0 * 10 * nk,                    # a2: gather 5 fields; particle records
+        "sne": 8.0 * 4 * tn * N + 8.0 * 8 * nn,                       # a4: gather 4 fields; particle records
+        "fold": 3 * 8.0 * buf_live * (Nb - N),                         # read ghosts, read-modify-write their owned images
+        "apply": N * (8.0 * buf_live + 96.0 * t + 32.0 * ts),          # live buffer words; 6 + 6 state words and 4 return words where touched
+        "return": 8.0 * 4 * ts * N + 8.0 * 12 * nk,
     }
+
+
+def run_sharded(args, rank, world, local_rank):
+    """--sharded: the z-slab decomposition of SURVEY.md 8(f)4.  Rank r holds the planes [n r, n (r + 1)) of a periodic
+    n x n x (n world) domain with its own config-5-shaped particle set (weak scaling); a step is the state halo exchange,
+    pm_deposit, pm_slab_pack, the exchange of the buffer's z ghost planes (Eq. 3), pm_fold_ghosts, pm_apply_limited, the
+    owner -> ghost copy of the return mesh (R16) and pm_return_to_particles.  With one rank the exchanges are copies onto the
+    rank itself and the result is the periodic single-domain step.  Same timing rules as the default arm."""
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    from paper_2509_18261_b200 import inputs, pm, sharded
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the CUDA path has no CPU fallback")
+    dev = torch.device(f"cuda:{local_rank}")
+    torch.cuda.set_device(dev)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    n = args.n
+    w = inputs.scaled_mixed(n, args.particles, seed_index=5 + rank)
+    params = dict(w.params, z_slab=1)
+    N, npart = n ** 3, w.sinks.n + w.sne.n
+    sk = pm.DeviceSinks.from_host(w.sinks, dev) if w.sinks.n else None
+    sn = pm.DeviceSNe.from_host(w.sne, dev) if w.sne.n else None
+
+    def make_ctx(flags):
+        c = pm.Context(params, device=str(dev), flags=flags)
+        return c, sharded.SlabStep(c, rank, world)
+
+    ctx, stepper = make_ctx(0)
+    g = ctx.ghost_width()
+    st = pm.DeviceState(*(torch.zeros((n + 2 * g) * n * n, dtype=torch.float64, device=dev) for _ in range(6)))
+    for dst, src in zip(st.fields(), w.state.fields()):
+        dst.view(n + 2 * g, n, n)[g:g + n].copy_(torch.from_numpy(src))
+    d = stepper.d
+    xbytes = 2 * (d["buf_send_lo"].numel() + (d["ret_send_lo"].numel() if d["ret_send_lo"] is not None else 0)) * 8 + 6 * 2 * g * n * n * 8
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    warm = max(args.warmup, 3)
+    for _ in range(warm):
+        stepper.step(st, sk, sn, w.dt)
+    ctx.pm_check()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    launches0 = ctx.pm_launch_count()
+    barrier()
+    ev0.record()
+    for _ in range(args.steps):
+        stepper.step(st, sk, sn, w.dt)
+    ev1.record()
+    barrier()
+    clocks = sampler.stop()
+    ctx.pm_check()
+    launches = ctx.pm_launch_count() - launches0
+    total_ms = reduce_max(ev0.elapsed_time(ev1), world, dev)
+    ctx.close()
+    ctx, stepper = make_ctx(pm.PM_FLAG_TIMING)
+    ks = []
+    for it in range(5):
+        stepper.step(st, sk, sn, w.dt)
+        if it >= 2:
+            ks.append(ctx.pm_kernel_times())
+    kernel_ms = {k: float(np.median([s_[k] for s_ in ks])) for k in pm.KERNEL_GROUPS}
+    # e2e: owned planes and particles from pinned host memory every step, result back to the host
+    hst = [torch.from_numpy(f).pin_memory() for f in w.state.fields()]
+    hsk = {f: torch.from_numpy(getattr(w.sinks, f)).pin_memory() for f in pm.DeviceSinks.IN} if w.sinks.n else None
+    hsn = {f: torch.from_numpy(getattr(w.sne, f)).pin_memory() for f in pm.DeviceSNe.IN} if w.sne.n else None
+    hout = [torch.empty_like(t) for t in hst]
+
+    def e2e_step():
+        for dst, src in zip(st.fields(), hst):
+            dst.view(n + 2 * g, n, n)[g:g + n].copy_(src, non_blocking=True)
+        if hsk:
+            for f in pm.DeviceSinks.IN:
+                getattr(sk, f).copy_(hsk[f], non_blocking=True)
+        if hsn:
+            for f in pm.DeviceSNe.IN:
+                getattr(sn, f).copy_(hsn[f], non_blocking=True)
+        stepper.step(st, sk, sn, w.dt)
+        for dst, src in zip(hout, st.fields()):
+            dst.copy_(src.view(n + 2 * g, n, n)[g:g + n], non_blocking=True)
+        if hsk:
+            for f in ("vx", "vy", "vz", "m"):
+                hsk[f].copy_(getattr(sk, f), non_blocking=True)
+        torch.cuda.synchronize(dev)
+
+    e2e_step()
+    barrier()
+    t0 = time.perf_counter()
+    e2e_steps = max(1, min(args.steps, args.e2e_steps))
+    for _ in range(e2e_steps):
+        e2e_step()
+    e2e_s = reduce_max((time.perf_counter() - t0) / e2e_steps, world, dev)
+    if rank == 0:
+        peak, peak_src = measured_peak()
+        Nb = (n + 2 * g) ** 3
+        ab = algorithmic_bytes(N, Nb, w.sinks.n, w.sne.n, 1.0, 1.0, 1.0)      # dense 8(d) figures (the fractions are the default arm's business)
+        dom = max((k for k in pm.KERNEL_GROUPS if kernel_ms[k] > 0), key=lambda k: kernel_ms[k])
+        gbs = ab[dom] / (kernel_ms[dom] * 1e-3) / 1e9
+        line = {"metric": METRIC, "value": whole_job_value(N, args.steps, world, total_ms), "unit": UNIT, "n_gpus": world,
+                "steps": args.steps, "warmup": warm, "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak",
+                "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+                "config": {"workload": f"config5-shaped {n}^3 slab per rank, z-slab decomposition over {world} rank(s) (--sharded)",
+                           "cells_per_rank": N, "particles_per_rank": npart, "multi_gpu": "z slabs, nearest-neighbour exchange of ghost planes",
+                           "exchange_bytes_per_rank_per_step": xbytes, "l2_policy": "inputs larger than L2"},
+                "particles_per_s": world * npart * args.steps / (total_ms * 1e-3), "kernel_ms": kernel_ms, "clocks": clocks,
+                "e2e": {"value": world * N / e2e_s / 1e6, "unit": UNIT, "h2d_bytes_per_step": 6 * N * 8 + (7 * w.sinks.n + 8 * w.sne.n) * 8,
+                        "d2h_bytes_per_step": 6 * N * 8 + 4 * w.sinks.n * 8, "ms_per_step": e2e_s * 1e3, "steps": e2e_steps,
+                        "api": "sharded.SlabStep.step with pinned host buffers copied in and out around it"},
+                "gpu_launches": launches,
+                "roofline": {"bound": "hbm", "kernel": dom, "achieved": gbs, "peak": peak, "unit": "GB/s", "frac": gbs / peak,
+                             "peak_source": peak_src, "traffic": None, "algorithmic_bytes_per_launch": ab[dom],
+                             "accounting": "SURVEY.md 8(d) dense figures"},
+                "context": "the exchange step of SURVEY 8(f)4; the paper reports ~50% weak-scaling efficiency of its particle update "
+                           "to 8192 GPUs (L437); with one rank every exchange is a device copy onto the rank itself"}
+        if not args.no_cpu_baseline:
+            r = time_oracle(ORACLE_SAMPLE_N, 1)
+            line["cpu_baseline"] = {k: r[k] for k in ("value", "unit", "cores", "kind", "sample", "host_cores", "workload")}
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
 
 
 def run_ours(args, rank, world, local_rank):
@@ -229,9 +371,11 @@ def run_ours(args, rank, world, local_rank):
     for _ in range(warm):
         one_step()
     ctx.pm_check()
-    # activity fractions of the buffer the timed steps will see, at 32-byte sector (4-cell) granularity
+    # activity fractions of the buffer the timed steps will see: per cell (SURVEY 8(d)'s unit) and per 32-byte sector (4 cells)
     ctx.pm_deposit(st, sk, sn, w.dt)
     ctx.pm_fold_ghosts()
+    n_tiles, live_k, live_n = ctx.debug_tile_counts()           # before the debug view below marks every tile live
+    fk, fn = live_k / n_tiles, live_n / n_tiles
     sink_touched = ctx.debug_buffer(0)[1] != 0
     sn_touched = ctx.debug_buffer(1)[1] != 0          # SN d rho > 0 wherever an SN stencil has omega > 0
     touched = sink_touched | sn_touched
@@ -239,7 +383,7 @@ def run_ours(args, rank, world, local_rank):
     def frac4(m):
         return float(m.reshape(-1, 4).any(dim=1).double().mean())
 
-    t_frac, ts_frac = float(touched.double().mean()), float(sink_touched.double().mean())
+    t_frac, ts_frac, tn_frac = float(touched.double().mean()), float(sink_touched.double().mean()), float(sn_touched.double().mean())
     t4, ts4, tn4 = frac4(touched), frac4(sink_touched), frac4(sn_touched)
     del touched, sink_touched, sn_touched
     ctx.pm_apply_limited(st)
@@ -356,15 +500,27 @@ def run_ours(args, rank, world, local_rank):
 
     if rank == 0:
         peak, peak_src = measured_peak()
-        abytes = algorithmic_bytes(N, Nb, w.sinks.n, w.sne.n, t4, ts4, tn4, nch)
+        abytes = algorithmic_bytes(N, Nb, w.sinks.n, w.sne.n, t_frac, ts_frac, tn_frac, fk, fn, nch)
+        sbytes = algorithmic_bytes(N, Nb, w.sinks.n, w.sne.n, t4, ts4, tn4, fk, fn, nch)
+        dbytes = algorithmic_bytes(N, Nb, w.sinks.n, w.sne.n, 1.0, 1.0, 1.0, 1.0, 1.0, nch)
         kernels = {}
         for k in pm.KERNEL_GROUPS:
             if kernel_ms[k] > 0:
                 gbs = abytes[k] / (kernel_ms[k] * 1e-3) / 1e9
+                tr = ncu_traffic(k)
                 kernels[k] = {"ms": kernel_ms[k], "algorithmic_bytes": abytes[k], "achieved_gbs": gbs,
-                              "frac_of_measured_peak": gbs / peak, "traffic": ncu_traffic(k)}
+                              "frac_of_measured_peak": gbs / peak, "sector_bytes": sbytes[k], "dense_bytes": dbytes[k],
+                              "traffic": tr, "traffic_over_algorithmic": (tr / abytes[k]) if tr else None}
+        # reset + deposit as the one stage SURVEY 8(d) books them as (a0-a5): write every live buffer word once, gather each
+        # touched state cell once, particle records
+        a05_ms = sum(kernel_ms[k] for k in ("zero", "sinks", "sne"))
+        a05_bytes = sum(abytes[k] for k in ("zero", "sinks", "sne"))
+        stage_a0_a5 = {"ms": a05_ms, "algorithmic_bytes": a05_bytes,
+                       "achieved_gbs": a05_bytes / (a05_ms * 1e-3) / 1e9 if a05_ms > 0 else None,
+                       "frac_of_measured_peak": a05_bytes / (a05_ms * 1e-3) / 1e9 / peak if a05_ms > 0 else None,
+                       "kernels": ["k_tiles_mark", "k_tiles_zero", "k_zero_sweep", "k_deposit_sinks_g4", "k_deposit_sne_g3n4"]}
         dom = max(kernels, key=lambda k: kernels[k]["ms"])
-        kname = {"sne": "k_deposit_sne_g3n4", "apply": "k_apply_limited", "zero": "k_zero_buffer", "sinks": "k_deposit_sinks_g4",
+        kname = {"sne": "k_deposit_sne_g3n4", "apply": "k_apply_limited", "zero": "k_zero_sweep", "sinks": "k_deposit_sinks_g4",
                  "fold": "k_fold_ghosts", "return": "k_return_sinks_g4", "bin": "k_bin_*"}[dom]
         step_bytes = sum(abytes.values())
         line = {
@@ -374,8 +530,9 @@ def run_ours(args, rank, world, local_rank):
             "config": {"workload": w.name + ("+appendixA_reproducible" if args.reproducible else ""), "cells": N, "particles": npart, "sinks": w.sinks.n, "sne": w.sne.n,
                        "multi_gpu": "replicas only" if world > 1 else "single GPU",
                        "l2_policy": "inputs larger than L2 (state 6 fields + 6-channel buffer, GBs >> 126 MB)",
-                       "touched_cell_fraction": t_frac, "sink_touched_fraction": ts_frac,
-                       "touched_sector_fraction": t4, "sink_sector_fraction": ts4, "sn_sector_fraction": tn4},
+                       "touched_cell_fraction": t_frac, "sink_cell_fraction": ts_frac, "sn_cell_fraction": tn_frac,
+                       "touched_sector_fraction": t4, "sink_sector_fraction": ts4, "sn_sector_fraction": tn4,
+                       "live_tile_fraction_accretion": fk, "live_tile_fraction_sn": fn},
             "particles_per_s": world * npart * args.steps / (total_ms * 1e-3),
             "stage_ms": stage_ms,
             "kernel_ms": kernel_ms,
@@ -386,16 +543,20 @@ def run_ours(args, rank, world, local_rank):
             "gpu_launches": launches,
             "roofline": {"bound": "hbm", "kernel": kname, "achieved": kernels[dom]["achieved_gbs"], "peak": peak,
                          "unit": "GB/s", "frac": kernels[dom]["frac_of_measured_peak"], "peak_source": peak_src,
-                         "traffic": kernels[dom]["traffic"], "algorithmic_bytes_per_launch": abytes[dom],
+                         "traffic": kernels[dom]["traffic"], "traffic_over_algorithmic": kernels[dom]["traffic_over_algorithmic"],
+                         "algorithmic_bytes_per_launch": abytes[dom], "sector_bytes_per_launch": sbytes[dom],
+                         "accounting": "SURVEY.md 8(d): each touched CELL once; the reset + write-back of the buffer is the `zero` "
+                                       "group's (8(d) row 1), not the deposit kernels'",
                          "launch_ms": kernels[dom]["ms"], "share_of_step": kernels[dom]["ms"] / sum(kernel_ms.values()),
                          "timing": "CUDA events recorded by the library on the launching stream (PM_FLAG_TIMING ctx, after the timed region), median of 3 steps",
                          "frac_of_8tbs_nominal": kernels[dom]["achieved_gbs"] / 8000.0},
             "kernels": kernels,
-            "step_roofline": {"algorithmic_bytes_per_step": step_bytes,
+            "stage_a0_a5": stage_a0_a5,
+            "step_roofline": {"algorithmic_bytes_per_step": step_bytes, "sector_bytes_per_step": sum(sbytes.values()),
                               "achieved_gbs": step_bytes / (ms_per_step * 1e-3) / 1e9,
                               "frac_of_measured_peak": step_bytes / (ms_per_step * 1e-3) / 1e9 / peak,
                               "frac_of_8tbs_nominal": step_bytes / (ms_per_step * 1e-3) / 1e9 / 8000.0,
-                              "dense_survey_bytes": 8.0 * nch * Nb + 8.0 * 5 * N + 120.0 * npart + 144.0 * (Nb - N) + 176.0 * N + 32.0 * ts4 * N},
+                              "dense_survey_bytes": sum(dbytes.values())},
         }
         if creation:
             line["sink_creation"] = creation
@@ -406,8 +567,8 @@ def run_ours(args, rank, world, local_rank):
             red_probe["sn_deposit_achieved"] = n_red / (kernel_ms["sne"] * 1e-3) / 1e9 if kernel_ms["sne"] > 0 else None
             line["red_throughput"] = red_probe
         if world == 1 and not args.no_cpu_baseline:
-            r = time_oracle(ORACLE_SAMPLE_N, 1)
-            line["cpu_baseline"] = {k: r[k] for k in ("value", "unit", "cores", "kind", "sample")}
+            r = time_oracle(512 if args.cpu_baseline_full else ORACLE_SAMPLE_N, 1)
+            line["cpu_baseline"] = {k: r[k] for k in ("value", "unit", "cores", "kind", "sample", "host_cores", "workload")}
         line["context"] = "paper: ~50% weak-scaling efficiency to 8192 MI250X GPUs on Frontier (PAPER.md L9, L437); no throughput published"
         print(json.dumps(line), flush=True)
     if world > 1:
@@ -426,12 +587,19 @@ def main():
                     help="time another BASELINE config instead of config 5 (for the table in DESIGN.md; the headline is config 5)")
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-baseline-full", action="store_true",
+                    help="time the oracle on config 5 itself (512^3, ~90 s per step, ~25 GB of host memory) instead of the bounded 256^3 sample")
+    ap.add_argument("--sharded", action="store_true",
+                    help="z-slab decomposition (SURVEY 8(f)4): every rank holds one n^3 slab of an n x n x (n world) domain and "
+                         "exchanges ghost planes with its z neighbours; default (without the flag): independent replicas")
     ap.add_argument("--reproducible", action="store_true",
                     help="Appendix A mode (PM_FLAG_REPRODUCIBLE): 4 more buffer channels + rounding pass; a separate workload variant")
     args = ap.parse_args()
     rank, world, local_rank = env_int("RANK", 0), env_int("WORLD_SIZE", 1), env_int("LOCAL_RANK", 0)
     if args.impl == "reference":
         run_reference(args, rank, world)
+    elif args.sharded:
+        run_sharded(args, rank, world, local_rank)
     else:
         run_ours(args, rank, world, local_rank)
 

@@ -86,6 +86,9 @@ typedef struct {
     double sn_eint_theta;        /* Eq. 21 floor: e_min = theta rho_2 (e_int,1/rho_1); 1 = as printed, 0 = e_int >= 0 only (R25) */
     double truelove_J;           /* Jeans number J of Eq. 12, rho_Tr = J^2 pi c_s^2 / (G dx^2); 0.25 in the paper (L148); 0 = the Truelove
                                   * terms of Eqs. 13-14 and 16 are off (all BASELINE configs) */
+    int32_t z_slab;              /* 0: one periodic domain (Step 2 is the in-device fold).  1: this ctx holds the nz planes of one z slab
+                                  * of a larger domain (periodic in x and y inside the ctx, cut along z): see pm_slab_describe */
+    int32_t pad_;
 } pm_params;
 
 enum {
@@ -134,6 +137,37 @@ int pm_apply_limited(pm_ctx *ctx, pm_state *state);
 
 /* Step 4.  Must be given the same sinks (same n, same positions) as the preceding pm_deposit. */
 int pm_return_to_particles(pm_ctx *ctx, pm_sinks *sinks);
+
+/* ---- z-slab decomposition.  Step 2 as the paper states it: "add the contents of the ghost zones on each
+ * rank to the corresponding real zones on other ranks" (L67-71, Eq. 3), the one non-local step (L97).  A ctx created with
+ * z_slab = 1 owns the planes k in [0, nz) of its slab; rank r's lower neighbour is r - 1, its upper neighbour r + 1 (periodic
+ * in the rank index).  What changes for the caller:
+ *   * every mesh array in pm_state holds (nz + 2g) ny nx values: g ghost planes (g = state_ghost_planes), the nz owned planes,
+ *     g ghost planes; the ghost planes must hold the neighbours' boundary planes BEFORE pm_deposit (the halo exchange every
+ *     hydro code already has; particles near a z face read gas across it).  pm_apply_limited updates owned planes only.
+ *   * sequence:  pm_deposit -> pm_slab_pack -> [send buf_send_lo to the lower neighbour's buf_recv_hi, buf_send_hi to the upper
+ *     neighbour's buf_recv_lo] -> pm_fold_ghosts -> pm_apply_limited -> [send ret_send_lo to the lower neighbour's ret_recv_hi,
+ *     ret_send_hi to the upper neighbour's ret_recv_lo; the same for rtr_* when truelove_J > 0] -> pm_return_to_particles.
+ *     The transfers are the caller's (NCCL / torch.distributed / cudaMemcpyPeer); they must be ordered after the preceding and
+ *     before the following call on the ctx's stream.  The second exchange is the owner -> ghost copy of (eta, v_old) that
+ *     Step 4 needs for sinks whose kernel crosses a z face (L79); the paper does not mention it (R16).
+ *   * a slab message is [channel][g planes][ny + 2g][row pitch] doubles, unfolded; the receiver adds the images of a cell in
+ *     the same fixed order as the single-domain fold (Appendix A), so one rank that is its own neighbour reproduces
+ *     the periodic fold bit for bit.
+ * Not available on a slab: pm_step_host and the PM-gravity calls. */
+typedef struct {
+    void *buf_send_lo, *buf_send_hi, *buf_recv_lo, *buf_recv_hi;   /* DEVICE, ctx-owned, buf_bytes each */
+    int64_t buf_bytes;
+    void *ret_send_lo, *ret_send_hi, *ret_recv_lo, *ret_recv_hi;   /* DEVICE, inside the ctx's return mesh, ret_bytes each (NULL / 0: no sinks) */
+    int64_t ret_bytes;
+    void *rtr_send_lo, *rtr_send_hi, *rtr_recv_lo, *rtr_recv_hi;   /* the same for the Truelove excess kept for Step 4 (NULL / 0 when off) */
+    int64_t rtr_bytes;
+    int32_t state_ghost_planes;                                     /* g */
+    int32_t pad_;
+} pm_slab_desc;
+int pm_slab_describe(pm_ctx *ctx, pm_slab_desc *out);
+/* After pm_deposit: fill buf_send_lo / buf_send_hi from the buffer mesh's z ghost planes (stale tiles as zeros). */
+int pm_slab_pack(pm_ctx *ctx);
 
 /* Margin M of Appendix A (N_bit = log2 r + 52 + M; default 28, the paper's example, L612).  Needs PM_FLAG_REPRODUCIBLE. */
 int pm_set_repro_margin(pm_ctx *ctx, int32_t M);
@@ -225,6 +259,10 @@ int pm_probe_red_f64(pm_ctx *ctx, int64_t footprint_bytes, int32_t channels, dou
  * cell (0,0,0); owned cell (i,j,k) sits at origin + (k*dims[1] + j)*dims[2] + i, ghost cells at i,j,k in [-g, n+g).
  * *ghost = g.  Stale tiles (no particle touched them in this step) are filled with the zeros they stand for first. */
 int pm_debug_buffer(pm_ctx *ctx, int channel, const double **dev_ptr, int64_t dims[3], int64_t *origin, int32_t *ghost);
+
+/* Tiles of the buffer mesh (8^3 cells, ghost tiles included) and how many of them the last pm_deposit marked live per channel
+ * group (K: accretion channel, N: supernova channels); stale tiles are neither reset nor read.  HOST outputs.  Synchronises. */
+int pm_debug_tile_counts(pm_ctx *ctx, int64_t *n_tiles, int64_t *live_k, int64_t *live_n);
 
 /* Return mesh: one record of 4 doubles per cell (eta of Eq. 4, pre-step velocity x, y, z), valid where buffer channel
  * 0 != 0.  *dev_ptr points at word `word` of cell 0; the same word of cell q is at dev_ptr[4 q]. */

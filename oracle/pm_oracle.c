@@ -84,6 +84,9 @@ typedef struct {
     int32_t *sink_count; /* number of sinks contributing to the cell */
     double *Tp;          /* Appendix A (L600-606): sum over SNe of |dp_x^s| + |dp_y^s| + |dp_z^s|, the magnitudes of the values ADDED */
     double *Te;          /* ... and of |dE^s|; one addition per particle and cell, as in the paper's E update */
+    double *Scond[5];    /* error scale only (L610, R36): how strongly the cell's SN terms depend on the ROUNDING of v_COM, which is a
+                          * cancelling stencil sum (Eq. 18): sum_s (omega rho + d rho) * [sum_cells omega rho V |v|]_s / M_snr,s for the
+                          * momentum channels, sum_s |p_rad| . (the same) for d E; [0] unused.  May be NULL. */
 } orc_mesh_out;
 
 #define FOUR_PI 12.566370614359172953850573533118
@@ -224,6 +227,7 @@ typedef struct {
     int64_t ih, jh, kh;
     int g;
     double m_snr, v_snr, vcx, vcy, vcz, e_kin, n_h, r_m, p_rad;
+    double pabs[3];           /* error scale only: sum over the stencil of omega rho V |v| per component (the terms of Eq. 18's sum) */
     int regime;
 } sn_scalars;
 
@@ -257,6 +261,7 @@ static void sn_compute_scalars(const orc_params *p, const orc_state *U, double x
     o->g = kernel_halfwidth(p->rk_sn, p->dx);
     const int g = o->g;
     double m_gas = 0.0, px = 0.0, py = 0.0, pz = 0.0, v_snr = 0.0;
+    o->pabs[0] = o->pabs[1] = o->pabs[2] = 0.0;
     for (int64_t k = o->kh - g; k <= o->kh + g; ++k)
         for (int64_t j = o->jh - g; j <= o->jh + g; ++j)
             for (int64_t i = o->ih - g; i <= o->ih + g; ++i) {
@@ -272,6 +277,7 @@ static void sn_compute_scalars(const orc_params *p, const orc_state *U, double x
                 py += mcell * vy;
                 pz += mcell * vz;
                 v_snr += omega * V;                                   /* R18 */
+                o->pabs[0] += mcell * fabs(vx); o->pabs[1] += mcell * fabs(vy); o->pabs[2] += mcell * fabs(vz);   /* error scale only */
             }
     o->m_snr = m_gas + m_ej;                                          /* L203 */
     o->v_snr = v_snr;
@@ -297,7 +303,7 @@ static void sn_compute_scalars(const orc_params *p, const orc_state *U, double x
 /* O5: Eq. 17 for one cell with omega > 0 (R21, R22). out = (d rho, d px, d py, d pz, d E). */
 static void sn_cell_deposit(const orc_params *p, const sn_scalars *sc, double xs, double ys, double zs,
                             double e_sn, double m_ej, int64_t i, int64_t j, int64_t k, int cnt,
-                            double rho, double vx, double vy, double vz, double out[5], double out_abs[5]) {
+                            double rho, double vx, double vy, double vz, double out[5], double out_abs[5], double out_cond[5]) {
     const double nsub3 = (double)p->sn_nsub * (double)p->sn_nsub * (double)p->sn_nsub;
     double omega = (double)cnt / nsub3;
     double ddx = cell_centre(p->x0[0], i, p->dx) - xs;
@@ -321,6 +327,13 @@ static void sn_cell_deposit(const orc_params *p, const sn_scalars *sc, double xs
     out_abs[2] = omega * rho * (fabs(sc->vcy) + fabs(vy)) + drho * fabs(sc->vcy) + fabs(pry);
     out_abs[3] = omega * rho * (fabs(sc->vcz) + fabs(vz)) + drho * fabs(sc->vcz) + fabs(prz);
     out_abs[4] = omega * (e_sn + sc->e_kin) / sc->v_snr + ((fabs(sc->vcx * prx) + fabs(sc->vcy * pry)) + fabs(sc->vcz * prz));
+    /* error scale only: v_COM is known to eps * (number of additions) * pabs / M_snr at best -- the stencil sum of Eq. 18 cancels
+     * when the gas already streams away from the particle -- and enters the terms above with these factors */
+    out_cond[0] = 0.0;
+    out_cond[1] = (omega * rho + drho) * (sc->pabs[0] / sc->m_snr);
+    out_cond[2] = (omega * rho + drho) * (sc->pabs[1] / sc->m_snr);
+    out_cond[3] = (omega * rho + drho) * (sc->pabs[2] / sc->m_snr);
+    out_cond[4] = (fabs(prx) * sc->pabs[0] + fabs(pry) * sc->pabs[1] + fabs(prz) * sc->pabs[2]) / sc->m_snr;
 }
 
 static void store_sn_diag(orc_sne *sn, int64_t s, const sn_scalars *sc) {
@@ -439,7 +452,7 @@ static void zero_mesh(double *a, int64_t n) { if (a) memset(a, 0, (size_t)n * si
 int orc_deposit(const orc_params *p, const orc_state *U, orc_sinks *sk, orc_sne *sn, double dt, orc_mesh_out *mo) {
     const int64_t N = (int64_t)p->nx * p->ny * p->nz;
     for (int f = 0; f < 6; ++f) { if (!mo->A[f]) return -1; zero_mesh(mo->A[f], N); zero_mesh(mo->Aabs[f], N); }
-    for (int f = 0; f < 5; ++f) { if (!mo->S[f]) return -1; zero_mesh(mo->S[f], N); zero_mesh(mo->Sabs[f], N); }
+    for (int f = 0; f < 5; ++f) { if (!mo->S[f]) return -1; zero_mesh(mo->S[f], N); zero_mesh(mo->Sabs[f], N); zero_mesh(mo->Scond[f], N); }
     if (mo->sn_count) memset(mo->sn_count, 0, (size_t)N * sizeof(int32_t));
     if (mo->sink_count) memset(mo->sink_count, 0, (size_t)N * sizeof(int32_t));
     zero_mesh(mo->Tp, N); zero_mesh(mo->Te, N);
@@ -488,12 +501,13 @@ int orc_deposit(const orc_params *p, const orc_state *U, orc_sinks *sk, orc_sne 
                     if (cnt == 0) continue;
                     int64_t c = cell_index(p, i, j, k);
                     double rho = U->rho[c];
-                    double d[5], da[5];
+                    double d[5], da[5], dc[5];
                     sn_cell_deposit(p, &sc, xs, ys, zs, sn->e_sn[s], sn->m_ej[s], i, j, k, cnt,
-                                    rho, U->mx[c] / rho, U->my[c] / rho, U->mz[c] / rho, d, da);
+                                    rho, U->mx[c] / rho, U->my[c] / rho, U->mz[c] / rho, d, da, dc);
                     for (int f = 0; f < 5; ++f) {
                         mo->S[f][c] += d[f];
                         if (mo->Sabs[f]) mo->Sabs[f][c] += da[f];
+                        if (mo->Scond[f]) mo->Scond[f][c] += dc[f];
                     }
                     if (mo->Tp) mo->Tp[c] += (fabs(d[1]) + fabs(d[2])) + fabs(d[3]);
                     if (mo->Te) mo->Te[c] += fabs(d[4]);
@@ -709,10 +723,11 @@ int orc_sample_cells(const orc_params *p, const orc_state *U, const orc_sinks *s
             if (cnt == 0) continue;
             sn_scalars sc;
             sn_compute_scalars(p, U, sn->x[s], sn->y[s], sn->z[s], sn->vx[s], sn->vy[s], sn->vz[s], sn->e_sn[s], sn->m_ej[s], &sc);
-            double d[5], da[5];
+            double d[5], da[5], dc[5];
             sn_cell_deposit(p, &sc, sn->x[s], sn->y[s], sn->z[s], sn->e_sn[s], sn->m_ej[s], ih + di, jh + dj, kh + dk, cnt,
-                            rho, U->mx[c] / rho, U->my[c] / rho, U->mz[c] / rho, d, da);
-            for (int f = 0; f < 5; ++f) { S[f] += d[f]; Sa[f] += da[f]; }
+                            rho, U->mx[c] / rho, U->my[c] / rho, U->mz[c] / rho, d, da, dc);
+            /* the sampled evaluation folds the v_COM conditioning into its one error scale (half the weight of a term) */
+            for (int f = 0; f < 5; ++f) { S[f] += d[f]; Sa[f] += da[f] + 0.5 * dc[f]; }
             nsn += 1;
         }
         double u[6] = { U->rho[c], U->mx[c], U->my[c], U->mz[c], U->etot[c], U->eint[c] };

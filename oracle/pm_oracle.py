@@ -61,7 +61,8 @@ class OrcSNe(C.Structure):
 
 class OrcMeshOut(C.Structure):
     _fields_ = [("A", c_dp * 6), ("S", c_dp * 5), ("Aabs", c_dp * 6), ("Sabs", c_dp * 5),
-                ("eta", c_dp), ("lam", c_dp), ("sn_count", c_ip), ("sink_count", c_ip), ("Tp", c_dp), ("Te", c_dp)]
+                ("eta", c_dp), ("lam", c_dp), ("sn_count", c_ip), ("sink_count", c_ip), ("Tp", c_dp), ("Te", c_dp),
+                ("Scond", c_dp * 5)]
 
 
 def build(force: bool = False) -> str:
@@ -158,7 +159,9 @@ SN_DIAG = ("m_snr", "v_snr", "vcx", "vcy", "vcz", "n_h", "r_m", "p_rad")
 class Oracle:
     """Holds one problem (params, state, particles; all numpy, modified in place by step())."""
 
-    def __init__(self, params: dict, state, sinks, sne, keep_abs: bool = True, mesh: bool = True):
+    def __init__(self, params: dict, state, sinks, sne, keep_abs: bool = True, mesh: bool = True, abs_channels=None):
+        """abs_channels = (accretion channels, SN channels) whose error-scale meshes (Aabs, Sabs) are kept; None: all of them
+        (with keep_abs) -- a 512^3 run keeps only the ones its comparisons read."""
         self.L = lib()
         self.pd = dict(params)
         self.p = make_params(params)
@@ -168,14 +171,17 @@ class Oracle:
         N = self.N if mesh else 0          # mesh=False: only sample_cells / particle_scalars / sink_amounts are used
         self.A = [np.zeros(N) for _ in range(6)]
         self.S = [np.zeros(N) for _ in range(5)]
-        self.Aabs = [np.zeros(N) for _ in range(6)] if keep_abs else [None] * 6
-        self.Sabs = [np.zeros(N) for _ in range(5)] if keep_abs else [None] * 5
+        ka, ks = (range(6), range(5)) if abs_channels is None else abs_channels
+        self.Aabs = [np.zeros(N) if (keep_abs and f in ka) else None for f in range(6)]
+        self.Sabs = [np.zeros(N) if (keep_abs and f in ks) else None for f in range(5)]
+        # how strongly a cell's SN terms depend on the rounding of v_COM, a cancelling stencil sum (error scale only, see the C file)
+        self.Scond = [np.zeros(N) if (keep_abs and f in ks and f > 0) else None for f in range(5)]
         self.eta = np.ones(N)
         self.lam = np.ones(N)
         self.sn_count = np.zeros(N, dtype=np.int32)
         self.sink_count = np.zeros(N, dtype=np.int32)
-        self.Tp = np.zeros(N) if keep_abs else None      # Appendix A error scales (sum of |values added| per cell)
-        self.Te = np.zeros(N) if keep_abs else None
+        self.Tp = np.zeros(N) if (keep_abs and abs_channels is None) else None      # Appendix A error scales (sum of |values added| per cell)
+        self.Te = np.zeros(N) if (keep_abs and abs_channels is None) else None
         self.sink_diag = {k: np.zeros(sinks.n) for k in SINK_DIAG}
         self.sink_diag["n_member"] = np.zeros(sinks.n, dtype=np.int32)
         self.sn_diag = {k: np.zeros(sne.n) for k in SN_DIAG}
@@ -218,6 +224,7 @@ class Oracle:
         for f in range(5):
             o.S[f] = _dp(self.S[f])
             o.Sabs[f] = _dp(self.Sabs[f])
+            o.Scond[f] = _dp(self.Scond[f])
         o.eta, o.lam = _dp(self.eta), _dp(self.lam)
         o.sn_count, o.sink_count = _ip(self.sn_count), _ip(self.sink_count)
         o.Tp, o.Te = _dp(self.Tp), _dp(self.Te)

@@ -14,6 +14,7 @@
 #include "pm_fast.cuh"
 #include "pm_create.cuh"
 #include "pm_gravity.cuh"
+#include "pm_slab.cuh"
 #include "../../include/pm.h"
 
 #include <algorithm>
@@ -71,6 +72,9 @@ struct pm_ctx {
     const double *gperm_x; long long gperm_n; bool gperm_valid;   // gravity: perm in grav_mem orders the n particles at gperm_x by host tile
     bool buffer_valid;  // a deposit + fold has filled the buffer mesh (sink creation reads its accretion channel)
     bool ever_deposited;
+    double *slab_mem;   // z-slab mode: send_lo | send_hi | recv_lo | recv_hi, each nch * g * pk doubles (pm_slab.cuh)
+    long long slab_elems;   // doubles per slab
+    bool slab_packed;   // pm_slab_pack has run since the last pm_deposit
     bool grav_in_ch1;   // buffer channel 1 holds the last pm_gravity_deposit (until the next pm_deposit): the debug view must not
                         // "fill in" its stale tiles
     bool timing;        // PM_FLAG_TIMING
@@ -396,9 +400,15 @@ __device__ __forceinline__ void stv(double *p, const double v[VEC]) {
 // either (a deposit that reaches a ghost cell also claims the tile of its image), so there is nothing to do for it.  Channel 0
 // belongs to group K, channels 1..7 to group N, the Appendix A count channel (8) is live where either group is.
 // STAMPS = false: plain fold of NCH channels starting at buf (PM gravity, which resets its one channel by a sweep).
+// Slab mode (P.zopen): the z images are not in this buffer but in the two slabs received from the z neighbours (Eq. 3 as the
+// paper states it: "add the contents of the ghost zones on each rank to the corresponding real zones on other ranks", L67):
+// recv_lo = the lower neighbour's HIGH ghost planes, recv_hi = the upper neighbour's LOW ghost planes, each packed as
+// [channel][g planes][ny + 2g][row pitch] with stale tiles already replaced by zeros (k_slab_pack).  Same image order, same
+// additions: with one rank (its own neighbour) the result is bit-identical to the periodic fold.
 template <int W, int NCH, bool STAMPS>
 __global__ void __launch_bounds__(256) k_fold_ghosts(const DevP P, double *__restrict__ buf, const Tiles T, long long n_edge,
-                                                     long long n_zslab, long long n_yslab) {
+                                                     long long n_zslab, long long n_yslab, const double *__restrict__ recv_lo,
+                                                     const double *__restrict__ recv_hi) {
     const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (t >= n_edge) return;
     const int g = P.g, nx = P.nx, ny = P.ny, nz = P.nz;
@@ -438,17 +448,23 @@ __global__ void __launch_bounds__(256) k_fold_ghosts(const DevP P, double *__res
     long long img[8];
     bool ok[8];
     unsigned lk = 0xffu, ln = 0xffu;       // bit m: image m's tile is live in group K / N (bit 0: the owned cell's own tile)
+    const bool slab = P.zopen != 0;
+    const long long slab_ch = (long long)P.g * P.pk;                 // elements of one channel of a received slab
+    const double *const rz = oz > 0 ? recv_lo : recv_hi;             // k < g: lower neighbour; k >= nz - g: upper neighbour
+    const int pz = oz > 0 ? k : k - (nz - g);                        // plane of the received slab that images plane k
 #pragma unroll
     for (int m = 1; m < 8; ++m) {
         const int cx = m & 1, cy = (m >> 1) & 1, cz = m >> 2;
         ok[m] = (!cx || ox) && (!cy || oy) && (!cz || oz);
-        img[m] = ghost_index(P, i + cx * ox, j + cy * oy, k + cz * oz);
+        img[m] = (slab && cz) ? (long long)pz * P.pk + (long long)(j + cy * oy + P.g) * P.pj + (i + cx * ox + P.gx)
+                              : ghost_index(P, i + cx * ox, j + cy * oy, k + cz * oz);
     }
     if (STAMPS) {
         lk = 0; ln = 0;
 #pragma unroll
         for (int m = 0; m < 8; ++m) {
             const int cx = m & 1, cy = (m >> 1) & 1, cz = m >> 2;
+            if (slab && cz) { if (ok[m]) { lk |= 1u << m; ln |= 1u << m; } continue; }      // received slabs hold values or zeros
             if (m == 0 || ok[m]) {
                 const unsigned f = T.live[tile_index(P, i + cx * ox, j + cy * oy, k + cz * oz)];
                 lk |= (f & kLiveK ? 1u : 0u) << m;
@@ -471,7 +487,7 @@ __global__ void __launch_bounds__(256) k_fold_ghosts(const DevP P, double *__res
             for (int m = 1; m < 8; ++m)
                 if (ok[m] && (live >> m & 1u)) {
                     double v[W];
-                    ldv<W>(b + img[m], v);
+                    ldv<W>(((slab && (m >> 2)) ? rz + (long long)ch * slab_ch : b) + img[m], v);
 #pragma unroll
                     for (int e = 0; e < W; ++e) a[e] += v[e];
                 }
@@ -544,7 +560,7 @@ __global__ void __launch_bounds__(kApplyThreads, 6) k_apply_limited(const DevP P
     const unsigned int row = item / items_per_row;
     const unsigned int i0 = (item - row * items_per_row) * VEC;
     const unsigned int k = row / (unsigned int)P.ny, j = row - k * (unsigned int)P.ny;
-    const long long q = (long long)row * P.nx + i0;
+    const long long q = (long long)row * P.nx + i0 + P.zoff;     // state / return-mesh index (zoff: ghost planes of a z slab)
     const long long gq = (long long)(k + P.g) * P.pk + (long long)(j + P.g) * P.pj + (i0 + P.gx);
     // a stale tile stands for zeros and is not read (pm_tiles.cuh); the VEC cells of an item lie in one tile (i0 is even)
     const unsigned lf = __ldg(T.live + tile_index(P, (int)i0, (int)j, (int)k));
@@ -584,7 +600,7 @@ __global__ void __launch_bounds__(kApplyThreads, 6) k_apply_limited(const DevP P
     // Skip at WARP granularity: a warp covers 32*VEC consecutive cells of each field (512 B per stream at VEC = 2), so
     // the state traffic is either whole coalesced lines or nothing (sector-sparse reads waste DRAM bursts).
     const bool wany = __any_sync(0xffffffffu, any);
-    if (LAM && valid && !any) { double one[VEC]; for (int v = 0; v < VEC; ++v) one[v] = 1.0; stv<VEC>(lam_out + q, one); }
+    if (LAM && valid && !any) { double one[VEC]; for (int v = 0; v < VEC; ++v) one[v] = 1.0; stv<VEC>(lam_out + (q - P.zoff), one); }
     if (!wany || !valid) return;                // dU^sum = 0 on the whole segment: U unchanged, nothing to read or write
     double *fld[6] = { U.rho, U.mx, U.my, U.mz, U.etot, U.eint };
     double u[6][VEC];
@@ -610,7 +626,7 @@ __global__ void __launch_bounds__(kApplyThreads, 6) k_apply_limited(const DevP P
     if (!any) return;                           // lanes of a touched segment whose own cells are untouched
 #pragma unroll
     for (int f = 0; f < 6; ++f) stv<VEC>(fld[f] + q, u[f]);
-    if (LAM) stv<VEC>(lam_out + q, lam);
+    if (LAM) stv<VEC>(lam_out + (q - P.zoff), lam);
 }
 
 // ---------------------------------------------------------------------------------------------------------------
@@ -697,7 +713,8 @@ extern "C" int pm_create(const pm_params *prm, int device, void *cuda_stream, pm
     if (g < 1 || g > 8) return PM_EINVAL;
     if (prm->nx < 2 * g + 1 || prm->ny < 2 * g + 1 || prm->nz < 2 * g + 1) return PM_EINVAL;     // R32
     const long long N = (long long)prm->nx * prm->ny * prm->nz;
-    if (N >= (1ll << 31)) return PM_EINVAL;
+    if (prm->z_slab != 0 && prm->z_slab != 1) return PM_EINVAL;
+    if ((long long)prm->nx * prm->ny * (prm->nz + (prm->z_slab ? 2 * g : 0)) >= (1ll << 31)) return PM_EINVAL;
     if ((long long)(prm->nx + 2 * g + 2) * (prm->ny + 2 * g) * (prm->nz + 2 * g) >= (1ll << 31)) return PM_EINVAL;
 
     pm_ctx *c = new (std::nothrow) pm_ctx();
@@ -728,6 +745,7 @@ extern "C" int pm_create(const pm_params *prm, int device, void *cuda_stream, pm
     P.ntile = (P.nsbx * P.nsby * P.nsbz) << (3 * kSbLog2);
     P.ntx = ((prm->nx + g + 7) >> 3) + 1; P.nty = ((prm->ny + g + 7) >> 3) + 1; P.ntz = ((prm->nz + g + 7) >> 3) + 1;
     c->ntiles = (long long)P.ntx * P.nty * P.ntz;
+    P.zopen = prm->z_slab; P.zoff = prm->z_slab ? g * prm->ny * prm->nx : 0;
 
     cudaError_t e = cudaSetDevice(device);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, device);
@@ -745,13 +763,19 @@ extern "C" int pm_create(const pm_params *prm, int device, void *cuda_stream, pm
     if (e == cudaSuccess) e = cudaMalloc(&c->tile_live, (size_t)c->ntiles);
     // before the first deposit every tile is stale = zeros
     if (e == cudaSuccess) e = cudaMemsetAsync(c->tile_live, 0, (size_t)c->ntiles, c->stream);
-    if (e == cudaSuccess && gs > 0) e = cudaMalloc(&c->ret, (size_t)kRetWords * N * sizeof(double));
-    if (e == cudaSuccess && gs > 0 && P.tl_num > 0.0) e = cudaMalloc(&c->ret_tr, (size_t)N * sizeof(double));
+    const long long Nst = N + 2ll * P.zoff;              // cells of a state array / of the return mesh (z ghost planes in slab mode)
+    if (e == cudaSuccess && gs > 0) e = cudaMalloc(&c->ret, (size_t)kRetWords * Nst * sizeof(double));
+    if (e == cudaSuccess && gs > 0 && P.tl_num > 0.0) e = cudaMalloc(&c->ret_tr, (size_t)Nst * sizeof(double));
+    if (e == cudaSuccess && P.zopen) {
+        c->slab_elems = (long long)c->nch * g * P.pk;
+        e = cudaMalloc(&c->slab_mem, (size_t)4 * c->slab_elems * sizeof(double));
+        if (e == cudaSuccess) e = cudaMemsetAsync(c->slab_mem, 0, (size_t)4 * c->slab_elems * sizeof(double), c->stream);
+    }
     if (e == cudaSuccess && (prm->flags & PM_FLAG_DEBUG_LAMBDA)) e = cudaMalloc(&c->lam, (size_t)N * sizeof(double));
     if (e == cudaSuccess) e = cudaMalloc(&c->err_flag, sizeof(int));
     if (e == cudaSuccess) e = cudaMallocHost(&c->err_host, 2 * sizeof(int));   // [0] error flag, [1] sink-creation count
     if (e == cudaSuccess) e = cudaMemsetAsync(c->err_flag, 0, sizeof(int), c->stream);
-    if (e == cudaSuccess && c->ret) e = cudaMemsetAsync(c->ret, 0, (size_t)kRetWords * N * sizeof(double), c->stream);
+    if (e == cudaSuccess && c->ret) e = cudaMemsetAsync(c->ret, 0, (size_t)kRetWords * Nst * sizeof(double), c->stream);
     if (e == cudaSuccess) {
         // opt in to the dynamic shared memory the SN kernel may need (<= 8 warps x tables)
         const size_t smem = kSnWarps * sn_table_bytes(2 * (gn > 0 ? gn : 1) + 1, P.nsub);
@@ -763,6 +787,7 @@ extern "C" int pm_create(const pm_params *prm, int device, void *cuda_stream, pm
         cudaGetLastError();
         if (c->buf) cudaFree(c->buf);
         if (c->tile_live) cudaFree(c->tile_live);
+        if (c->slab_mem) cudaFree(c->slab_mem);
         if (c->ret) cudaFree(c->ret);
         if (c->ret_tr) cudaFree(c->ret_tr);
         if (c->lam) cudaFree(c->lam);
@@ -792,6 +817,7 @@ extern "C" int pm_destroy(pm_ctx *c) {
     if (c->bin_mem) cudaFree(c->bin_mem);
     if (c->grav_mem) cudaFree(c->grav_mem);
     if (c->tile_live) cudaFree(c->tile_live);
+    if (c->slab_mem) cudaFree(c->slab_mem);
     if (c->create_mem) cudaFree(c->create_mem);
     if (c->err_flag) cudaFree(c->err_flag);
     if (c->err_host) cudaFreeHost(c->err_host);
@@ -835,7 +861,7 @@ extern "C" int pm_deposit(pm_ctx *c, const pm_state *st, const pm_sinks *sk, con
     const long long np = nk + nn;
     int *keys = nullptr, *perm = nullptr, *counts = nullptr, *live = nullptr;
     unsigned char *occ = nullptr;
-    if (np > 0) {   // a1: bin particles by host tile
+    if (np > 0 || P.zopen) {   // a1: bin particles by host tile (a slab without particles still needs the scratch of the reset)
         if (np >= (1ll << 31)) PM_FAIL(c, PM_EINVAL, "pm_deposit: too many particles");
         const int nkeys = 2 * P.ntile + 1;
         const int nscan = (nkeys + kScanChunk - 1) / kScanChunk;
@@ -853,23 +879,25 @@ extern "C" int pm_deposit(pm_ctx *c, const pm_state *st, const pm_sinks *sk, con
         occ = reinterpret_cast<unsigned char *>(sums + nscan);
         live = sums + nscan + nocc;
         PM_CUDA(c, cudaMemsetAsync(counts, 0, (size_t)(nkeys + nscan + nocc + 2) * sizeof(int), c->stream));
-        const unsigned blocks = (unsigned)((np + 255) / 256);
-        tick(c, PM_K_BIN, 0);
-        k_bin_count<<<blocks, 256, 0, c->stream>>>(P, nk ? sk->x : nullptr, nk ? sk->y : nullptr, nk ? sk->z : nullptr, nk,
-                                                   nn ? sn->x : nullptr, nn ? sn->y : nullptr, nn ? sn->z : nullptr, nn, keys, counts, occ);
-        if ((rc = check_launch(c, "k_bin_count")) != PM_OK) return rc;
-        k_bin_scan_local<<<nscan, 256, 0, c->stream>>>(counts, nkeys, sums);
-        if ((rc = check_launch(c, "k_bin_scan_local")) != PM_OK) return rc;
-        k_bin_scan_sums<<<1, 1024, 0, c->stream>>>(sums, nscan);
-        if ((rc = check_launch(c, "k_bin_scan_sums")) != PM_OK) return rc;
-        k_bin_fill<<<blocks, 256, 0, c->stream>>>(keys, counts, sums, perm, np, nk);
-        if ((rc = check_launch(c, "k_bin_fill")) != PM_OK) return rc;
-        tick(c, PM_K_BIN, 1);
+        if (np > 0) {
+            const unsigned blocks = (unsigned)((np + 255) / 256);
+            tick(c, PM_K_BIN, 0);
+            k_bin_count<<<blocks, 256, 0, c->stream>>>(P, nk ? sk->x : nullptr, nk ? sk->y : nullptr, nk ? sk->z : nullptr, nk,
+                                                       nn ? sn->x : nullptr, nn ? sn->y : nullptr, nn ? sn->z : nullptr, nn, keys, counts, occ);
+            if ((rc = check_launch(c, "k_bin_count")) != PM_OK) return rc;
+            k_bin_scan_local<<<nscan, 256, 0, c->stream>>>(counts, nkeys, sums);
+            if ((rc = check_launch(c, "k_bin_scan_local")) != PM_OK) return rc;
+            k_bin_scan_sums<<<1, 1024, 0, c->stream>>>(sums, nscan);
+            if ((rc = check_launch(c, "k_bin_scan_sums")) != PM_OK) return rc;
+            k_bin_fill<<<blocks, 256, 0, c->stream>>>(keys, counts, sums, perm, np, nk);
+            if ((rc = check_launch(c, "k_bin_fill")) != PM_OK) return rc;
+            tick(c, PM_K_BIN, 1);
+        }
     }
     // a0: reset (L59 "all cells initialized to zero").  The tiles this step's particles can add into are marked live (from the
     // bin occupancy) and zeroed; all others are stale and taken as zeros by the readers (pm_tiles.cuh).
-    if (np == 0) PM_CUDA(c, cudaMemsetAsync(c->tile_live, 0, (size_t)c->ntiles, c->stream));
-    if (np > 0) {
+    if (np == 0 && !P.zopen) PM_CUDA(c, cudaMemsetAsync(c->tile_live, 0, (size_t)c->ntiles, c->stream));
+    if (np > 0 || P.zopen) {
         const Tiles T = tiles_of(c);
         tick(c, PM_K_ZERO, 0);
         k_tiles_mark<<<(unsigned)((c->ntiles + 255) / 256), 256, 0, c->stream>>>(P, T, occ, (int)c->ntiles, nk > 0, nn > 0, live);
@@ -909,6 +937,7 @@ extern "C" int pm_deposit(pm_ctx *c, const pm_state *st, const pm_sinks *sk, con
     c->n_sinks_dep = nk; c->n_sne_dep = nn; c->dt = dt;
     c->ever_deposited = true;
     c->grav_in_ch1 = false;
+    c->slab_packed = false;
     c->stage = ST_DEPOSITED;
     c->buffer_valid = false;              // unfolded until pm_fold_ghosts
     return PM_OK;
@@ -928,12 +957,14 @@ extern "C" int pm_fold_ghosts(pm_ctx *c) {
     const unsigned blocks = (unsigned)((n_edge + 255) / 256);
     tick(c, PM_K_FOLD, 0);
     const Tiles T = tiles_of(c);
+    if (P.zopen && !c->slab_packed) PM_FAIL(c, PM_EORDER, "pm_fold_ghosts (z slab): pm_slab_pack and the exchange of the slabs come first");
+    const double *rlo = P.zopen ? c->slab_mem + 2 * c->slab_elems : nullptr, *rhi = P.zopen ? c->slab_mem + 3 * c->slab_elems : nullptr;
     if (c->repro) {
-        if (W == 2) k_fold_ghosts<2, kReproChannels, true><<<blocks, 256, 0, c->stream>>>(P, c->buf, T, n_edge, n_z, n_y);
-        else k_fold_ghosts<1, kReproChannels, true><<<blocks, 256, 0, c->stream>>>(P, c->buf, T, n_edge, n_z, n_y);
+        if (W == 2) k_fold_ghosts<2, kReproChannels, true><<<blocks, 256, 0, c->stream>>>(P, c->buf, T, n_edge, n_z, n_y, rlo, rhi);
+        else k_fold_ghosts<1, kReproChannels, true><<<blocks, 256, 0, c->stream>>>(P, c->buf, T, n_edge, n_z, n_y, rlo, rhi);
     } else {
-        if (W == 2) k_fold_ghosts<2, kBufChannels, true><<<blocks, 256, 0, c->stream>>>(P, c->buf, T, n_edge, n_z, n_y);
-        else k_fold_ghosts<1, kBufChannels, true><<<blocks, 256, 0, c->stream>>>(P, c->buf, T, n_edge, n_z, n_y);
+        if (W == 2) k_fold_ghosts<2, kBufChannels, true><<<blocks, 256, 0, c->stream>>>(P, c->buf, T, n_edge, n_z, n_y, rlo, rhi);
+        else k_fold_ghosts<1, kBufChannels, true><<<blocks, 256, 0, c->stream>>>(P, c->buf, T, n_edge, n_z, n_y, rlo, rhi);
     }
     int rc = check_launch(c, "k_fold_ghosts");
     tick(c, PM_K_FOLD, 1);
@@ -1004,6 +1035,50 @@ extern "C" int pm_return_to_particles(pm_ctx *c, pm_sinks *sk) {
     return PM_OK;
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// (f)4: z-slab decomposition (pm_slab.cuh)
+// ---------------------------------------------------------------------------------------------------------------
+extern "C" int pm_slab_describe(pm_ctx *c, pm_slab_desc *d) {
+    if (!c || !d) return PM_EINVAL;
+    if (!c->P.zopen) PM_FAIL(c, PM_EINVAL, "pm_slab_describe: the ctx was not created with z_slab = 1");
+    std::memset(d, 0, sizeof(*d));
+    const DevP &P = c->P;
+    d->buf_bytes = c->slab_elems * (int64_t)sizeof(double);
+    d->buf_send_lo = c->slab_mem; d->buf_send_hi = c->slab_mem + c->slab_elems;
+    d->buf_recv_lo = c->slab_mem + 2 * c->slab_elems; d->buf_recv_hi = c->slab_mem + 3 * c->slab_elems;
+    const long long plane = (long long)P.ny * P.nx, gp = (long long)P.g * plane;
+    if (c->ret) {      // planes of the return mesh, in units of records of kRetWords doubles
+        d->ret_bytes = gp * kRetWords * (int64_t)sizeof(double);
+        d->ret_recv_lo = c->ret;                                          // ghost planes k in [-g, 0)
+        d->ret_send_lo = c->ret + kRetWords * gp;                         // owned planes k in [0, g): the lower neighbour's high ghosts
+        d->ret_send_hi = c->ret + kRetWords * (long long)P.nz * plane;    // owned planes k in [nz - g, nz): the upper neighbour's low ghosts
+        d->ret_recv_hi = c->ret + kRetWords * ((long long)P.nz * plane + gp);   // ghost planes k in [nz, nz + g)
+    }
+    if (c->ret_tr) {
+        d->rtr_bytes = gp * (int64_t)sizeof(double);
+        d->rtr_recv_lo = c->ret_tr; d->rtr_send_lo = c->ret_tr + gp;
+        d->rtr_send_hi = c->ret_tr + (long long)P.nz * plane; d->rtr_recv_hi = c->ret_tr + (long long)P.nz * plane + gp;
+    }
+    d->state_ghost_planes = P.g;
+    return PM_OK;
+}
+
+extern "C" int pm_slab_pack(pm_ctx *c) {
+    if (!c) return PM_EINVAL;
+    if (!c->P.zopen) PM_FAIL(c, PM_EINVAL, "pm_slab_pack: the ctx was not created with z_slab = 1");
+    if (c->stage != ST_DEPOSITED) PM_FAIL(c, PM_EORDER, "pm_slab_pack must follow pm_deposit");
+    PM_CUDA(c, cudaSetDevice(c->device));
+    const DevP &P = c->P;
+    const long long n = 2ll * P.g * P.pk;
+    const unsigned blocks = (unsigned)((n + 255) / 256);
+    if (c->repro) k_slab_pack<kReproChannels><<<blocks, 256, 0, c->stream>>>(P, c->buf, tiles_of(c), c->slab_mem, c->slab_mem + c->slab_elems);
+    else k_slab_pack<kBufChannels><<<blocks, 256, 0, c->stream>>>(P, c->buf, tiles_of(c), c->slab_mem, c->slab_mem + c->slab_elems);
+    int rc = check_launch(c, "k_slab_pack");
+    if (rc != PM_OK) return rc;
+    c->slab_packed = true;
+    return PM_OK;
+}
+
 extern "C" int pm_create_sinks(pm_ctx *c, pm_state *st, int64_t max_new, double *x, double *y, double *z, double *vx,
                                double *vy, double *vz, double *m, int64_t *n_new) {
     if (!c) return PM_EINVAL;
@@ -1066,8 +1141,8 @@ static int fold_gravity_channel(pm_ctx *c, double *gbuf) {
     const long long n_x = (long long)(P.nz - g2) * (P.ny - g2) * g2 / W;
     const long long n_edge = n_z + n_y + n_x;
     const unsigned blocks = (unsigned)((n_edge + 255) / 256);
-    if (W == 2) k_fold_ghosts<2, 1, false><<<blocks, 256, 0, c->stream>>>(P, gbuf, tiles_of(c), n_edge, n_z, n_y);
-    else k_fold_ghosts<1, 1, false><<<blocks, 256, 0, c->stream>>>(P, gbuf, tiles_of(c), n_edge, n_z, n_y);
+    if (W == 2) k_fold_ghosts<2, 1, false><<<blocks, 256, 0, c->stream>>>(P, gbuf, tiles_of(c), n_edge, n_z, n_y, nullptr, nullptr);
+    else k_fold_ghosts<1, 1, false><<<blocks, 256, 0, c->stream>>>(P, gbuf, tiles_of(c), n_edge, n_z, n_y, nullptr, nullptr);
     return check_launch(c, "k_fold_ghosts<1 channel>");
 }
 
@@ -1115,6 +1190,7 @@ extern "C" int pm_gravity_deposit(pm_ctx *c, const double *rho_gas, int64_t n, c
     if (!c) return PM_EINVAL;
     if (n < 0 || !rho_tot) PM_FAIL(c, PM_EINVAL, "pm_gravity_deposit: null output or negative particle count");
     if (n > 0 && !(x && y && z && m)) PM_FAIL(c, PM_EINVAL, "pm_gravity_deposit: null particle array");
+    if (c->P.zopen) PM_FAIL(c, PM_EINVAL, "pm_gravity_deposit: not available on a z slab (the gravity calls are single-domain)");
     if (c->stage == ST_DEPOSITED || c->stage == ST_FOLDED)
         PM_FAIL(c, PM_EORDER, "pm_gravity_deposit: the buffer mesh is in use (finish the exchange step first)");
     PM_CUDA(c, cudaSetDevice(c->device));
@@ -1151,6 +1227,7 @@ extern "C" int pm_gravity_kick(pm_ctx *c, const double *gx, const double *gy, co
     if (has_v && !(vx && vy && vz)) PM_FAIL(c, PM_EINVAL, "pm_gravity_kick: give all of vx, vy, vz or none");
     if (has_a && !(ax && ay && az)) PM_FAIL(c, PM_EINVAL, "pm_gravity_kick: give all of ax, ay, az or none");
     if (!has_v && !has_a) PM_FAIL(c, PM_EINVAL, "pm_gravity_kick: nothing to write (no velocities, no acceleration output)");
+    if (c->P.zopen) PM_FAIL(c, PM_EINVAL, "pm_gravity_kick: not available on a z slab (the gravity calls are single-domain)");
     PM_CUDA(c, cudaSetDevice(c->device));
     const int *perm;
     int rc;
@@ -1188,6 +1265,7 @@ extern "C" int pm_check(pm_ctx *c) {
 extern "C" int pm_step_host(pm_ctx *c, pm_state *hs, pm_sinks *hk, const pm_sne *hn, double dt) {
     if (!c) return PM_EINVAL;
     if (!state_ok(hs)) PM_FAIL(c, PM_EINVAL, "pm_step_host: null state pointer");
+    if (c->P.zopen) PM_FAIL(c, PM_EINVAL, "pm_step_host: not available on a z slab (the exchanges between the calls are the caller's)");
     PM_CUDA(c, cudaSetDevice(c->device));
     const long long N = c->P.N, nk = hk ? hk->n : 0, nn = hn ? hn->n : 0;
     int rc;
@@ -1265,9 +1343,24 @@ extern "C" int pm_debug_buffer(pm_ctx *c, int channel, const double **dev_ptr, i
     return PM_OK;
 }
 
+extern "C" int pm_debug_tile_counts(pm_ctx *c, int64_t *n_tiles, int64_t *live_k, int64_t *live_n) {
+    if (!c || !n_tiles || !live_k || !live_n) return PM_EINVAL;
+    PM_CUDA(c, cudaSetDevice(c->device));
+    unsigned char *h = new (std::nothrow) unsigned char[(size_t)c->ntiles];
+    if (!h) return PM_ENOMEM;
+    cudaError_t e = cudaMemcpyAsync(h, c->tile_live, (size_t)c->ntiles, cudaMemcpyDeviceToHost, c->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+    if (e != cudaSuccess) { delete[] h; snprintf(c->msg, sizeof(c->msg), "pm_debug_tile_counts: %s", cudaGetErrorString(e)); return PM_ECUDA; }
+    int64_t k = 0, n = 0;
+    for (long long t = 0; t < c->ntiles; ++t) { k += (h[t] & kLiveK) ? 1 : 0; n += (h[t] & kLiveN) ? 1 : 0; }
+    delete[] h;
+    *n_tiles = c->ntiles; *live_k = k; *live_n = n;
+    return PM_OK;
+}
+
 extern "C" int pm_debug_return_mesh(pm_ctx *c, int word, const double **dev_ptr) {
     if (!c || !dev_ptr || word < 0 || word >= kRetWords || !c->ret) return PM_EINVAL;
-    *dev_ptr = c->ret + word;          // record of cell q at 4 q: stride kRetWords between cells
+    *dev_ptr = c->ret + (long long)kRetWords * c->P.zoff + word;   // record of OWNED cell q at 4 q (behind the ghost planes of a slab)
     return PM_OK;
 }
 

@@ -25,11 +25,11 @@ __global__ void __launch_bounds__(256) k_create_find(const DevP P, const DevStat
     const int lane = threadIdx.x & 31;
     const bool valid = c_raw < P.N;
     const long long c = valid ? c_raw : 0;
-    const double rho = U.rho[c];
+    const double rho = U.rho[c + P.zoff];             // zoff: ghost planes of a z slab in front of the owned cells
     const int i = (int)(c % P.nx);
     const long long row = c / P.nx;
     const int j = (int)(row % P.ny), k = (int)(row / P.ny);
-    bool cand = valid && rho > truelove_rho(P, rho, U.eint[c]);                       // (i)   above rho_Tr
+    bool cand = valid && rho > truelove_rho(P, rho, U.eint[c + P.zoff]);              // (i)   above rho_Tr
     // (iii) inside another sink's kernel (L177); a tile no sink touched in the last step is stale and stands for zeros
     if (cand && buf0 && (T.live[tile_index(P, i, j, k)] & kLiveK) && buf0[ghost_index(P, i, j, k)] != 0.0) cand = false;
     unsigned todo = __ballot_sync(0xffffffffu, cand);
@@ -88,10 +88,11 @@ __global__ void __launch_bounds__(128) k_create_apply(const DevP P, const DevSta
                                                       double *__restrict__ m) {
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= n) return;
-    const long long c = cells[s];
-    const int i = (int)(c % P.nx);
-    const long long row = c / P.nx;
+    const long long c0 = cells[s];
+    const int i = (int)(c0 % P.nx);
+    const long long row = c0 / P.nx;
     const int j = (int)(row % P.ny), k = (int)(row / P.ny);
+    const long long c = c0 + P.zoff;
     const double rho = U.rho[c];
     const double rtr = truelove_rho(P, rho, U.eint[c]);
     const double keep = rtr / rho;                       // same velocity and specific energies (L183)

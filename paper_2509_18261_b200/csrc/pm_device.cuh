@@ -42,6 +42,12 @@ struct DevP {
     int ntile;              // bin keys per particle kind: super-blocks x tiles per super-block
     int ntx, nty, ntz;      // buffer-mesh tiles of 8^3 cells per axis, ghost tiles included (pm_tiles.cuh): tile t holds the
                             // cells [8 (t - 1), 8 t) of owned coordinates
+    // z-slab decomposition (pm_slab.cuh): zopen = 1 means this ctx holds one slab of a domain cut along z.  The
+    // caller's state arrays and the return mesh then carry g ghost planes below and above the nz owned ones (filled by halo
+    // exchanges), so a stencil that leaves the slab in z reads the neighbour's cells in place instead of wrapping; the buffer
+    // mesh's z ghost planes travel to the neighbours (Eq. 3 as the paper states it, L67-71) instead of being folded in place.
+    int zopen;
+    int zoff;               // cells of the state arrays before owned cell (0,0,0): g ny nx when zopen, else 0
 };
 
 struct DevState { double *rho, *mx, *my, *mz, *etot, *eint; };
@@ -73,8 +79,11 @@ __device__ __forceinline__ double dist2(double ddx, double ddy, double ddz) { re
 // periodic wrap of an index known to lie in [-n, 2n)
 __device__ __forceinline__ int wrap1(int i, int n) { return i < 0 ? i + n : (i >= n ? i - n : i); }
 
+// index into a STATE array (or the return mesh) of unwrapped cell (i, j, k): periodic wrap, except along z of a slab, where
+// the array holds the neighbours' planes k in [-g, 0) and [nz, nz + g) itself
+__device__ __forceinline__ int state_k(const DevP &P, int k) { return P.zopen ? k + P.g : wrap1(k, P.nz); }
 __device__ __forceinline__ long long owned_index(const DevP &P, int i, int j, int k) {
-    return ((long long)wrap1(k, P.nz) * P.ny + wrap1(j, P.ny)) * P.nx + wrap1(i, P.nx);
+    return ((long long)state_k(P, k) * P.ny + wrap1(j, P.ny)) * P.nx + wrap1(i, P.nx);
 }
 // ghosted index of UNWRAPPED cell (i,j,k), each in [-g, n+g)
 __device__ __forceinline__ long long ghost_index(const DevP &P, int i, int j, int k) {

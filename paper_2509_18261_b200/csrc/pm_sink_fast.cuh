@@ -36,7 +36,7 @@ __device__ __forceinline__ int sink_member_list_g4(const DevP &P, SinkWarpSmem &
         const int u = h - 4 + c;
         const double d = cell_centre(x0, u, P.dx) - ps;
         sm.d2[ax][c] = d * d;
-        const int wq = wrap1(u, n);
+        const int wq = (ax == 2) ? state_k(P, u) : wrap1(u, n);
         sm.off[ax][c] = ax == 0 ? wq : (ax == 1 ? wq * P.nx : wq * P.nx * P.ny);
         if (ax > 0) sm.goff[ax - 1][c] = (int)((u + P.g) * (ax == 1 ? P.pj : P.pk));
     }

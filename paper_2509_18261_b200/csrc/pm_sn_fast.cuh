@@ -34,6 +34,12 @@ struct __align__(16) SnWarpSmem {
     unsigned char cnt[448];         // omega counts (0..64) by packed code
 };
 
+// cnt += (s <= t), as one DSETP and one predicated add (the C form compiles to a select and costs a third instruction:
+// 866 -> 590 warp instructions per particle in the 64-sample tests, the largest single item of the kernel)
+__device__ __forceinline__ void count_le(int &cnt, const double s, const double t) {
+    asm("{ .reg .pred p; setp.le.f64 p, %1, %2; @p add.s32 %0, %0, 1; }" : "+r"(cnt) : "d"(s), "d"(t));
+}
+
 __device__ __forceinline__ unsigned lanemask_lt() {
     unsigned m;
     asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m));
@@ -94,7 +100,7 @@ __device__ __forceinline__ void sn_deposit_one(const DevP &P, const DevState &U,
         const int n = ax == 0 ? P.nx : (ax == 1 ? P.ny : P.nz);
         const int u = h - 3 + c;                                  // unwrapped cell index
         sm.dc[ax][c] = cell_centre(x0, u, P.dx) - ps;
-        const int wq = wrap1(u, n);
+        const int wq = (ax == 2) ? state_k(P, u) : wrap1(u, n);      // z of a slab: the state holds the neighbour's planes itself
         sm.off[ax][c] = ax == 0 ? wq : (ax == 1 ? wq * P.nx : wq * P.nx * P.ny);
     }
     __syncwarp();
@@ -160,7 +166,7 @@ __device__ __forceinline__ void sn_deposit_one(const DevP &P, const DevState &U,
 #pragma unroll
             for (int qy = 0; qy < 4; ++qy) {
                 const double sy = zv[qz] + yv[qy];
-                cnt += (sy <= t0) + (sy <= t1) + (sy <= t2) + (sy <= t3);
+                count_le(cnt, sy, t0); count_le(cnt, sy, t1); count_le(cnt, sy, t2); count_le(cnt, sy, t3);
             }
         sm.cnt[pc] = (unsigned char)cnt;
     }
@@ -201,9 +207,9 @@ __device__ __forceinline__ void sn_deposit_one(const DevP &P, const DevState &U,
     double m_gas = 0.0, px = 0.0, py = 0.0, pz = 0.0, v_snr = 0.0;
     // owned index of a box cell: plain strides when the box does not cross the periodic seam (warp-uniform), else the
     // wrapped per-axis tables
-    const bool inner = ih >= 3 && ih + 3 < P.nx && jh >= 3 && jh + 3 < P.ny && kh >= 3 && kh + 3 < P.nz;
+    const bool inner = ih >= 3 && ih + 3 < P.nx && jh >= 3 && jh + 3 < P.ny && (P.zopen || (kh >= 3 && kh + 3 < P.nz));
     const int nxny = P.nx * P.ny;
-    const int qb = ((kh - 3) * P.ny + (jh - 3)) * P.nx + (ih - 3);
+    const int qb = ((kh - 3) * P.ny + (jh - 3)) * P.nx + (ih - 3) + P.zoff;
     // batches of kSnGatherBatch list entries per lane: all their loads are in flight together (the gather is latency-bound)
 #pragma unroll 1
     for (int base = lane; base < na; base += 32 * kSnGatherBatch) {

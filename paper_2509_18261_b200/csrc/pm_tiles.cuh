@@ -72,13 +72,15 @@ __device__ __forceinline__ void tile_zero(const DevP &P, double *__restrict__ bu
 // Host-cell ranges (one axis) from which a particle with kernel half-width g reaches tile t: directly, or through the fold --
 // the tile's owned cells within g of a face also receive what was added to their ghost images one box length away (Eq. 3).
 // Writes up to three inclusive ranges of BIN indices (host cell >> 3) into lo[] / hi[]; returns their number.
-__device__ __forceinline__ int tile_host_bins(int t, int n, int g, int lo[3], int hi[3]) {
+// open: the axis is not periodic inside this ctx (z of a slab): no images.
+__device__ __forceinline__ int tile_host_bins(int t, int n, int g, int lo[3], int hi[3], bool open = false) {
     const int a = 8 * (t - 1), b = 8 * t - 1;              // the tile's cells
     int cnt = 0;
 #pragma unroll
     for (int s = -1; s <= 1; ++s) {                         // image shift s n: cells a + s n .. b + s n
         int ca = a, cb = b;
         if (s != 0) {                                       // only owned cells have images, and an image lies in [-g, n + g)
+            if (open) continue;
             const int oa = max(a, 0), ob = min(b, n - 1);
             if (oa > ob) continue;
             ca = max(oa + s * n, -g); cb = min(ob + s * n, n + g - 1);
@@ -107,7 +109,7 @@ __global__ void __launch_bounds__(256) k_tiles_mark(const DevP P, const Tiles T,
             const int g = grp == 0 ? P.gs : P.gn;
             int xl[3], xh[3], yl[3], yh[3], zl[3], zh[3];
             const int cx = tile_host_bins(tx, P.nx, g, xl, xh), cy = tile_host_bins(ty, P.ny, g, yl, yh),
-                      cz = tile_host_bins(tz, P.nz, g, zl, zh);
+                      cz = tile_host_bins(tz, P.nz, g, zl, zh, P.zopen != 0);
             const unsigned char *o = occ + (grp == 0 ? 0 : P.ntile);
             bool hit = false;
             for (int c = 0; c < cz && !hit; ++c)
@@ -118,6 +120,12 @@ __global__ void __launch_bounds__(256) k_tiles_mark(const DevP P, const Tiles T,
                                 for (int bx = xl[a]; bx <= xh[a]; ++bx)
                                     if (o[bin_key(P, bx << 3, by << 3, bz << 3)]) { hit = true; break; }
             any[grp] = hit;
+        }
+        // z slab: the owned cells within g of a z face receive what the NEIGHBOUR's particles added to its ghost planes; what
+        // those are is not known here, so these tiles are live in every group the run uses
+        if (P.zopen && 8 * tz > 0 && 8 * (tz - 1) < P.nz && (8 * (tz - 1) < P.g || 8 * tz > P.nz - P.g)) {
+            any[0] = any[0] || P.gs > 0;
+            any[1] = any[1] || P.gn > 0;
         }
         T.live[t] = (unsigned char)((any[0] ? kLiveK : 0u) | (any[1] ? kLiveN : 0u));
     }

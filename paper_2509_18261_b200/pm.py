@@ -8,6 +8,7 @@ from __future__ import annotations
 
 import ctypes as C
 import glob
+import math
 import os
 import subprocess
 
@@ -24,7 +25,7 @@ KERNEL_GROUPS = ("bin", "zero", "sinks", "sne", "fold", "apply", "return")
 STATUS_NAMES = {0: "PM_OK", -1: "PM_EINVAL", -2: "PM_ENOMEM", -3: "PM_ECUDA", -4: "PM_EORDER", -5: "PM_EDOMAIN"}
 
 EXPORTS = ["pm_create", "pm_deposit", "pm_fold_ghosts", "pm_apply_limited", "pm_return_to_particles", "pm_check",
-           "pm_step_host", "pm_destroy", "pm_last_error", "pm_launch_count", "pm_kernel_times", "pm_probe_red_f64", "pm_set_repro_margin", "pm_create_sinks", "pm_gravity_deposit", "pm_gravity_kick", "pm_drift", "pm_debug_round_buffers", "pm_debug_buffer",
+           "pm_step_host", "pm_destroy", "pm_last_error", "pm_launch_count", "pm_kernel_times", "pm_probe_red_f64", "pm_set_repro_margin", "pm_create_sinks", "pm_gravity_deposit", "pm_gravity_kick", "pm_drift", "pm_slab_describe", "pm_slab_pack", "pm_debug_round_buffers", "pm_debug_buffer", "pm_debug_tile_counts",
            "pm_debug_return_mesh", "pm_debug_lambda", "pm_debug_sink_scalars", "pm_debug_sn_scalars",
            "pm_debug_stencil"]
 
@@ -44,7 +45,15 @@ class PmParams(C.Structure):
         ("sn_psnr_coeff", C.c_double), ("sn_psnr_exp", C.c_double),
         ("sn_mu_h", C.c_double), ("sn_nh_unit", C.c_double),
         ("sn_eint_theta", C.c_double), ("truelove_J", C.c_double),
+        ("z_slab", C.c_int32), ("pad_", C.c_int32),
     ]
+
+
+class PmSlabDesc(C.Structure):
+    _fields_ = ([(f, C.c_void_p) for f in ("buf_send_lo", "buf_send_hi", "buf_recv_lo", "buf_recv_hi")] + [("buf_bytes", C.c_int64)] +
+                [(f, C.c_void_p) for f in ("ret_send_lo", "ret_send_hi", "ret_recv_lo", "ret_recv_hi")] + [("ret_bytes", C.c_int64)] +
+                [(f, C.c_void_p) for f in ("rtr_send_lo", "rtr_send_hi", "rtr_recv_lo", "rtr_recv_hi")] + [("rtr_bytes", C.c_int64)] +
+                [("state_ghost_planes", C.c_int32), ("pad_", C.c_int32)])
 
 
 class PmState(C.Structure):
@@ -111,6 +120,9 @@ def lib():
         L.pm_probe_red_f64.argtypes = [vp, C.c_int64, C.c_int32, C.POINTER(C.c_double)]
         L.pm_debug_round_buffers.argtypes = [vp]
         L.pm_debug_buffer.argtypes = [vp, C.c_int, C.POINTER(vp), i64p, i64p, i32p]
+        L.pm_debug_tile_counts.argtypes = [vp, i64p, i64p, i64p]
+        L.pm_slab_describe.argtypes = [vp, C.POINTER(PmSlabDesc)]
+        L.pm_slab_pack.argtypes = [vp]
         L.pm_debug_return_mesh.argtypes = [vp, C.c_int, C.POINTER(vp)]
         L.pm_debug_lambda.argtypes = [vp, C.POINTER(vp)]
         L.pm_debug_sink_scalars.argtypes = [vp, C.POINTER(vp), i64p]
@@ -132,6 +144,10 @@ def make_params(p: dict, flags: int = 0) -> PmParams:
             o.x0[0], o.x0[1], o.x0[2] = (float(v) for v in p["x0"])
         elif k == "truelove_J":
             o.truelove_J = float(p.get("truelove_J", 0.0))
+        elif k == "z_slab":
+            o.z_slab = int(p.get("z_slab", 0))
+        elif k == "pad_":
+            o.pad_ = 0
         else:
             setattr(o, k, p[k])
     return o
@@ -256,7 +272,30 @@ class Context:
             raise PmError(rc, where, self.L.pm_last_error(self.h).decode())
 
     def _cells(self):
-        return self.params["nx"] * self.params["ny"] * self.params["nz"]
+        """Length of a state array: owned cells, plus g ghost planes below and above on a z slab."""
+        p = self.params
+        nz = p["nz"] + (2 * self.ghost_width() if p.get("z_slab", 0) else 0)
+        return p["nx"] * p["ny"] * nz
+
+    def ghost_width(self) -> int:
+        p = self.params
+        return max(math.ceil(p["rk_sink"] / p["dx"]) if p["rk_sink"] > 0 else 0, math.ceil(p["rk_sn"] / p["dx"]) if p["rk_sn"] > 0 else 0)
+
+    # ---- z-slab decomposition (SURVEY 8(f)4) -------------------------------------------------------
+    def pm_slab_pack(self):
+        self._chk(self.L.pm_slab_pack(self.h), "pm_slab_pack")
+
+    def pm_slab_describe(self) -> dict:
+        """Device tensors (views of ctx-owned memory) of the slab messages: buf / ret / rtr x send_lo, send_hi, recv_lo, recv_hi."""
+        d = PmSlabDesc()
+        self._chk(self.L.pm_slab_describe(self.h, C.byref(d)), "pm_slab_describe")
+        out = {"state_ghost_planes": int(d.state_ghost_planes)}
+        for grp in ("buf", "ret", "rtr"):
+            nbytes = getattr(d, grp + "_bytes")
+            for side in ("send_lo", "send_hi", "recv_lo", "recv_hi"):
+                ptr = getattr(d, f"{grp}_{side}")
+                out[f"{grp}_{side}"] = _from_ptr(ptr, nbytes // 8, self.device) if (ptr and nbytes) else None
+        return out
 
     def _on_device(self, *objs):
         for o in objs:
@@ -388,6 +427,12 @@ class Context:
         ox = origin.value - (gz * d[1] + gz) * d[2]
         owned = t[gz:gz + nz, gz:gz + ny, ox:ox + nx]
         return t, owned, gz, ox
+
+    def debug_tile_counts(self):
+        """(tiles of the buffer mesh, tiles live in group K, tiles live in group N) after the last pm_deposit."""
+        n, k, m = C.c_int64(), C.c_int64(), C.c_int64()
+        self._chk(self.L.pm_debug_tile_counts(self.h, C.byref(n), C.byref(k), C.byref(m)), "pm_debug_tile_counts")
+        return int(n.value), int(k.value), int(m.value)
 
     def debug_return_mesh(self, word: int):
         ptr = C.c_void_p()

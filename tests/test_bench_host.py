@@ -48,11 +48,16 @@ def test_single_rank_is_identity():
 
 
 def test_algorithmic_bytes_dense_limits():
-    """With every sector touched the per-kernel figures reduce to SURVEY.md 8(d): apply 176 B/cell, zero 48 B per buffer cell."""
+    """With every cell touched and every tile live the per-kernel figures are SURVEY.md 8(d)'s: apply 176 B/cell, reset +
+    write-back 48 B per buffer cell, fold 3 x 48 B per ghost cell, gathers 40 / 32 B per cell; the deposit kernels carry no
+    write-back (8(d) books it once, with the reset)."""
     N, Nb = 512 ** 3, 520 ** 3
     b = bench.algorithmic_bytes(N, Nb, 10 ** 5, 9 * 10 ** 5, 1.0, 1.0, 1.0)
     assert b["apply"] == 176.0 * N
     assert b["zero"] == 48.0 * Nb
     assert b["fold"] == 3 * 48.0 * (Nb - N)
-    b0 = bench.algorithmic_bytes(N, Nb, 0, 0, 0.0, 0.0, 0.0)
-    assert b0["apply"] == 48.0 * N and b0["sne"] == 0.0 and b0["sinks"] == 0.0
+    assert b["sinks"] == 40.0 * N + 80.0 * 10 ** 5 and b["sne"] == 32.0 * N + 64.0 * 9 * 10 ** 5
+    b0 = bench.algorithmic_bytes(N, Nb, 0, 0, 0.0, 0.0, 0.0, 0.0, 0.0)
+    assert b0["apply"] == 0.0 and b0["sne"] == 0.0 and b0["sinks"] == 0.0 and b0["zero"] == 0.0
+    # SN deposit at config 5's probed cell fraction (SURVEY 8(d): T_SN ~ 0.48): ~2.1 GB, not the 6.4 GB of round 1's line
+    assert 2.0e9 < bench.algorithmic_bytes(N, Nb, 10 ** 5, 9 * 10 ** 5, 0.55, 0.12, 0.48)["sne"] < 2.2e9

@@ -103,3 +103,36 @@ def test_creation_full_size_properties():
         dz, dy, dx = np.meshgrid(np.arange(-4, 5), np.arange(-4, 5), np.arange(-4, 5), indexing="ij")
         inside = (dz * dz + dy * dy + dx * dx <= 16) & ((dz != 0) | (dy != 0) | (dx != 0))
         assert np.all(nb[inside] < rho0[k, j, i])
+
+
+def test_creation_after_a_gravity_deposit_still_sees_the_retained_buffer():
+    """L107-109 puts the gravity deposit before the step's accretion, and sink creation after it; a pm_gravity_deposit between
+    a step and pm_create_sinks must not switch criterion (iii) off: gravity works in buffer channel 1, the retained
+    accretion channel 0 stays.  An unfolded deposit is refused."""
+    w = inputs.scaled_mixed(40, 200, seed_index=5, n_clusters=2)
+    w.params["truelove_J"] = 0.8
+    g = parity.GpuRun(w)
+    o = parity.make_oracle(w)
+    o.step(w.dt)
+    g.step()
+    # After a step with the Truelove terms on, no cell inside a sink's kernel is left above rho_Tr (Eq. 14: "the density falls
+    # to rho_Tr"), so criterion (iii) has nothing to exclude by itself.  Plant a peak inside a kernel: a cell whose accretion
+    # channel is non-zero gets 100 x the maximum density -- a strict local maximum far above rho_Tr that ONLY (iii) can stop.
+    inside = np.flatnonzero(o.A[0] != 0.0)
+    c_star = int(inside[len(inside) // 2])
+    o.state.rho.reshape(-1)[c_star] = 100.0 * o.state.rho.max()
+    g.state = pm.DeviceState.from_host(o.state, g.dev)
+    gw = inputs.gravity_workload(40, 500, seed_index=13)
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(g.dev)
+    rho_tot = torch.empty((40, 40, 40), dtype=torch.float64, device=g.dev)
+    g.ctx.pm_gravity_deposit(None, t(gw.x), t(gw.y), t(gw.z), t(gw.m), rho_tot)
+    probe = po.Oracle(w.params, o.state.copy(), w.sinks.copy(), inputs.empty_sne())
+    n_without, made = probe.create_sinks(4096, use_buffer=False)
+    assert c_star in made["cells"]                               # without the retained buffer the planted peak creates a sink
+    n_with = _compare(g, o, 4096)                                # GPU (after the gravity deposit) == oracle WITH the retained buffer
+    assert n_with < n_without
+    # deposit without fold: the retained buffer is neither the old nor the new one
+    g.ctx.pm_deposit(g.state, g.sinks, g.sne, w.dt)
+    with pytest.raises(pm.PmError) as e:
+        g.ctx.pm_create_sinks(g.state, 16)
+    assert e.value.status == pm.PM_EORDER

@@ -296,3 +296,48 @@ def test_bin_ordered_path_above_the_sort_threshold():
     for c in range(3):
         assert np.array_equal(a[c].cpu().numpy(), go.gravity_interpolate(p, w.g[c], *pos))
     ctx.close()
+
+
+def test_kick_between_deposit_and_return_keeps_the_sink_order():
+    """ADVICE r1 / VERDICT r1: a pm_gravity_kick with n >= 65536 particles between pm_deposit and pm_return_to_particles used
+    to rebuild its particle order in the memory Step 4 reads the sink order from.  Gravity has its own scratch now: deposit ->
+    kick -> fold -> kick -> apply -> kick -> return must give the oracle's sinks (m, dm strictly; v within the reorder bound),
+    conserve mass, and interpolate exactly as a kick outside a step does."""
+    from tests import parity
+    w = inputs.scaled_mixed(64, 3000, seed_index=5)
+    gw = inputs.gravity_workload(64, 70_000, seed_index=12)
+    g = parity.GpuRun(w)
+    o = parity.make_oracle(w)
+    x, y, z = dev(gw.x), dev(gw.y), dev(gw.z)
+    gx, gy, gz = (dev(a) for a in gw.g)
+    acc = [[torch.empty_like(x) for _ in range(3)] for _ in range(3)]
+    m0, _ = g.totals()
+    g.ctx.pm_deposit(g.state, g.sinks, g.sne, w.dt)
+    g.ctx.pm_gravity_kick(gx, gy, gz, x, y, z, a=acc[0])
+    g.ctx.pm_fold_ghosts()
+    g.ctx.pm_gravity_kick(gx, gy, gz, x, y, z, a=acc[1])
+    g.ctx.pm_apply_limited(g.state)
+    g.ctx.pm_gravity_kick(gx, gy, gz, x, y, z, a=acc[2])
+    g.ctx.pm_return_to_particles(g.sinks)
+    g.ctx.pm_check()
+    o.step(w.dt)
+    parity.compare_sinks(g, o)
+    m1, _ = g.totals()
+    assert abs((m1 - m0) - float(w.sne.m_ej.sum())) <= 1e-13 * abs(m1)
+    for c in range(3):
+        ref = go.gravity_interpolate(gw.params, gw.g[c], gw.x, gw.y, gw.z)
+        for k in range(3):
+            assert np.array_equal(acc[k][c].cpu().numpy(), ref)
+    # a gravity deposit between apply and return (it works in buffer channel 1) does not disturb Step 4 either
+    g2 = parity.GpuRun(w)
+    rho = torch.empty((64, 64, 64), dtype=torch.float64, device=DEV)
+    g2.ctx.pm_deposit(g2.state, g2.sinks, g2.sne, w.dt)
+    g2.ctx.pm_fold_ghosts()
+    g2.ctx.pm_apply_limited(g2.state)
+    g2.ctx.pm_gravity_deposit(None, x, y, z, dev(gw.m), rho)
+    g2.ctx.pm_return_to_particles(g2.sinks)
+    g2.ctx.pm_check()
+    parity.compare_sinks(g2, o)
+    ref = go.gravity_deposit(gw.params, None, gw.x, gw.y, gw.z, gw.m)
+    assert np.all(np.abs(rho.cpu().numpy() - ref) <= 1e-12 * np.abs(ref) + 1e-300)
+    g.ctx.close(); g2.ctx.close()
