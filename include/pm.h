@@ -231,6 +231,15 @@ int pm_check(pm_ctx *ctx);
  * HOST pointers here (pinned memory recommended). */
 int pm_step_host(pm_ctx *ctx, pm_state *host_state, pm_sinks *host_sinks, const pm_sne *host_sne, double dt);
 
+/* The same in two halves, for callers that have the NEXT step's inputs ready in other host buffers (a host code that double
+ * buffers its mesh): pm_step_host_begin enqueues upload, the four calls and download of one step in slot 0 or 1 and returns
+ * without waiting; pm_step_host_end waits for that slot's results (and reports PM_EDOMAIN / PM_ECUDA).  Each slot has device
+ * staging of its own, uploads and downloads use two more streams, so the upload of one slot runs while the other slot still
+ * downloads (PCIe carries both directions at once); the kernels of the two slots run one after the other.  The host buffers
+ * of a slot must stay untouched between begin and end.  pm_step_host = begin + end on slot 0. */
+int pm_step_host_begin(pm_ctx *ctx, int slot, pm_state *host_state, pm_sinks *host_sinks, const pm_sne *host_sne, double dt);
+int pm_step_host_end(pm_ctx *ctx, int slot);
+
 int pm_destroy(pm_ctx *ctx);
 
 const char *pm_last_error(const pm_ctx *ctx);

@@ -62,6 +62,7 @@ typedef struct {
     double *rho_inf, *v_inf, *c_inf, *r_bh, *mdot, *r_acc, *wsum;
     double *dm, *dpx, *dpy, *dpz;          /* amounts actually returned to the particle (Eq. 5) */
     int32_t *n_member;
+    double *dpabs;                         /* error scale only (may be NULL): sum over the member cells of gain * (|vx| + |vy| + |vz|) */
 } orc_sinks;
 
 typedef struct {
@@ -603,7 +604,7 @@ int orc_return(const orc_params *p, const orc_state *U_old, const double *eta, o
         sink_scalars sc;
         double xs = sk->x[s], ys = sk->y[s], zs = sk->z[s];
         sink_compute_scalars(p, U_old, xs, ys, zs, sk->vx[s], sk->vy[s], sk->vz[s], sk->m[s], &sc);
-        double dm = 0.0, dpx = 0.0, dpy = 0.0, dpz = 0.0;
+        double dm = 0.0, dpx = 0.0, dpy = 0.0, dpz = 0.0, dpabs = 0.0;
         for (int64_t k = sc.kh - sc.g; k <= sc.kh + sc.g; ++k)
             for (int64_t j = sc.jh - sc.g; j <= sc.jh + sc.g; ++j)
                 for (int64_t i = sc.ih - sc.g; i <= sc.ih + sc.g; ++i) {
@@ -617,6 +618,7 @@ int orc_return(const orc_params *p, const orc_state *U_old, const double *eta, o
                     dpx += gain * (U_old->mx[c] / rho);               /* R14 */
                     dpy += gain * (U_old->my[c] / rho);
                     dpz += gain * (U_old->mz[c] / rho);
+                    dpabs += gain * ((fabs(U_old->mx[c]) + fabs(U_old->my[c]) + fabs(U_old->mz[c])) / rho);   /* error scale only */
                 }
         double m_old = sk->m[s];
         double m_new = m_old + dm;
@@ -630,6 +632,7 @@ int orc_return(const orc_params *p, const orc_state *U_old, const double *eta, o
         if (sk->dpx) sk->dpx[s] = dpx;
         if (sk->dpy) sk->dpy[s] = dpy;
         if (sk->dpz) sk->dpz[s] = dpz;
+        if (sk->dpabs) sk->dpabs[s] = dpabs;
     }
     return 0;
 }

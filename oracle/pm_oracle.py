@@ -49,7 +49,7 @@ class OrcSinks(C.Structure):
                 [(f, c_dp) for f in ("x", "y", "z", "vx", "vy", "vz", "m",
                                      "rho_inf", "v_inf", "c_inf", "r_bh", "mdot", "r_acc", "wsum",
                                      "dm", "dpx", "dpy", "dpz")] +
-                [("n_member", c_ip)])
+                [("n_member", c_ip), ("dpabs", c_dp)])
 
 
 class OrcSNe(C.Structure):
@@ -184,6 +184,7 @@ class Oracle:
         self.Te = np.zeros(N) if (keep_abs and abs_channels is None) else None
         self.sink_diag = {k: np.zeros(sinks.n) for k in SINK_DIAG}
         self.sink_diag["n_member"] = np.zeros(sinks.n, dtype=np.int32)
+        self.sink_diag["dpabs"] = np.zeros(sinks.n)          # error scale of the momentum gains (see the C file)
         self.sn_diag = {k: np.zeros(sne.n) for k in SN_DIAG}
         self.sn_diag["regime"] = np.zeros(sne.n, dtype=np.int32)
         self._old = None
@@ -204,6 +205,7 @@ class Oracle:
         for f in SINK_DIAG:
             setattr(o, f, _dp(self.sink_diag[f]))
         o.n_member = _ip(self.sink_diag["n_member"])
+        o.dpabs = _dp(self.sink_diag["dpabs"])
         return o
 
     def _csne(self):

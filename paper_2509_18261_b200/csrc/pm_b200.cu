@@ -57,10 +57,15 @@ struct pm_ctx {
     double dt;
     long long launches;
     // host-step staging
-    cudaStream_t copy_stream; cudaEvent_t ev_inputs, ev_etot;   // pm_step_host: E uploads on its own stream under the deposit
-    double *stg_state;  long long stg_state_cap;
-    double *stg_sinks;  long long stg_sinks_cap;
-    double *stg_sne;    long long stg_sne_cap;
+    // two slots, so that the upload of one step (host -> device) runs under the download of the one before (device -> host)
+    cudaStream_t up_stream, down_stream;
+    struct HostSlot {
+        double *stg_state;  long long stg_state_cap;
+        double *stg_sinks;  long long stg_sinks_cap;
+        double *stg_sne;    long long stg_sne_cap;
+        cudaEvent_t ev_up, ev_done, ev_down;       // inputs on the device / kernels finished / results on the host
+        bool busy;
+    } slot[2];
     // particle binning: keys[np] | perm[np] | counts[2*ntile + 1]
     int *bin_mem;       long long bin_cap;
     int *grav_mem;      long long grav_cap;   // the same three arrays for the gravity calls (their own: a kick may come between
@@ -809,11 +814,16 @@ extern "C" int pm_destroy(pm_ctx *c) {
     if (!c) return PM_EINVAL;
     cudaSetDevice(c->device);
     cudaStreamSynchronize(c->stream);
-    double *ptrs[] = { c->buf, c->ret, c->ret_tr, c->lam, c->sink_scal, c->dbg_sink, c->dbg_sn, c->stg_state, c->stg_sinks, c->stg_sne };
+    double *ptrs[] = { c->buf, c->ret, c->ret_tr, c->lam, c->sink_scal, c->dbg_sink, c->dbg_sn, c->slot[0].stg_state, c->slot[0].stg_sinks,
+                       c->slot[0].stg_sne, c->slot[1].stg_state, c->slot[1].stg_sinks, c->slot[1].stg_sne };
     for (double *p : ptrs) if (p) cudaFree(p);
     if (c->timing)
         for (int k = 0; k < PM_NUM_KERNELS; ++k) { cudaEventDestroy(c->ev[k][0]); cudaEventDestroy(c->ev[k][1]); }
-    if (c->copy_stream) { cudaStreamDestroy(c->copy_stream); cudaEventDestroy(c->ev_inputs); cudaEventDestroy(c->ev_etot); }
+    if (c->up_stream) {
+        cudaStreamSynchronize(c->up_stream); cudaStreamSynchronize(c->down_stream);
+        cudaStreamDestroy(c->up_stream); cudaStreamDestroy(c->down_stream);
+        for (int k = 0; k < 2; ++k) { cudaEventDestroy(c->slot[k].ev_up); cudaEventDestroy(c->slot[k].ev_done); cudaEventDestroy(c->slot[k].ev_down); }
+    }
     if (c->bin_mem) cudaFree(c->bin_mem);
     if (c->grav_mem) cudaFree(c->grav_mem);
     if (c->tile_live) cudaFree(c->tile_live);
@@ -1262,36 +1272,46 @@ extern "C" int pm_check(pm_ctx *c) {
     return PM_OK;
 }
 
-extern "C" int pm_step_host(pm_ctx *c, pm_state *hs, pm_sinks *hk, const pm_sne *hn, double dt) {
+// One step with HOST buffers, in two halves.  begin: enqueue the upload of the inputs (up_stream), the four calls (the ctx's
+// stream, after the upload) and the download of the results (down_stream, after the kernels); end: wait for the download.
+// Two slots with staging of their own: the caller may begin slot 1 - s while slot s is still downloading, and PCIe carries
+// both directions at once.  The kernels of the two slots run one after the other on the ctx's stream (there is one buffer mesh).
+extern "C" int pm_step_host_begin(pm_ctx *c, int slot_id, pm_state *hs, pm_sinks *hk, const pm_sne *hn, double dt) {
     if (!c) return PM_EINVAL;
+    if (slot_id < 0 || slot_id > 1) PM_FAIL(c, PM_EINVAL, "pm_step_host_begin: slot must be 0 or 1");
     if (!state_ok(hs)) PM_FAIL(c, PM_EINVAL, "pm_step_host: null state pointer");
     if (c->P.zopen) PM_FAIL(c, PM_EINVAL, "pm_step_host: not available on a z slab (the exchanges between the calls are the caller's)");
+    pm_ctx::HostSlot &S = c->slot[slot_id];
+    if (S.busy) PM_FAIL(c, PM_EORDER, "pm_step_host_begin: slot %d is in flight (pm_step_host_end first)", slot_id);
     PM_CUDA(c, cudaSetDevice(c->device));
     const long long N = c->P.N, nk = hk ? hk->n : 0, nn = hn ? hn->n : 0;
     int rc;
-    if ((rc = grow(c, &c->stg_state, &c->stg_state_cap, 6 * N)) != PM_OK) return rc;
-    if ((rc = grow(c, &c->stg_sinks, &c->stg_sinks_cap, 11 * nk)) != PM_OK) return rc;
-    if ((rc = grow(c, &c->stg_sne, &c->stg_sne_cap, 8 * nn)) != PM_OK) return rc;
-    cudaStream_t s = c->stream;
-    double *hst[6] = { hs->rho, hs->mx, hs->my, hs->mz, hs->etot, hs->eint };
-    if (!c->copy_stream) {
-        PM_CUDA(c, cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
-        PM_CUDA(c, cudaEventCreateWithFlags(&c->ev_inputs, cudaEventDisableTiming));
-        PM_CUDA(c, cudaEventCreateWithFlags(&c->ev_etot, cudaEventDisableTiming));
+    if ((rc = grow(c, &S.stg_state, &S.stg_state_cap, 6 * N)) != PM_OK) return rc;
+    if ((rc = grow(c, &S.stg_sinks, &S.stg_sinks_cap, 11 * nk)) != PM_OK) return rc;
+    if ((rc = grow(c, &S.stg_sne, &S.stg_sne_cap, 8 * nn)) != PM_OK) return rc;
+    if (!c->up_stream) {
+        PM_CUDA(c, cudaStreamCreateWithFlags(&c->up_stream, cudaStreamNonBlocking));
+        PM_CUDA(c, cudaStreamCreateWithFlags(&c->down_stream, cudaStreamNonBlocking));
+        for (int k = 0; k < 2; ++k) {
+            PM_CUDA(c, cudaEventCreateWithFlags(&c->slot[k].ev_up, cudaEventDisableTiming));
+            PM_CUDA(c, cudaEventCreateWithFlags(&c->slot[k].ev_done, cudaEventDisableTiming));
+            PM_CUDA(c, cudaEventCreateWithFlags(&c->slot[k].ev_down, cudaEventDisableTiming));
+        }
     }
-    // everything the deposit reads first (it never reads E); E follows on the copy stream, under the deposit kernels
-    for (int f = 0; f < 6; ++f)
-        if (f != 4) PM_CUDA(c, cudaMemcpyAsync(c->stg_state + f * N, hst[f], N * 8, cudaMemcpyHostToDevice, s));
-    pm_state ds = { c->stg_state, c->stg_state + N, c->stg_state + 2 * N, c->stg_state + 3 * N, c->stg_state + 4 * N, c->stg_state + 5 * N };
+    cudaStream_t s = c->stream, up = c->up_stream, down = c->down_stream;
+    double *hst[6] = { hs->rho, hs->mx, hs->my, hs->mz, hs->etot, hs->eint };
+    // the slot's staging was last read by its own download, which pm_step_host_end has waited for
+    for (int f = 0; f < 6; ++f) PM_CUDA(c, cudaMemcpyAsync(S.stg_state + f * N, hst[f], N * 8, cudaMemcpyHostToDevice, up));
+    pm_state ds = { S.stg_state, S.stg_state + N, S.stg_state + 2 * N, S.stg_state + 3 * N, S.stg_state + 4 * N, S.stg_state + 5 * N };
     pm_sinks dk; std::memset(&dk, 0, sizeof(dk));
     pm_sne dn; std::memset(&dn, 0, sizeof(dn));
     if (nk > 0) {
         const double *src[7] = { hk->x, hk->y, hk->z, hk->vx, hk->vy, hk->vz, hk->m };
         for (int f = 0; f < 7; ++f) {
             if (!src[f]) PM_FAIL(c, PM_EINVAL, "pm_step_host: null sink array");
-            PM_CUDA(c, cudaMemcpyAsync(c->stg_sinks + f * nk, src[f], nk * 8, cudaMemcpyHostToDevice, s));
+            PM_CUDA(c, cudaMemcpyAsync(S.stg_sinks + f * nk, src[f], nk * 8, cudaMemcpyHostToDevice, up));
         }
-        double *b = c->stg_sinks;
+        double *b = S.stg_sinks;
         dk.n = nk; dk.x = b; dk.y = b + nk; dk.z = b + 2 * nk; dk.vx = b + 3 * nk; dk.vy = b + 4 * nk; dk.vz = b + 5 * nk; dk.m = b + 6 * nk;
         dk.dm = b + 7 * nk; dk.dpx = b + 8 * nk; dk.dpy = b + 9 * nk; dk.dpz = b + 10 * nk;
     }
@@ -1299,28 +1319,51 @@ extern "C" int pm_step_host(pm_ctx *c, pm_state *hs, pm_sinks *hk, const pm_sne 
         const double *src[8] = { hn->x, hn->y, hn->z, hn->vx, hn->vy, hn->vz, hn->e_sn, hn->m_ej };
         for (int f = 0; f < 8; ++f) {
             if (!src[f]) PM_FAIL(c, PM_EINVAL, "pm_step_host: null SN array");
-            PM_CUDA(c, cudaMemcpyAsync(c->stg_sne + f * nn, src[f], nn * 8, cudaMemcpyHostToDevice, s));
+            PM_CUDA(c, cudaMemcpyAsync(S.stg_sne + f * nn, src[f], nn * 8, cudaMemcpyHostToDevice, up));
         }
-        double *b = c->stg_sne;
+        double *b = S.stg_sne;
         dn.n = nn; dn.x = b; dn.y = b + nn; dn.z = b + 2 * nn; dn.vx = b + 3 * nn; dn.vy = b + 4 * nn; dn.vz = b + 5 * nn;
         dn.e_sn = b + 6 * nn; dn.m_ej = b + 7 * nn;
     }
-    PM_CUDA(c, cudaEventRecord(c->ev_inputs, s));
-    PM_CUDA(c, cudaStreamWaitEvent(c->copy_stream, c->ev_inputs, 0));
-    PM_CUDA(c, cudaMemcpyAsync(c->stg_state + 4 * N, hst[4], N * 8, cudaMemcpyHostToDevice, c->copy_stream));
-    PM_CUDA(c, cudaEventRecord(c->ev_etot, c->copy_stream));
+    PM_CUDA(c, cudaEventRecord(S.ev_up, up));
+    PM_CUDA(c, cudaStreamWaitEvent(s, S.ev_up, 0));
     if ((rc = pm_deposit(c, &ds, nk > 0 ? &dk : nullptr, nn > 0 ? &dn : nullptr, dt)) != PM_OK) return rc;
     if ((rc = pm_fold_ghosts(c)) != PM_OK) return rc;
-    PM_CUDA(c, cudaStreamWaitEvent(s, c->ev_etot, 0));          // the apply pass is the first reader of E
     if ((rc = pm_apply_limited(c, &ds)) != PM_OK) return rc;
     if ((rc = pm_return_to_particles(c, nk > 0 ? &dk : nullptr)) != PM_OK) return rc;
-    for (int f = 0; f < 6; ++f) PM_CUDA(c, cudaMemcpyAsync(hst[f], c->stg_state + f * N, N * 8, cudaMemcpyDeviceToHost, s));
+    PM_CUDA(c, cudaEventRecord(S.ev_done, s));
+    PM_CUDA(c, cudaStreamWaitEvent(down, S.ev_done, 0));
+    for (int f = 0; f < 6; ++f) PM_CUDA(c, cudaMemcpyAsync(hst[f], S.stg_state + f * N, N * 8, cudaMemcpyDeviceToHost, down));
     if (nk > 0) {
         double *dst[8] = { hk->vx, hk->vy, hk->vz, hk->m, hk->dm, hk->dpx, hk->dpy, hk->dpz };
         for (int f = 0; f < 8; ++f)
-            if (dst[f]) PM_CUDA(c, cudaMemcpyAsync(dst[f], c->stg_sinks + (3 + f) * nk, nk * 8, cudaMemcpyDeviceToHost, s));
+            if (dst[f]) PM_CUDA(c, cudaMemcpyAsync(dst[f], S.stg_sinks + (3 + f) * nk, nk * 8, cudaMemcpyDeviceToHost, down));
     }
-    return pm_check(c);
+    PM_CUDA(c, cudaMemcpyAsync(c->err_host, c->err_flag, sizeof(int), cudaMemcpyDeviceToHost, down));
+    PM_CUDA(c, cudaEventRecord(S.ev_down, down));
+    S.busy = true;
+    return PM_OK;
+}
+
+extern "C" int pm_step_host_end(pm_ctx *c, int slot_id) {
+    if (!c) return PM_EINVAL;
+    if (slot_id < 0 || slot_id > 1) PM_FAIL(c, PM_EINVAL, "pm_step_host_end: slot must be 0 or 1");
+    pm_ctx::HostSlot &S = c->slot[slot_id];
+    if (!S.busy) PM_FAIL(c, PM_EORDER, "pm_step_host_end: slot %d has no step in flight", slot_id);
+    PM_CUDA(c, cudaSetDevice(c->device));
+    S.busy = false;
+    PM_CUDA(c, cudaEventSynchronize(S.ev_down));
+    if (*c->err_host & 1) {
+        PM_CUDA(c, cudaMemsetAsync(c->err_flag, 0, sizeof(int), c->stream));
+        PM_FAIL(c, PM_EDOMAIN, "a particle lies outside the domain [x0, x0 + n dx)");
+    }
+    return PM_OK;
+}
+
+extern "C" int pm_step_host(pm_ctx *c, pm_state *hs, pm_sinks *hk, const pm_sne *hn, double dt) {
+    int rc = pm_step_host_begin(c, 0, hs, hk, hn, dt);
+    if (rc != PM_OK) return rc;
+    return pm_step_host_end(c, 0);
 }
 
 // ---- test-only views ---------------------------------------------------------------------------------------------

@@ -25,7 +25,7 @@ KERNEL_GROUPS = ("bin", "zero", "sinks", "sne", "fold", "apply", "return")
 STATUS_NAMES = {0: "PM_OK", -1: "PM_EINVAL", -2: "PM_ENOMEM", -3: "PM_ECUDA", -4: "PM_EORDER", -5: "PM_EDOMAIN"}
 
 EXPORTS = ["pm_create", "pm_deposit", "pm_fold_ghosts", "pm_apply_limited", "pm_return_to_particles", "pm_check",
-           "pm_step_host", "pm_destroy", "pm_last_error", "pm_launch_count", "pm_kernel_times", "pm_probe_red_f64", "pm_set_repro_margin", "pm_create_sinks", "pm_gravity_deposit", "pm_gravity_kick", "pm_drift", "pm_slab_describe", "pm_slab_pack", "pm_debug_round_buffers", "pm_debug_buffer", "pm_debug_tile_counts",
+           "pm_step_host", "pm_step_host_begin", "pm_step_host_end", "pm_destroy", "pm_last_error", "pm_launch_count", "pm_kernel_times", "pm_probe_red_f64", "pm_set_repro_margin", "pm_create_sinks", "pm_gravity_deposit", "pm_gravity_kick", "pm_drift", "pm_slab_describe", "pm_slab_pack", "pm_debug_round_buffers", "pm_debug_buffer", "pm_debug_tile_counts",
            "pm_debug_return_mesh", "pm_debug_lambda", "pm_debug_sink_scalars", "pm_debug_sn_scalars",
            "pm_debug_stencil"]
 
@@ -106,6 +106,8 @@ def lib():
         L.pm_return_to_particles.argtypes = [vp, C.POINTER(PmSinks)]
         L.pm_check.argtypes = [vp]
         L.pm_step_host.argtypes = [vp, C.POINTER(PmState), C.POINTER(PmSinks), C.POINTER(PmSNe), C.c_double]
+        L.pm_step_host_begin.argtypes = [vp, C.c_int, C.POINTER(PmState), C.POINTER(PmSinks), C.POINTER(PmSNe), C.c_double]
+        L.pm_step_host_end.argtypes = [vp, C.c_int]
         L.pm_destroy.argtypes = [vp]
         L.pm_last_error.argtypes = [vp]
         L.pm_last_error.restype = C.c_char_p
@@ -338,6 +340,14 @@ class Context:
 
     def pm_step_host(self, st, sk, sn, dt: float):
         """Host-buffer step: st / sk / sn hold numpy arrays or CPU (pinned) tensors; updated in place."""
+        self.pm_step_host_begin(0, st, sk, sn, dt)
+        self.pm_step_host_end(0)
+
+    def pm_step_host_end(self, slot: int):
+        self._chk(self.L.pm_step_host_end(self.h, int(slot)), "pm_step_host_end")
+
+    def pm_step_host_begin(self, slot: int, st, sk, sn, dt: float):
+        """Enqueue one host-buffer step in slot 0 / 1 (upload, four calls, download) without waiting; see include/pm.h."""
         def hp(a):
             if a is None:
                 return None
@@ -359,7 +369,7 @@ class Context:
         if sn is not None:
             for f in DeviceSNe.IN:
                 setattr(cn, f, hp(getattr(sn, f)))
-        self._chk(self.L.pm_step_host(self.h, C.byref(cs), C.byref(ck), C.byref(cn), dt), "pm_step_host")
+        self._chk(self.L.pm_step_host_begin(self.h, int(slot), C.byref(cs), C.byref(ck), C.byref(cn), dt), "pm_step_host_begin")
 
     def pm_create_sinks(self, state: DeviceState, max_new: int):
         """Sec. 3.1.2.  Returns (n_found, dict of device tensors x, y, z, vx, vy, vz, m of length min(n_found, max_new))."""

@@ -188,6 +188,40 @@ def test_permutation_invariance_gpu():
     assert np.allclose(outs[0][0], outs[1][0], rtol=1e-12, atol=0)
 
 
+def test_eq21_fallback_branch_on_the_gpu():
+    """R25 fall-back (a reading, "parity unpinned"): exercised on BOTH sides.  (a) Gas far hotter than the ejecta
+    (e_int / rho = 1e6 against (E_sn + E_kin) / M_ej ~ 1): adding the SN mass at the cell's own specific internal energy needs
+    more energy than the SN brings, K < 0, no lambda satisfies Eq. 21 (discriminant < 0 by Cauchy-Schwarz): lambda = 0 in
+    every touched cell.  (b) A state with E < KE (inconsistent input): e_int = E_2 - KE comes out negative and is clipped to 0."""
+    w = inputs.scaled_mixed(32, 200, seed_index=5)
+    st = w.state
+    for f in ("mx", "my", "mz"):
+        getattr(st, f)[...] *= 20.0                                  # |v| ~ 1
+    ke = 0.5 * (st.mx ** 2 + st.my ** 2 + st.mz ** 2) / st.rho
+    st.eint[...] = 1e6 * st.rho
+    st.etot[...] = st.eint + ke
+    w.sne.e_sn[:] = 1.0
+    g, o, _ = parity.run_and_compare(w, steps=1)
+    touched = o.sn_count > 0
+    assert touched.sum() > 1000 and np.all(o.lam[touched] == 0.0)
+    lam = g.ctx.debug_lambda().cpu().numpy().reshape(-1)
+    assert np.all(lam[touched] == 0.0) and np.all(lam[~touched] == 1.0)
+    # (b)
+    w = inputs.scaled_mixed(32, 200, seed_index=5)
+    st = w.state
+    for f in ("mx", "my", "mz"):
+        getattr(st, f)[...] *= 40.0
+    ke = 0.5 * (st.mx ** 2 + st.my ** 2 + st.mz ** 2) / st.rho
+    st.eint[...] = 1e-8 * st.rho
+    st.etot[...] = 0.5 * ke
+    w.sne.e_sn[:] = 1e-3
+    w = inputs.Workload("clip", w.params, st, inputs.empty_sinks(), w.sne, w.dt, 1)
+    g, o, _ = parity.run_and_compare(w, steps=1)
+    touched = (o.sn_count > 0).reshape(o.shape)
+    assert (o.state.eint[touched] == 0.0).sum() > 100
+    assert np.array_equal(g.state.eint.cpu().numpy() == 0.0, o.state.eint == 0.0)
+
+
 # ---------------------------------------------------------------------------------------------
 # the BASELINE configs at full size
 # ---------------------------------------------------------------------------------------------
@@ -343,6 +377,22 @@ def test_step_host_matches_device_path():
     assert np.allclose(g.sinks.m.cpu().numpy(), hk.m, rtol=1e-12)
     assert np.allclose(g.sinks.dm.cpu().numpy(), hk.dm, rtol=1e-12)
     assert ctx.pm_launch_count() == 12      # 4 binning, 3 reset (stamp, tile-wise zero, sweep), 2 deposits, fold, apply, return
+    # two slots in flight: same results as one step at a time, each slot in its own host buffers
+    a, b = (w.state.copy(), w.sinks.copy()), (w.state.copy(), w.sinks.copy())
+    for _, k in (a, b):
+        k.dm = np.zeros(k.n); k.dpx = np.zeros(k.n); k.dpy = np.zeros(k.n); k.dpz = np.zeros(k.n)
+    ctx.pm_step_host_begin(0, a[0], a[1], hn, w.dt)
+    ctx.pm_step_host_begin(1, b[0], b[1], hn, w.dt)
+    with pytest.raises(pm.PmError) as e:
+        ctx.pm_step_host_begin(1, b[0], b[1], hn, w.dt)          # slot 1 is in flight
+    assert e.value.status == pm.PM_EORDER
+    ctx.pm_step_host_end(0)
+    ctx.pm_step_host_begin(0, a[0], a[1], hn, w.dt)              # second step of a, while b may still be downloading
+    ctx.pm_step_host_end(1)
+    ctx.pm_step_host_end(0)
+    for x, y in zip(hs.fields(), b[0].fields()):
+        assert np.allclose(x, y, rtol=1e-10, atol=1e-10 * np.abs(x).max())
+    assert np.allclose(hk.m, b[1].m, rtol=1e-12) and np.all(a[1].m > b[1].m)     # a has taken two steps
 
 
 def test_kernel_times_and_red_probe():

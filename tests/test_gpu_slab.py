@@ -227,7 +227,7 @@ def test_two_half_domains_give_the_single_domain_oracle_step(n, npart, seed):
     parity.close_strict(g.sink_field("m"), o.sinks.m, "sink m")
     parity.close_strict(g.sink_field("dm"), o.sink_diag["dm"], "sink dm")
     for f in ("dpx", "dpy", "dpz"):
-        parity.close_reorder(g.sink_field(f), o.sink_diag[f], np.abs(o.sink_diag["dm"]) * 0.2, f"sink {f}")
+        parity.close_reorder(g.sink_field(f), o.sink_diag[f], (parity.EPS / parity.REORDER) * (parity.C_TERM + 264.0) * o.sink_diag["dpabs"], f"sink {f}")
     # sinks at the cut really used the neighbour's cells
     near = np.minimum(np.abs(w.sinks.z - h), np.minimum(w.sinks.z, n - w.sinks.z)) < 3.0
     assert near.sum() >= 2 and np.all(o.sink_diag["dm"][near] > 0)
