@@ -488,28 +488,39 @@ def run_ours(args, rank, world, local_rank):
     e2e_steps = max(2, min(max(args.steps, 2), args.e2e_steps))
     hA = inputs.State(*(torch.from_numpy(f).pin_memory() for f in w.state.fields()))
     hB = inputs.State(*(t.clone().pin_memory() for t in hA.fields()))
-    hkA = w.sinks.copy()
-    for f in ("dm", "dpx", "dpy", "dpz"):
-        setattr(hkA, f, np.zeros(hkA.n))
-    hkB = w.sinks.copy()
-    for f in ("dm", "dpx", "dpy", "dpz"):
-        setattr(hkB, f, np.zeros(hkB.n))
+    class _Host:            # particle arrays in pinned memory too: a copy to or from pageable memory blocks the calling thread
+        pass
+
+    def pinned_sinks():
+        o = _Host()
+        o.n = w.sinks.n
+        for f in pm.DeviceSinks.IN:
+            setattr(o, f, torch.from_numpy(getattr(w.sinks, f).copy()).pin_memory())
+        for f in pm.DeviceSinks.OUT:
+            setattr(o, f, torch.zeros(w.sinks.n, dtype=torch.float64).pin_memory())
+        return o
+
+    hkA, hkB = pinned_sinks(), pinned_sinks()
+    hsn = _Host()
+    hsn.n = w.sne.n
+    for f in pm.DeviceSNe.IN:
+        setattr(hsn, f, torch.from_numpy(getattr(w.sne, f)).pin_memory())
     del st
     torch.cuda.empty_cache()
-    ctx.pm_step_host(hA, hkA, w.sne, w.dt)      # warm-up (allocates the staging of both slots)
-    ctx.pm_step_host_begin(1, hB, hkB, w.sne, w.dt)
+    ctx.pm_step_host(hA, hkA, hsn, w.dt)      # warm-up (allocates the staging of both slots)
+    ctx.pm_step_host_begin(1, hB, hkB, hsn, w.dt)
     ctx.pm_step_host_end(1)
     barrier()
     t0 = time.perf_counter()
-    ctx.pm_step_host(hA, hkA, w.sne, w.dt)
+    ctx.pm_step_host(hA, hkA, hsn, w.dt)
     torch.cuda.synchronize(dev)
     serial_s = reduce_max(time.perf_counter() - t0, world, dev)
     host = ((hA, hkA), (hB, hkB))
     barrier()
     t0 = time.perf_counter()
-    ctx.pm_step_host_begin(0, hA, hkA, w.sne, w.dt)
+    ctx.pm_step_host_begin(0, hA, hkA, hsn, w.dt)
     for i in range(1, e2e_steps):
-        ctx.pm_step_host_begin(i % 2, host[i % 2][0], host[i % 2][1], w.sne, w.dt)
+        ctx.pm_step_host_begin(i % 2, host[i % 2][0], host[i % 2][1], hsn, w.dt)
         ctx.pm_step_host_end((i - 1) % 2)
     ctx.pm_step_host_end((e2e_steps - 1) % 2)
     torch.cuda.synchronize(dev)

@@ -28,6 +28,7 @@ using namespace pm;
 // Preferred shared-memory carve-out (% of the 256 KB L1) of the sink kernels: measured on config 5, 25 / 50 / 75 / 100 %
 // give 0.52 / 0.50 / 0.53 / 0.79 ms (deposit) and 0.22 / 0.20 / 0.20 / 0.27 ms (return); the SN kernel is best at the default.
 constexpr int kSinkCarveout = 50;
+constexpr size_t kSnDenseSmem = (size_t)5 * kAccCells * sizeof(double) + (size_t)kSnDenseWarps * sizeof(SnWarpSmem);
 
 // ---------------------------------------------------------------------------------------------------------------
 // context
@@ -80,6 +81,7 @@ struct pm_ctx {
     double *slab_mem;   // z-slab mode: send_lo | send_hi | recv_lo | recv_hi, each nch * g * pk doubles (pm_slab.cuh)
     long long slab_elems;   // doubles per slab
     bool slab_packed;   // pm_slab_pack has run since the last pm_deposit
+    bool dense_smem_ok; // the device grants the dense SN kernel its shared memory (tile accumulator, 150 KB)
     bool grav_in_ch1;   // buffer channel 1 holds the last pm_gravity_deposit (until the next pm_deposit): the debug view must not
                         // "fill in" its stale tiles
     bool timing;        // PM_FLAG_TIMING
@@ -194,13 +196,15 @@ __global__ void __launch_bounds__(1024) k_bin_scan_sums(int *__restrict__ sums, 
     for (int i = lo; i < hi; ++i) { const int c = sums[i]; sums[i] = run; run += c; }
 }
 
-__global__ void __launch_bounds__(256) k_bin_fill(const int *__restrict__ keys, int *__restrict__ cursor,
+// start[key] (exclusive prefix inside its scan chunk) and sums[chunk] stay as they are, fillc[key] ends as the bin's count: both
+// are read again after the fill (dense-bin list, k_deposit_sne_dense)
+__global__ void __launch_bounds__(256) k_bin_fill(const int *__restrict__ keys, const int *__restrict__ start, int *__restrict__ fillc,
                                                   const int *__restrict__ sums, int *__restrict__ perm, long long np,
                                                   long long nk) {
     const long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= np) return;
     const int key = keys[p];
-    const int pos = atomicAdd(cursor + key, 1) + sums[key / kScanChunk];
+    const int pos = start[key] + sums[key / kScanChunk] + atomicAdd(fillc + key, 1);
     perm[pos] = (int)(p < nk ? p : p - nk);
 }
 
@@ -604,6 +608,7 @@ __global__ void __launch_bounds__(kApplyThreads, 6) k_apply_limited(const DevP P
     any = any && valid;
     // Skip at WARP granularity: a warp covers 32*VEC consecutive cells of each field (512 B per stream at VEC = 2), so
     // the state traffic is either whole coalesced lines or nothing (sector-sparse reads waste DRAM bursts).
+    // (16- and 8-thread groups, i.e. whole 128- / 64-byte pieces, measured the same 3.41 ms)
     const bool wany = __any_sync(0xffffffffu, any);
     if (LAM && valid && !any) { double one[VEC]; for (int v = 0; v < VEC; ++v) one[v] = 1.0; stv<VEC>(lam_out + (q - P.zoff), one); }
     if (!wany || !valid) return;                // dU^sum = 0 on the whole segment: U unchanged, nothing to read or write
@@ -761,6 +766,10 @@ extern "C" int pm_create(const pm_params *prm, int device, void *cuda_stream, pm
         if (e == cudaSuccess) e = cudaFuncSetAttribute(k_deposit_sinks_g4<true, true>, cudaFuncAttributePreferredSharedMemoryCarveout, kSinkCarveout);
         if (e == cudaSuccess) e = cudaFuncSetAttribute(k_return_sinks_g4, cudaFuncAttributePreferredSharedMemoryCarveout, kSinkCarveout);
     }
+    if (e == cudaSuccess) {
+        c->dense_smem_ok = cudaFuncSetAttribute(k_deposit_sne_dense, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSnDenseSmem) == cudaSuccess;
+        cudaGetLastError();
+    }
     c->repro = (prm->flags & PM_FLAG_REPRODUCIBLE) != 0;
     c->repro_M = 28;                                  // the paper's example margin (L612)
     c->nch = c->repro ? kReproChannels : kBufChannels;
@@ -869,14 +878,16 @@ extern "C" int pm_deposit(pm_ctx *c, const pm_state *st, const pm_sinks *sk, con
 
     for (int k = 0; k < PM_NUM_KERNELS; ++k) c->ev_used[k] = false;
     const long long np = nk + nn;
-    int *keys = nullptr, *perm = nullptr, *counts = nullptr, *live = nullptr;
+    int *keys = nullptr, *perm = nullptr, *counts = nullptr, *sums = nullptr, *live = nullptr, *fillc = nullptr, *dense_n = nullptr, *dense_list = nullptr;
     unsigned char *occ = nullptr;
     if (np > 0 || P.zopen) {   // a1: bin particles by host tile (a slab without particles still needs the scratch of the reset)
         if (np >= (1ll << 31)) PM_FAIL(c, PM_EINVAL, "pm_deposit: too many particles");
         const int nkeys = 2 * P.ntile + 1;
         const int nscan = (nkeys + kScanChunk - 1) / kScanChunk;
         const int nocc = (2 * P.ntile + 3) / 4;                         // bin occupancy bytes, in ints
-        const long long need = 2 * np + nkeys + nscan + nocc + 2;
+        // keys | perm | start (counts, then their scan) | chunk sums | fill counters | occupancy | live-tile counters (2) |
+        // dense-bin counters (front, back, queue head) | dense-bin list
+        const long long need = 2 * np + nkeys + nscan + nkeys + nocc + 2 + 3 + P.ntile;
         if (need > c->bin_cap) {
             if (c->bin_mem) { PM_CUDA(c, cudaFree(c->bin_mem)); c->bin_mem = nullptr; c->bin_cap = 0; }
             const long long cap = need + need / 4;
@@ -885,10 +896,13 @@ extern "C" int pm_deposit(pm_ctx *c, const pm_state *st, const pm_sinks *sk, con
             c->bin_cap = cap;
         }
         keys = c->bin_mem; perm = keys + np; counts = perm + np;
-        int *sums = counts + nkeys;
-        occ = reinterpret_cast<unsigned char *>(sums + nscan);
-        live = sums + nscan + nocc;
-        PM_CUDA(c, cudaMemsetAsync(counts, 0, (size_t)(nkeys + nscan + nocc + 2) * sizeof(int), c->stream));
+        sums = counts + nkeys;
+        fillc = sums + nscan;
+        occ = reinterpret_cast<unsigned char *>(fillc + nkeys);
+        live = fillc + nkeys + nocc;
+        dense_n = live + 2;
+        dense_list = dense_n + 3;
+        PM_CUDA(c, cudaMemsetAsync(counts, 0, (size_t)(nkeys + nscan + nkeys + nocc + 2 + 3) * sizeof(int), c->stream));
         if (np > 0) {
             const unsigned blocks = (unsigned)((np + 255) / 256);
             tick(c, PM_K_BIN, 0);
@@ -899,7 +913,7 @@ extern "C" int pm_deposit(pm_ctx *c, const pm_state *st, const pm_sinks *sk, con
             if ((rc = check_launch(c, "k_bin_scan_local")) != PM_OK) return rc;
             k_bin_scan_sums<<<1, 1024, 0, c->stream>>>(sums, nscan);
             if ((rc = check_launch(c, "k_bin_scan_sums")) != PM_OK) return rc;
-            k_bin_fill<<<blocks, 256, 0, c->stream>>>(keys, counts, sums, perm, np, nk);
+            k_bin_fill<<<blocks, 256, 0, c->stream>>>(keys, counts, fillc, sums, perm, np, nk);
             if ((rc = check_launch(c, "k_bin_fill")) != PM_OK) return rc;
             tick(c, PM_K_BIN, 1);
         }
@@ -937,9 +951,22 @@ extern "C" int pm_deposit(pm_ctx *c, const pm_state *st, const pm_sinks *sk, con
         const unsigned blocks = (unsigned)((nn + kSnWarps - 1) / kSnWarps);
         const size_t smem = kSnWarps * sn_table_bytes(2 * P.gn + 1, P.nsub);
         tick(c, PM_K_SNE, 0);
-        if (P.gn == 3 && P.nsub == 4 && !c->force_generic && 7 * P.pk < (1ll << 31))   // box offsets are 32-bit there
-            (c->repro ? k_deposit_sne_g3n4<true> : k_deposit_sne_g3n4<false>)<<<(unsigned)((nn + kFastSnWarps - 1) / kFastSnWarps), kFastSnWarps * 32, 0, c->stream>>>(P, U, S, c->buf, dbg ? c->dbg_sn : nullptr, c->err_flag, perm + nk);
-        else
+        if (P.gn == 3 && P.nsub == 4 && !c->force_generic && 7 * P.pk < (1ll << 31)) {   // box offsets are 32-bit there
+            // bins with many particles go through the shared-memory tile accumulator (pm_sn_fast.cuh), the others add directly
+            // (opt-in, PM_FLAG_SMEM_TILES: measured slower than the direct path at every threshold on B200)
+            const bool dense = !c->repro && c->dense_smem_ok && (c->prm.flags & PM_FLAG_SMEM_TILES) != 0;
+            const int *keys_sn = keys + nk, *cnt_sn = dense ? fillc + P.ntile : nullptr;
+            if (dense) {
+                k_sn_dense_bins<<<(unsigned)((P.ntile + 255) / 256), 256, 0, c->stream>>>(P.ntile, cnt_sn, dense_list, dense_n);
+                if ((rc = check_launch(c, "k_sn_dense_bins")) != PM_OK) return rc;
+            }
+            (c->repro ? k_deposit_sne_g3n4<true> : k_deposit_sne_g3n4<false>)<<<(unsigned)((nn + kFastSnWarps - 1) / kFastSnWarps), kFastSnWarps * 32, 0, c->stream>>>(P, U, S, c->buf, dbg ? c->dbg_sn : nullptr, c->err_flag, perm + nk, keys_sn, cnt_sn, kSnDenseMin);
+            if (dense) {
+                if ((rc = check_launch(c, "k_deposit_sne_g3n4")) != PM_OK) return rc;
+                k_deposit_sne_dense<<<c->sm_count, kSnDenseWarps * 32, kSnDenseSmem, c->stream>>>(P, U, S, c->buf, dbg ? c->dbg_sn : nullptr, c->err_flag, perm + nk,
+                                                                                               counts, sums, cnt_sn, dense_list, dense_n, dense_n + 2, kScanChunk, (int)nk);
+            }
+        } else
             (c->repro ? k_deposit_sne<true> : k_deposit_sne<false>)<<<blocks, kSnWarps * 32, smem, c->stream>>>(P, U, S, c->buf, dbg ? c->dbg_sn : nullptr, c->err_flag, perm + nk);
         if ((rc = check_launch(c, "k_deposit_sne")) != PM_OK) return rc;
         tick(c, PM_K_SNE, 1);
@@ -1170,7 +1197,7 @@ static int grav_order(pm_ctx *c, const double *x, const double *y, const double 
     const int nscan = (nkeys + kScanChunk - 1) / kScanChunk;
     if (c->gperm_valid && c->gperm_x == x && c->gperm_n == n) { *perm_out = c->grav_mem + n; return PM_OK; }
     c->gperm_valid = false;
-    const long long need = 2 * n + nkeys + nscan;
+    const long long need = 2 * n + nkeys + nscan + nkeys;
     if (need > c->grav_cap) {
         if (c->grav_mem) { PM_CUDA(c, cudaFree(c->grav_mem)); c->grav_mem = nullptr; c->grav_cap = 0; }
         const long long cap = need + need / 4;
@@ -1178,9 +1205,9 @@ static int grav_order(pm_ctx *c, const double *x, const double *y, const double 
         if (e != cudaSuccess) { c->grav_mem = nullptr; PM_FAIL(c, PM_ENOMEM, "cudaMalloc of bins failed: %s", cudaGetErrorString(e)); }
         c->grav_cap = cap;
     }
-    int *keys = c->grav_mem, *perm = keys + n, *counts = perm + n, *sums = counts + nkeys;
+    int *keys = c->grav_mem, *perm = keys + n, *counts = perm + n, *sums = counts + nkeys, *fillc = sums + nscan;
     int rc;
-    PM_CUDA(c, cudaMemsetAsync(counts, 0, (size_t)nkeys * sizeof(int), c->stream));
+    PM_CUDA(c, cudaMemsetAsync(counts, 0, (size_t)(nkeys + nscan + nkeys) * sizeof(int), c->stream));
     const unsigned blocks = (unsigned)((n + 255) / 256);
     k_bin_count<<<blocks, 256, 0, c->stream>>>(P, x, y, z, n, nullptr, nullptr, nullptr, 0, keys, counts, nullptr);
     if ((rc = check_launch(c, "k_bin_count")) != PM_OK) return rc;
@@ -1188,7 +1215,7 @@ static int grav_order(pm_ctx *c, const double *x, const double *y, const double 
     if ((rc = check_launch(c, "k_bin_scan_local")) != PM_OK) return rc;
     k_bin_scan_sums<<<1, 1024, 0, c->stream>>>(sums, nscan);
     if ((rc = check_launch(c, "k_bin_scan_sums")) != PM_OK) return rc;
-    k_bin_fill<<<blocks, 256, 0, c->stream>>>(keys, counts, sums, perm, n, n);
+    k_bin_fill<<<blocks, 256, 0, c->stream>>>(keys, counts, fillc, sums, perm, n, n);
     if ((rc = check_launch(c, "k_bin_fill")) != PM_OK) return rc;
     c->gperm_x = x; c->gperm_n = n; c->gperm_valid = true;
     *perm_out = perm;

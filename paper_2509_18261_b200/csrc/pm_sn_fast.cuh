@@ -66,12 +66,24 @@ __device__ __forceinline__ double sn_threshold(const double x, const double R) {
 
 __device__ __forceinline__ double pick3(int ax, double a, double b, double c) { return ax == 0 ? a : (ax == 1 ? b : c); }
 
+// Shared-memory-privatised tile accumulator (north_star): the five SN channels of the 14^3 cells a particle hosted in
+// one 8^3 tile can reach (tile + 3-cell halo), 5 x 2744 doubles = 107 KB, owned by ONE CTA that processes all particles of
+// the tile.  fp64 has no native shared-memory atomic add (atomicAdd(double*) on shared memory compiles to a CAS loop,
+// ATOMS.CAST.SPIN.64), so the warps of the CTA take turns under one CTA-wide lock and add with plain loads and stores:
+// 5 x (LDS, DADD, STS) per 32 cells.
+constexpr int kAccSide = 14, kAccCells = kAccSide * kAccSide * kAccSide;
+struct SnTileAcc {
+    double *acc;        // [5][kAccCells] in shared memory
+    int *lock;          // 0 = free
+    int ox, oy, oz;     // owned coordinates of accumulator cell (0, 0, 0): tile origin - 3
+};
+
 // The whole deposit of ONE supernova by one warp (all 32 lanes must call).  s = particle index; sm = this warp's shared
 // scratch.
-template <bool REPRO>
+template <bool REPRO, bool DENSE = false>
 __device__ __forceinline__ void sn_deposit_one(const DevP &P, const DevState &U, const DevSNe &S, double *__restrict__ buf,
                                                double *__restrict__ dbg, int *__restrict__ err, const long long s,
-                                               SnWarpSmem &sm, const int lane) {
+                                               SnWarpSmem &sm, const int lane, const SnTileAcc *tile = nullptr) {
     const double xs = S.x[s], ys = S.y[s], zs = S.z[s];
     const int ih = host_cell(xs, P.x0[0], P.inv_dx), jh = host_cell(ys, P.x0[1], P.inv_dx), kh = host_cell(zs, P.x0[2], P.inv_dx);
     if (ih < 0 || ih >= P.nx || jh < 0 || jh >= P.ny || kh < 0 || kh >= P.nz) {
@@ -245,6 +257,44 @@ __device__ __forceinline__ void sn_deposit_one(const DevP &P, const DevState &U,
     const double k_p = sc.p_rad * inv_vsnr;
     double *const sbuf = buf + P.Nb + ((long long)(kh - 3 + P.g) * P.pk + (long long)(jh - 3 + P.g) * P.pj + (ih - 3 + P.gx));
     const int pj = (int)P.pj, pk = (int)P.pk;
+    if (DENSE) {
+        // the same values, added into the CTA's tile accumulator: all 32 lanes stay in the loop (the lock is taken per warp)
+        volatile double *const acc = tile->acc;
+        const int lb = ((kh - 3 - tile->oz) * kAccSide + (jh - 3 - tile->oy)) * kAccSide + (ih - 3 - tile->ox);
+#pragma unroll 1
+        for (int base = 0; base < na; base += 32) {
+            const int idx = base + lane;
+            const bool on = idx < na;
+            const int e = on ? sm.list[idx] : 0;
+            const int a = e & 7, b = (e >> 3) & 7, cc = (e >> 6) & 7;
+            const double omega = (double)((e >> 9) + 1) * (1.0 / 64.0);
+            const int q = inner ? qb + cc * nxny + b * P.nx + a : sm.off[2][cc] + sm.off[1][b] + sm.off[0][a];
+            const double rho = U.rho[q], mx = U.mx[q], my = U.my[q], mz = U.mz[q];
+            const double ddx = sm.dc[0][a], ddy = sm.dc[1][b], ddz = sm.dc[2][cc];
+            const double r2 = dist2(ddx, ddy, ddz);
+            const double ir = r2 > 0.0 ? rsqrt(r2) : 0.0;
+            const double drho = omega * k_rho;
+            const double pscale = (k_p * omega) * ir;
+            const double prx = pscale * ddx, pry = pscale * ddy, prz = pscale * ddz;
+            const double dpx = fma(omega, fma(rho, sc.vcx, -mx), fma(drho, sc.vcx, prx));
+            const double dpy = fma(omega, fma(rho, sc.vcy, -my), fma(drho, sc.vcy, pry));
+            const double dpz = fma(omega, fma(rho, sc.vcz, -mz), fma(drho, sc.vcz, prz));
+            const double de = fma(omega, k_e, fma(sc.vcx, prx, fma(sc.vcy, pry, sc.vcz * prz)));
+            const int li = lb + (cc * kAccSide + b) * kAccSide + a;
+            if (lane == 0) while (atomicCAS(tile->lock, 0, 1) != 0) { }
+            __syncwarp();
+            if (on) {
+                acc[li] += drho;
+                acc[kAccCells + li] += dpx;
+                acc[2 * kAccCells + li] += dpy;
+                acc[3 * kAccCells + li] += dpz;
+                acc[4 * kAccCells + li] += de;
+            }
+            __threadfence_block();
+            __syncwarp();
+            if (lane == 0) atomicExch(tile->lock, 0);
+        }
+    } else
 #pragma unroll 1
     for (int idx = lane; idx < na; idx += 32) {
         const int e = sm.list[idx];
@@ -286,12 +336,101 @@ __device__ __forceinline__ void sn_deposit_one(const DevP &P, const DevState &U,
 template <bool REPRO>
 __global__ void __launch_bounds__(kFastSnWarps * 32, kFastSnMinBlocks) k_deposit_sne_g3n4(const DevP P, const DevState U, const DevSNe S,
                                                                             double *__restrict__ buf, double *__restrict__ dbg,
-                                                                            int *__restrict__ err, const int *__restrict__ perm) {
+                                                                            int *__restrict__ err, const int *__restrict__ perm,
+                                                                            const int *__restrict__ keys_sn, const int *__restrict__ cnt_sn,
+                                                                            const int dense_min) {
     __shared__ SnWarpSmem sm_all[kFastSnWarps];
     const int wib = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const long long w = (long long)blockIdx.x * kFastSnWarps + wib;
     if (w >= S.n) return;
-    sn_deposit_one<REPRO>(P, U, S, buf, dbg, err, perm[w], sm_all[wib], lane);
+    const int s = perm[w];
+    // particles of a dense bin are left to k_deposit_sne_dense (cnt_sn == nullptr: no dense path in this launch)
+    if (cnt_sn && cnt_sn[keys_sn[s] - P.ntile] >= dense_min) return;
+    sn_deposit_one<REPRO>(P, U, S, buf, dbg, err, s, sm_all[wib], lane);
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// Dense bins: one CTA owns an 8^3 tile with many particles, accumulates all of them in shared memory and adds the tile
+// accumulator to the buffer mesh once (north_star: "a shared-memory-privatised tile accumulator for clustered particles").
+// Which bins take this path is decided per bin from its particle count (kSnDenseMin): a particle costs ~183 cells x 5 = 915
+// global REDs on the direct path, the flush of a tile 14^3 x 5 = 13720, break-even at 15 particles per tile in RED count;
+// the accumulation under the CTA-wide lock and the lower occupancy (one CTA of 16 warps per SM) put the measured break-even
+// higher.
+// ---------------------------------------------------------------------------------------------------------------
+constexpr int kSnDenseWarps = 16;
+#ifndef PM_SN_DENSE_MIN
+#define PM_SN_DENSE_MIN 48
+#endif
+constexpr int kSnDenseMin = PM_SN_DENSE_MIN;
+
+// inverse of bin_key: owned tile coordinates of an SN bin
+__device__ __forceinline__ void bin_tile(const DevP &P, int key, int &tx, int &ty, int &tz) {
+    const int sb = key >> (3 * kSbLog2), local = key & ((1 << (3 * kSbLog2)) - 1);
+    int lx = 0, ly = 0, lz = 0;
+#pragma unroll
+    for (int bit = 0; bit < kSbLog2; ++bit) {
+        lx |= ((local >> (3 * bit)) & 1) << bit; ly |= ((local >> (3 * bit + 1)) & 1) << bit; lz |= ((local >> (3 * bit + 2)) & 1) << bit;
+    }
+    const int sx = sb % P.nsbx, r = sb / P.nsbx, sy = r % P.nsby, sz = r / P.nsby;
+    tx = (sx << kSbLog2) + lx; ty = (sy << kSbLog2) + ly; tz = (sz << kSbLog2) + lz;
+}
+
+// SN bins with at least kSnDenseMin particles, the fullest first (they bound the tail of the dense kernel): bins with >= 4 x
+// the minimum are listed from the front, the others from the back of dense_list[0 .. ntile).
+__global__ void __launch_bounds__(256) k_sn_dense_bins(const int ntile, const int *__restrict__ cnt_sn, int *__restrict__ dense_list,
+                                                       int *__restrict__ dense_n) {
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= ntile) return;
+    const int c = cnt_sn[b];
+    if (c < kSnDenseMin) return;
+    if (c >= 4 * kSnDenseMin) dense_list[atomicAdd(dense_n, 1)] = b;
+    else dense_list[ntile - 1 - atomicAdd(dense_n + 1, 1)] = b;
+}
+
+__global__ void __launch_bounds__(kSnDenseWarps * 32, 1) k_deposit_sne_dense(const DevP P, const DevState U, const DevSNe S,
+                                                                             double *__restrict__ buf, double *__restrict__ dbg,
+                                                                             int *__restrict__ err, const int *__restrict__ perm,
+                                                                             const int *__restrict__ start_local, const int *__restrict__ sums,
+                                                                             const int *__restrict__ cnt_sn, const int *__restrict__ dense_list,
+                                                                             const int *__restrict__ dense_n, int *__restrict__ next,
+                                                                             const int scan_chunk, const int nk) {
+    extern __shared__ __align__(16) unsigned char dsm[];
+    double *acc = reinterpret_cast<double *>(dsm);
+    SnWarpSmem *sm_all = reinterpret_cast<SnWarpSmem *>(dsm + (size_t)5 * kAccCells * sizeof(double));
+    __shared__ int lock, item;
+    const int wib = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    for (int e = threadIdx.x; e < 5 * kAccCells; e += blockDim.x) acc[e] = 0.0;
+    if (threadIdx.x == 0) lock = 0;
+    const int n_front = dense_n[0], n_back = dense_n[1];
+    for (;;) {
+        __syncthreads();
+        if (threadIdx.x == 0) item = atomicAdd(next, 1);
+        __syncthreads();
+        const int it = item;
+        if (it >= n_front + n_back) break;
+        const int b = it < n_front ? dense_list[it] : dense_list[P.ntile - 1 - (it - n_front)];
+        const int key = P.ntile + b;                                          // SN keys follow the sink keys
+        const int first = start_local[key] + sums[key / scan_chunk] - nk;    // position in the SN part of perm
+        const int count = cnt_sn[b];
+        int tx, ty, tz;
+        bin_tile(P, b, tx, ty, tz);
+        SnTileAcc tile = { acc, &lock, 8 * tx - 3, 8 * ty - 3, 8 * tz - 3 };
+        for (int p = wib; p < count; p += kSnDenseWarps)
+            sn_deposit_one<false, true>(P, U, S, buf, dbg, err, perm[first + p], sm_all[wib], lane, &tile);
+        __syncthreads();
+        // flush: one RED per non-zero accumulator word, then the word is cleared for the next tile
+        for (int e = threadIdx.x; e < kAccCells; e += blockDim.x) {
+            const int lx = e % kAccSide, r = e / kAccSide, ly = r % kAccSide, lz = r / kAccSide;
+            const int i = tile.ox + lx, j = tile.oy + ly, k = tile.oz + lz;
+            if (i >= P.nx + P.g || j >= P.ny + P.g || k >= P.nz + P.g) continue;      // beyond the ghost zone (ragged last tile): never touched
+            double *dst = buf + P.Nb + ghost_index(P, i, j, k);
+#pragma unroll
+            for (int f = 0; f < 5; ++f) {
+                const double v = acc[f * kAccCells + e];
+                if (v != 0.0) { red_add(dst + (long long)f * P.Nb, v); acc[f * kAccCells + e] = 0.0; }
+            }
+        }
+    }
 }
 
 }  // namespace pm

@@ -20,7 +20,7 @@ SRC = [os.path.join(_HERE, "csrc", "pm_b200.cu")]
 HDRS = sorted(glob.glob(os.path.join(_HERE, "csrc", "*.cuh"))) + [os.path.join(os.path.dirname(_HERE), "include", "pm.h")]
 
 PM_OK, PM_EINVAL, PM_ENOMEM, PM_ECUDA, PM_EORDER, PM_EDOMAIN = 0, -1, -2, -3, -4, -5
-PM_FLAG_DEBUG_SCALARS, PM_FLAG_DEBUG_LAMBDA, PM_FLAG_GENERIC_KERNELS, PM_FLAG_TIMING, PM_FLAG_REPRODUCIBLE = 1, 2, 4, 8, 16
+PM_FLAG_DEBUG_SCALARS, PM_FLAG_DEBUG_LAMBDA, PM_FLAG_GENERIC_KERNELS, PM_FLAG_TIMING, PM_FLAG_REPRODUCIBLE, PM_FLAG_SMEM_TILES = 1, 2, 4, 8, 16, 32
 KERNEL_GROUPS = ("bin", "zero", "sinks", "sne", "fold", "apply", "return")
 STATUS_NAMES = {0: "PM_OK", -1: "PM_EINVAL", -2: "PM_ENOMEM", -3: "PM_ECUDA", -4: "PM_EORDER", -5: "PM_EDOMAIN"}
 

@@ -129,6 +129,28 @@ def test_stacked_particles_contention():
     parity.run_and_compare(w, steps=1)
 
 
+def test_shared_memory_tile_accumulator_path(monkeypatch):
+    """PM_FLAG_SMEM_TILES: supernova bins with >= 48 particles go through the shared-memory-privatised tile accumulator (one
+    CTA per tile, flushed once), the rest through the direct path; both in one step.  Clustered workloads, a stack of 100
+    supernovae on one spot, a cluster on the periodic corner (the flush reaches ghost zones in all three directions)."""
+    flags = pm.PM_FLAG_DEBUG_SCALARS | pm.PM_FLAG_DEBUG_LAMBDA | pm.PM_FLAG_SMEM_TILES
+    orig = parity.GpuRun.__init__
+    monkeypatch.setattr(parity.GpuRun, "__init__", lambda self, w_, device="cuda:0", flags=flags: orig(self, w_, device, flags))
+    w = inputs.scaled_mixed(48, 4000, seed_index=5, n_clusters=2)       # two clusters of ~900 supernovae: bins of 50-300
+    g, o, _ = parity.run_and_compare(w, steps=2)
+    sn_bins = np.bincount((np.floor(w.sne.z / 8) * 36 + np.floor(w.sne.y / 8) * 6 + np.floor(w.sne.x / 8)).astype(int), minlength=216)
+    assert (sn_bins >= 48).sum() >= 3 and ((sn_bins > 0) & (sn_bins < 48)).sum() >= 20      # both paths are taken
+    w = inputs.scaled_mixed(32, 120, seed_index=5)
+    rng = np.random.default_rng(9)
+    for prt, c in ((w.sinks, (15.7, 16.2, 0.4)), (w.sne, (31.6, 0.3, 31.9))):          # the SN stack sits on the periodic corner
+        prt.x[:] = np.mod(c[0] + 1e-3 * rng.standard_normal(prt.n), 32.0)
+        prt.y[:] = np.mod(c[1] + 1e-3 * rng.standard_normal(prt.n), 32.0)
+        prt.z[:] = np.mod(c[2] + 1e-3 * rng.standard_normal(prt.n), 32.0)
+    parity.run_and_compare(w, steps=1)
+    w = inputs.scaled_mixed(37, 3000, seed_index=5, n_clusters=1)       # odd grid: scalar paths, ragged last tile
+    parity.run_and_compare(w, steps=1)
+
+
 def test_only_sinks_and_only_sne_and_empty():
     w = inputs.scaled_mixed(32, 200, seed_index=5)
     w1 = inputs.Workload("sinks", w.params, w.state.copy(), w.sinks.copy(), inputs.empty_sne(), w.dt, 1)
