@@ -226,6 +226,35 @@ int pm_gravity_kick(pm_ctx *ctx, const double *gx, const double *gy, const doubl
 int pm_drift(pm_ctx *ctx, int64_t n, double *x, double *y, double *z, const double *vx, const double *vy, const double *vz,
              double dt);
 
+/* ---- one entry point that allocates nothing -------------------------------------------------------------------
+ * pm_gravity_deposit for callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses
+ * that forbid it): no ctx, no cudaMalloc / cudaFree / allocating library routine, on any call.  The ghost-zoned accumulation
+ * mesh of Step 1 (L59) lives in ONE file-scope __device__ array of PM_NOALLOC_SCRATCH_BYTES (2.5 MiB + 256 bytes) that every
+ * GPU loading the library holds until the process exits.  Limit: (nx + 4)(ny + 2)(nz + 2) <= PM_NOALLOC_MAX_GHOSTED_CELLS
+ * (cubes up to 66^3 cells fit; one ghost layer, the x origin rounded up to 2 cells); a larger mesh is refused with PM_EINVAL and a message
+ * that names the limit -- use a ctx for it.  At least 3 cells per axis (R32).
+ *
+ * Same operation, kernels and argument meaning as pm_gravity_deposit: rho_tot := rho_gas + sum_s m_s W(x_ijk - x_s) / V (L51,
+ * cloud-in-cell, R40), rho_gas may be NULL and may alias rho_tot, all array pointers DEVICE fp64 (particle arrays n values,
+ * meshes nx*ny*nz, x fastest), x0 = HOST pointer to the 3 coordinates of the low corner.  Particles are taken in the order
+ * given (no bin ordering: the mesh fits in L2).  outside: optional DEVICE int32; receives 1 when some particle lay outside
+ * [x0, x0 + n dx) (it was skipped), else 0 -- the PM_EDOMAIN of pm_check, without a synchronisation.
+ * Asynchronous on cuda_stream (a cudaStream_t, NULL = the legacy default stream) of `device`; the caller owns every buffer.
+ *
+ * The scratch array is shared by all calls on a device and keeps the last call's contents; every call clears the part it uses
+ * first (stream-ordered).  Calls whose GPU work can overlap -- different streams, different host threads -- RACE on it:
+ * serialise them (one stream, or events).  The first call on a device looks the array's device address up
+ * (cudaGetSymbolAddress, once per device); pm_noalloc_setup(device) does only that, for callers that want it out of the way
+ * before a capture starts.  Errors: PM_EINVAL (arguments, mesh too large), PM_ECUDA; pm_noalloc_last_error() returns the
+ * message of the calling thread's last failing call ("" after a success). */
+#define PM_NOALLOC_MAX_GHOSTED_CELLS 327680
+#define PM_NOALLOC_SCRATCH_BYTES ((PM_NOALLOC_MAX_GHOSTED_CELLS + 32) * 8)
+int pm_noalloc_setup(int device);
+int pm_gravity_deposit_noalloc(int device, void *cuda_stream, int32_t nx, int32_t ny, int32_t nz, const double *x0, double dx,
+                               const double *rho_gas, int64_t n, const double *x, const double *y, const double *z,
+                               const double *m, double *rho_tot, int32_t *outside);
+const char *pm_noalloc_last_error(void);
+
 /* Synchronise the ctx's stream and report PM_ECUDA / PM_EDOMAIN raised by earlier asynchronous work. */
 int pm_check(pm_ctx *ctx);
 

@@ -21,6 +21,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 
 using namespace pm;
@@ -1540,5 +1541,109 @@ extern "C" int pm_probe_red_f64(pm_ctx *c, int64_t footprint_bytes, int32_t chan
     if (e != cudaSuccess) { snprintf(c->msg, sizeof(c->msg), "pm_probe_red_f64: %s", cudaGetErrorString(e)); return PM_ECUDA; }
     const double ops = (double)blocks * 8 * 28 * iters * channels;      // 8 warps per CTA, 28 active lanes
     *gops = ops / (ms * 1e-3) / 1e9;
+    return PM_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// pm_gravity_deposit_noalloc: the PM-gravity mass deposit (Steps 1, 2, 5; L51, L95) for callers that cannot allocate --
+// code under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc.  Same kernels and the same
+// arithmetic as pm_gravity_deposit; the ghost-zoned accumulation mesh (the scratch of Step 1, L59) lives in a file-scope
+// __device__ array instead of a ctx's buffer mesh, so no ctx and no allocation is needed.  Every GPU that loads the library
+// holds the array until the process exits (PM_NOALLOC_SCRATCH_BYTES).
+//
+// In host code the name g_noalloc_scratch is a host-side stand-in, not a device address: the address the kernels get comes
+// from cudaGetSymbolAddress, asked once per device with that device current (noalloc_scratch below).
+//
+// Layout: [0, 32) doubles = 256 bytes of flag words ([0] as int: "a particle lies outside the domain"); then the mesh,
+// (nx + 4)(ny + 2)(nz + 2) doubles (one ghost layer, r_K = dx for cloud-in-cell, R40; x origin rounded to even as in a ctx).
+// All calls share the array and it keeps the last call's contents: every call clears the part it uses first.  Two calls
+// whose work overlaps on the GPU (different streams, different host threads) race on it.
+// ---------------------------------------------------------------------------------------------------------------
+constexpr long long kNoallocFlagDoubles = 32;
+constexpr long long kNoallocMeshMax = PM_NOALLOC_MAX_GHOSTED_CELLS;
+static_assert((kNoallocFlagDoubles + kNoallocMeshMax) * sizeof(double) == PM_NOALLOC_SCRATCH_BYTES, "pm.h states the size of the array");
+static __device__ __align__(256) double g_noalloc_scratch[kNoallocFlagDoubles + kNoallocMeshMax];
+
+constexpr int kNoallocMaxDevices = 64;
+static std::mutex g_noalloc_mu;
+static double *g_noalloc_ptr[kNoallocMaxDevices];       // device address of g_noalloc_scratch, per device; NULL = not asked yet
+static thread_local char g_noalloc_msg[384] = "";
+
+#define NOALLOC_FAIL(code, ...) do { snprintf(g_noalloc_msg, sizeof(g_noalloc_msg), __VA_ARGS__); return (code); } while (0)
+#define NOALLOC_CUDA(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { \
+    snprintf(g_noalloc_msg, sizeof(g_noalloc_msg), "%s failed: %s", #call, cudaGetErrorString(e_)); return PM_ECUDA; } } while (0)
+
+// Set-up, once per device: makes `device` current and asks the runtime where this device keeps g_noalloc_scratch.
+static int noalloc_scratch(int device, double **out) {
+    if (device < 0 || device >= kNoallocMaxDevices) NOALLOC_FAIL(PM_EINVAL, "device %d: the no-alloc entry point serves devices 0..%d", device, kNoallocMaxDevices - 1);
+    NOALLOC_CUDA(cudaSetDevice(device));
+    std::lock_guard<std::mutex> lock(g_noalloc_mu);
+    if (!g_noalloc_ptr[device]) {
+        double *p = nullptr;
+        NOALLOC_CUDA(cudaGetSymbolAddress((void **)&p, g_noalloc_scratch));
+        if (!p) NOALLOC_FAIL(PM_ECUDA, "cudaGetSymbolAddress gave a null address for the scratch array on device %d", device);
+        g_noalloc_ptr[device] = p;
+    }
+    *out = g_noalloc_ptr[device];
+    return PM_OK;
+}
+
+extern "C" const char *pm_noalloc_last_error(void) { return g_noalloc_msg; }
+
+extern "C" int pm_noalloc_setup(int device) {
+    double *p;
+    return noalloc_scratch(device, &p);
+}
+
+extern "C" int pm_gravity_deposit_noalloc(int device, void *cuda_stream, int32_t nx, int32_t ny, int32_t nz, const double *x0,
+                                          double dx, const double *rho_gas, int64_t n, const double *x, const double *y,
+                                          const double *z, const double *m, double *rho_tot, int32_t *outside) {
+    g_noalloc_msg[0] = 0;
+    if (!x0 || !rho_tot || n < 0 || n >= (1ll << 31)) NOALLOC_FAIL(PM_EINVAL, "pm_gravity_deposit_noalloc: null x0 / rho_tot, or a particle count outside [0, 2^31)");
+    if (n > 0 && !(x && y && z && m)) NOALLOC_FAIL(PM_EINVAL, "pm_gravity_deposit_noalloc: null particle array");
+    if (nx < 3 || ny < 3 || nz < 3 || !(dx > 0.0)) NOALLOC_FAIL(PM_EINVAL, "pm_gravity_deposit_noalloc: needs dx > 0 and at least 3 cells per axis (R32 with one ghost layer)");
+    const long long Nb = ((long long)nx + 4) * ((long long)ny + 2) * ((long long)nz + 2);
+    if (Nb > kNoallocMeshMax)
+        NOALLOC_FAIL(PM_EINVAL, "pm_gravity_deposit_noalloc: a mesh of %d x %d x %d cells needs (nx + 4)(ny + 2)(nz + 2) = %lld doubles of scratch; "
+                     "the static array holds PM_NOALLOC_MAX_GHOSTED_CELLS = %lld (cubes up to 66^3 fit); use pm_gravity_deposit on a ctx",
+                     (int)nx, (int)ny, (int)nz, Nb, kNoallocMeshMax);
+    double *scr;
+    int rc;
+    if ((rc = noalloc_scratch(device, &scr)) != PM_OK) return rc;
+    cudaStream_t stream = (cudaStream_t)cuda_stream;
+
+    DevP P;
+    std::memset(&P, 0, sizeof(P));
+    P.nx = nx; P.ny = ny; P.nz = nz;
+    P.g = 1; P.gx = 2;
+    P.pj = nx + 2 * P.gx; P.pk = P.pj * (ny + 2 * P.g);
+    P.N = (long long)nx * ny * nz; P.Nb = Nb;
+    P.dx = dx; P.inv_dx = 1.0 / dx; P.V = dx * dx * dx;
+    for (int a = 0; a < 3; ++a) P.x0[a] = x0[a];
+
+    int *const flag = reinterpret_cast<int *>(scr);
+    double *const mesh = scr + kNoallocFlagDoubles;
+    // Step 1: "all cells initialized to zero" (L59) -- and the flag words: the array still holds the previous call's sums
+    NOALLOC_CUDA(cudaMemsetAsync(scr, 0, (size_t)(kNoallocFlagDoubles + Nb) * sizeof(double), stream));
+    if (n > 0) {
+        k_grav_deposit<<<(unsigned)((n + 255) / 256), 256, 0, stream>>>(P, x, y, z, m, n, nullptr, mesh, flag);
+        NOALLOC_CUDA(cudaGetLastError());
+    }
+    {                                                                                     // Step 2 (Eq. 3), one channel, W = 1 (g odd)
+        const long long g2 = 2 * P.g;
+        const long long n_z = g2 * P.ny * P.nx;
+        const long long n_y = (long long)(P.nz - g2) * g2 * P.nx;
+        const long long n_x = (long long)(P.nz - g2) * (P.ny - g2) * g2;
+        const long long n_edge = n_z + n_y + n_x;
+        k_fold_ghosts<1, 1, false><<<(unsigned)((n_edge + 255) / 256), 256, 0, stream>>>(P, mesh, Tiles{nullptr}, n_edge, n_z, n_y, nullptr, nullptr);
+        NOALLOC_CUDA(cudaGetLastError());
+    }
+    const bool vec = P.nx % 2 == 0 && aligned16(rho_tot) && (!rho_gas || aligned16(rho_gas));      // Step 5 (Eq. 6, eta = 1)
+    const long long work = vec ? P.N / 2 : P.N;
+    const unsigned blocks = (unsigned)((work + 255) / 256);          // at most 1024 CTAs at the maximum mesh
+    if (vec) k_grav_apply<2><<<blocks, 256, 0, stream>>>(P, rho_gas, mesh, rho_tot);
+    else k_grav_apply<1><<<blocks, 256, 0, stream>>>(P, rho_gas, mesh, rho_tot);
+    NOALLOC_CUDA(cudaGetLastError());
+    if (outside) NOALLOC_CUDA(cudaMemcpyAsync(outside, flag, sizeof(int), cudaMemcpyDeviceToDevice, stream));
     return PM_OK;
 }

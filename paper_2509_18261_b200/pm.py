@@ -27,9 +27,10 @@ STATUS_NAMES = {0: "PM_OK", -1: "PM_EINVAL", -2: "PM_ENOMEM", -3: "PM_ECUDA", -4
 EXPORTS = ["pm_create", "pm_deposit", "pm_fold_ghosts", "pm_apply_limited", "pm_return_to_particles", "pm_check",
            "pm_step_host", "pm_step_host_begin", "pm_step_host_end", "pm_destroy", "pm_last_error", "pm_launch_count", "pm_kernel_times", "pm_probe_red_f64", "pm_set_repro_margin", "pm_create_sinks", "pm_gravity_deposit", "pm_gravity_kick", "pm_drift", "pm_slab_describe", "pm_slab_pack", "pm_debug_round_buffers", "pm_debug_buffer", "pm_debug_tile_counts",
            "pm_debug_return_mesh", "pm_debug_lambda", "pm_debug_sink_scalars", "pm_debug_sn_scalars",
-           "pm_debug_stencil"]
+           "pm_debug_stencil", "pm_noalloc_setup", "pm_gravity_deposit_noalloc", "pm_noalloc_last_error"]
 
 c_dp = C.POINTER(C.c_double)
+PM_NOALLOC_MAX_GHOSTED_CELLS = 327680      # include/pm.h
 
 
 class PmParams(C.Structure):
@@ -130,8 +131,12 @@ def lib():
         L.pm_debug_sink_scalars.argtypes = [vp, C.POINTER(vp), i64p]
         L.pm_debug_sn_scalars.argtypes = [vp, C.POINTER(vp), i64p]
         L.pm_debug_stencil.argtypes = [vp, C.c_int, C.c_double, C.c_double, C.c_double, vp, i32p, i32p]
+        L.pm_noalloc_setup.argtypes = [C.c_int]
+        L.pm_gravity_deposit_noalloc.argtypes = [C.c_int, vp, C.c_int32, C.c_int32, C.c_int32, c_dp, C.c_double, vp, C.c_int64] + [vp] * 6
+        L.pm_noalloc_last_error.argtypes = []
+        L.pm_noalloc_last_error.restype = C.c_char_p
         for name in EXPORTS:
-            if name not in ("pm_last_error", "pm_launch_count"):
+            if name not in ("pm_last_error", "pm_launch_count", "pm_noalloc_last_error"):
                 getattr(L, name).restype = C.c_int
         _lib = L
     return _lib
@@ -487,3 +492,35 @@ class Context:
             self.close()
         except Exception:
             pass
+
+
+# ---- the entry point that allocates nothing (include/pm.h) ------------------------------------------------------
+def pm_gravity_deposit_noalloc(params: dict, rho_gas, x, y, z, m, rho_tot, outside=None, stream=None):
+    """rho_tot := rho_gas + CIC deposit of the particle masses, through the static scratch array of the library: no ctx, no
+    allocation.  params: nx, ny, nz, x0, dx.  outside: optional int32 CUDA tensor of one element (1 = a particle lay outside)."""
+    L = lib()
+    dev = rho_tot.device
+    assert dev.type == "cuda", "device tensors only"
+    idx = dev.index if dev.index is not None else 0
+    if stream is None:
+        stream = torch.cuda.current_stream(dev)
+    n = int(x.numel()) if x is not None else 0
+    ncell = params["nx"] * params["ny"] * params["nz"]
+    _ptr(rho_tot, ncell), _ptr(rho_gas, ncell)
+    for t in (x, y, z, m):
+        _ptr(t, n)
+    if outside is not None:
+        assert outside.is_cuda and outside.dtype == torch.int32 and outside.numel() == 1
+    x0 = (C.c_double * 3)(*(float(v) for v in params["x0"]))
+    rc = L.pm_gravity_deposit_noalloc(idx, C.c_void_p(stream.cuda_stream), params["nx"], params["ny"], params["nz"], x0,
+                                      float(params["dx"]), _dptr(rho_gas), n, _dptr(x), _dptr(y), _dptr(z), _dptr(m),
+                                      _dptr(rho_tot), C.c_void_p(outside.data_ptr()) if outside is not None else None)
+    if rc != PM_OK:
+        raise PmError(rc, "pm_gravity_deposit_noalloc", L.pm_noalloc_last_error().decode())
+
+
+def pm_noalloc_setup(device=0):
+    L = lib()
+    rc = L.pm_noalloc_setup(int(device))
+    if rc != PM_OK:
+        raise PmError(rc, "pm_noalloc_setup", L.pm_noalloc_last_error().decode())
