@@ -92,6 +92,10 @@ struct pm_ctx {
     char msg[256];
 };
 
+// tile flags (one byte per tile) followed, 16-byte aligned, by the two `swept` words of Tiles
+static size_t tile_swept_offset(long long ntiles) { return (size_t)((ntiles + 15) & ~15ll); }
+static size_t tile_flag_bytes(long long ntiles) { return tile_swept_offset(ntiles) + 16; }
+
 #define PM_FAIL(ctx, code, ...) do { snprintf((ctx)->msg, sizeof((ctx)->msg), __VA_ARGS__); return (code); } while (0)
 #define PM_CUDA(ctx, call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { \
     snprintf((ctx)->msg, sizeof((ctx)->msg), "%s failed: %s", #call, cudaGetErrorString(e_)); return PM_ECUDA; } } while (0)
@@ -469,7 +473,8 @@ __global__ void __launch_bounds__(256) k_fold_ghosts(const DevP P, double *__res
         img[m] = (slab && cz) ? (long long)pz * P.pk + (long long)(j + cy * oy + P.g) * P.pj + (i + cx * ox + P.gx)
                               : ghost_index(P, i + cx * ox, j + cy * oy, k + cz * oz);
     }
-    if (STAMPS) {
+    if (STAMPS && !(tiles_swept(T, 0) && tiles_swept(T, 1))) {
+        const bool sk = tiles_swept(T, 0), sn = tiles_swept(T, 1);
         lk = 0; ln = 0;
 #pragma unroll
         for (int m = 0; m < 8; ++m) {
@@ -477,8 +482,8 @@ __global__ void __launch_bounds__(256) k_fold_ghosts(const DevP P, double *__res
             if (slab && cz) { if (ok[m]) { lk |= 1u << m; ln |= 1u << m; } continue; }      // received slabs hold values or zeros
             if (m == 0 || ok[m]) {
                 const unsigned f = T.live[tile_index(P, i + cx * ox, j + cy * oy, k + cz * oz)];
-                lk |= (f & kLiveK ? 1u : 0u) << m;
-                ln |= (f & kLiveN ? 1u : 0u) << m;
+                lk |= ((f & kLiveK) || sk ? 1u : 0u) << m;
+                ln |= ((f & kLiveN) || sn ? 1u : 0u) << m;
             }
         }
         if (!((lk | ln) & 1u)) return;
@@ -573,8 +578,9 @@ __global__ void __launch_bounds__(kApplyThreads, 6) k_apply_limited(const DevP P
     const long long q = (long long)row * P.nx + i0 + P.zoff;     // state / return-mesh index (zoff: ghost planes of a z slab)
     const long long gq = (long long)(k + P.g) * P.pk + (long long)(j + P.g) * P.pj + (i0 + P.gx);
     // a stale tile stands for zeros and is not read (pm_tiles.cuh); the VEC cells of an item lie in one tile (i0 is even)
-    const unsigned lf = __ldg(T.live + tile_index(P, (int)i0, (int)j, (int)k));
-    const bool live_k = lf & kLiveK, live_n = lf & kLiveN;
+    const bool sw_k = tiles_swept(T, 0), sw_n = tiles_swept(T, 1);
+    const unsigned lf = (sw_k && sw_n) ? (kLiveK | kLiveN) : __ldg(T.live + tile_index(P, (int)i0, (int)j, (int)k));
+    const bool live_k = sw_k || (lf & kLiveK), live_n = sw_n || (lf & kLiveN);
     double b[kBufChannels][VEC];
 #pragma unroll
     for (int ch = 0; ch < kBufChannels; ++ch) {
@@ -775,9 +781,9 @@ extern "C" int pm_create(const pm_params *prm, int device, void *cuda_stream, pm
     c->repro_M = 28;                                  // the paper's example margin (L612)
     c->nch = c->repro ? kReproChannels : kBufChannels;
     if (e == cudaSuccess) e = cudaMalloc(&c->buf, (size_t)c->nch * P.Nb * sizeof(double));
-    if (e == cudaSuccess) e = cudaMalloc(&c->tile_live, (size_t)c->ntiles);
+    if (e == cudaSuccess) e = cudaMalloc(&c->tile_live, tile_flag_bytes(c->ntiles));
     // before the first deposit every tile is stale = zeros
-    if (e == cudaSuccess) e = cudaMemsetAsync(c->tile_live, 0, (size_t)c->ntiles, c->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(c->tile_live, 0, tile_flag_bytes(c->ntiles), c->stream);
     const long long Nst = N + 2ll * P.zoff;              // cells of a state array / of the return mesh (z ghost planes in slab mode)
     if (e == cudaSuccess && gs > 0) e = cudaMalloc(&c->ret, (size_t)kRetWords * Nst * sizeof(double));
     if (e == cudaSuccess && gs > 0 && P.tl_num > 0.0) e = cudaMalloc(&c->ret_tr, (size_t)Nst * sizeof(double));
@@ -856,7 +862,7 @@ extern "C" int pm_set_repro_margin(pm_ctx *c, int32_t M) {
 extern "C" const char *pm_last_error(const pm_ctx *c) { return c ? c->msg : "null ctx"; }
 extern "C" int64_t pm_launch_count(const pm_ctx *c) { return c ? c->launches : 0; }
 
-static Tiles tiles_of(const pm_ctx *c) { return Tiles{ c->tile_live }; }
+static Tiles tiles_of(const pm_ctx *c) { return Tiles{ c->tile_live, reinterpret_cast<int *>(c->tile_live + tile_swept_offset(c->ntiles)) }; }
 
 static bool state_ok(const pm_state *s) { return s && s->rho && s->mx && s->my && s->mz && s->etot && s->eint; }
 
@@ -921,7 +927,7 @@ extern "C" int pm_deposit(pm_ctx *c, const pm_state *st, const pm_sinks *sk, con
     }
     // a0: reset (L59 "all cells initialized to zero").  The tiles this step's particles can add into are marked live (from the
     // bin occupancy) and zeroed; all others are stale and taken as zeros by the readers (pm_tiles.cuh).
-    if (np == 0 && !P.zopen) PM_CUDA(c, cudaMemsetAsync(c->tile_live, 0, (size_t)c->ntiles, c->stream));
+    if (np == 0 && !P.zopen) PM_CUDA(c, cudaMemsetAsync(c->tile_live, 0, tile_flag_bytes(c->ntiles), c->stream));   // flags and `swept`
     if (np > 0 || P.zopen) {
         const Tiles T = tiles_of(c);
         tick(c, PM_K_ZERO, 0);
@@ -930,7 +936,7 @@ extern "C" int pm_deposit(pm_ctx *c, const pm_state *st, const pm_sinks *sk, con
         const unsigned zblocks = (unsigned)std::min<long long>((c->ntiles + 7) / 8, (long long)c->sm_count * 16);
         k_tiles_zero<<<zblocks, 256, 0, c->stream>>>(P, c->buf, T, c->repro, (int)c->ntiles, live);
         if ((rc = check_launch(c, "k_tiles_zero")) != PM_OK) return rc;
-        k_zero_sweep<<<c->sm_count * 16, 256, 0, c->stream>>>(P, c->buf, c->repro, (int)c->ntiles, live);
+        k_zero_sweep<<<c->sm_count * 16, 256, 0, c->stream>>>(P, c->buf, c->repro, (int)c->ntiles, live, T.swept);
         if ((rc = check_launch(c, "k_zero_sweep")) != PM_OK) return rc;
         tick(c, PM_K_ZERO, 1);
     }
@@ -1635,7 +1641,7 @@ extern "C" int pm_gravity_deposit_noalloc(int device, void *cuda_stream, int32_t
         const long long n_y = (long long)(P.nz - g2) * g2 * P.nx;
         const long long n_x = (long long)(P.nz - g2) * (P.ny - g2) * g2;
         const long long n_edge = n_z + n_y + n_x;
-        k_fold_ghosts<1, 1, false><<<(unsigned)((n_edge + 255) / 256), 256, 0, stream>>>(P, mesh, Tiles{nullptr}, n_edge, n_z, n_y, nullptr, nullptr);
+        k_fold_ghosts<1, 1, false><<<(unsigned)((n_edge + 255) / 256), 256, 0, stream>>>(P, mesh, Tiles{nullptr, nullptr}, n_edge, n_z, n_y, nullptr, nullptr);
         NOALLOC_CUDA(cudaGetLastError());
     }
     const bool vec = P.nx % 2 == 0 && aligned16(rho_tot) && (!rho_gas || aligned16(rho_gas));      // Step 5 (Eq. 6, eta = 1)

@@ -26,7 +26,10 @@ namespace pm {
 constexpr unsigned kLiveK = 1u, kLiveN = 2u;
 struct Tiles {
     unsigned char *live;      // per tile: kLiveK | kLiveN
+    int *swept;               // [2]: 1 when the last reset swept the whole of group K / N (k_zero_sweep): every tile of that group then
+                              // holds zeros or this step's sums, so a reader may take all of them as live without loading the flags
 };
+__device__ __forceinline__ bool tiles_swept(const Tiles &T, int grp) { return __ldg(T.swept + grp) != 0; }
 
 // fp64 atomic addition without return (REDG.E.ADD.F64), the Step 1 accumulation of Eq. 2
 __device__ __forceinline__ void red_add(double *p, double v) {
@@ -140,7 +143,8 @@ __global__ void __launch_bounds__(256) k_tiles_mark(const DevP P, const Tiles T,
 // k_tiles_mark found live (both kernels are always launched; the one that has nothing to do returns at once):
 //   sparse group (fewer than kDenseNum / kDenseDen of the tiles live): k_tiles_zero, one warp per live tile;
 //   dense group: k_zero_sweep, a linear sweep over the group's channels at the store bandwidth of the device (tile by tile,
-//   64-byte row pieces, costs 1.40 ms for the whole mesh of config 5 against 1.03 ms for the sweep).
+//   64-byte row pieces, costs 1.40 ms for the whole mesh of config 5 against 1.03 ms for the sweep).  The sweep also records
+//   that it ran (Tiles::swept): fold and apply then skip the flag loads of that group.
 constexpr int kDenseNum = 3, kDenseDen = 5;
 __device__ __forceinline__ bool group_dense(const int *__restrict__ live, int grp, int ntiles) {
     return (long long)live[grp] * kDenseDen >= (long long)ntiles * kDenseNum;
@@ -175,8 +179,9 @@ __device__ __forceinline__ void zero_range(double *__restrict__ p, long long n, 
 }
 
 __global__ void __launch_bounds__(256) k_zero_sweep(const DevP P, double *__restrict__ buf, const bool repro, const int ntiles,
-                                                    const int *__restrict__ live) {
+                                                    const int *__restrict__ live, int *__restrict__ swept) {
     const bool dk = group_dense(live, 0, ntiles), dn = group_dense(live, 1, ntiles);
+    if (blockIdx.x == 0 && threadIdx.x == 0) { swept[0] = dk; swept[1] = dn; }
     if (!dk && !dn) return;
     const long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x, nth = (long long)gridDim.x * blockDim.x;
     if (dk) zero_range(buf, P.Nb, tid, nth);
