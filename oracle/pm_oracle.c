@@ -23,6 +23,13 @@
  *   - the Eq. 21 fall-back branch (R25: no admissible root => lambda = 0, e_int clipped at 0).
  *
  * Build: gcc -O2 -ffp-contract=off -fPIC -shared -o liboracle_pm.so pm_oracle.c -lm
+ *
+ * The "#pragma omp" lines are inert in that build (no -fopenmp: gcc skips them, the program is the sequential one above and
+ * is the parity reference).  bench.py's all-host-cores timing leg ("all host cores via OpenMP
+ * (omp atomic deposits, parallel cell loops)") compiles this same file a second time with -fopenmp into
+ * liboracle_pm_omp.so; there the particle loops of Steps 1 and 4 and the cell loop of Steps 3 + 5 run on all cores, mesh
+ * additions are "omp atomic", and sums depend on the order of the additions like the GPU's.  That build is timed, never
+ * compared against.
  */
 #ifndef _GNU_SOURCE
 #define _GNU_SOURCE
@@ -459,7 +466,8 @@ int orc_deposit(const orc_params *p, const orc_state *U, orc_sinks *sk, orc_sne 
     zero_mesh(mo->Tp, N); zero_mesh(mo->Te, N);
     if (2 * kernel_halfwidth(p->rk_sink, p->dx) + 1 > p->nx && sk && sk->n > 0) return -2;   /* R32 */
 
-    for (int64_t s = 0; sk && s < sk->n; ++s) {
+    #pragma omp parallel for schedule(dynamic, 16)
+    for (int64_t s = 0; s < (sk ? sk->n : 0); ++s) {
         sink_scalars sc;
         double xs = sk->x[s], ys = sk->y[s], zs = sk->z[s];
         sink_compute_scalars(p, U, xs, ys, zs, sk->vx[s], sk->vy[s], sk->vz[s], sk->m[s], &sc);
@@ -484,13 +492,21 @@ int orc_deposit(const orc_params *p, const orc_state *U, orc_sinks *sk, orc_sne 
                      * a ~ exp(-r^2/r_acc^2) amplifies a relative change of r_acc^2 by r^2/r_acc^2 (up to 16 r_K^2/dx^2) */
                     double cond = 1.0 + r2 / (sc.r_acc * sc.r_acc);
                     for (int f = 0; f < 6; ++f) {
+                        #pragma omp atomic
                         mo->A[f][c] += d[f];
-                        if (mo->Aabs[f]) mo->Aabs[f][c] += fabs(d[f]) * cond;
+                        if (mo->Aabs[f]) {
+                            #pragma omp atomic
+                            mo->Aabs[f][c] += fabs(d[f]) * cond;
+                        }
                     }
-                    if (mo->sink_count) mo->sink_count[c] += 1;
+                    if (mo->sink_count) {
+                        #pragma omp atomic
+                        mo->sink_count[c] += 1;
+                    }
                 }
     }
-    for (int64_t s = 0; sn && s < sn->n; ++s) {
+    #pragma omp parallel for schedule(dynamic, 16)
+    for (int64_t s = 0; s < (sn ? sn->n : 0); ++s) {
         sn_scalars sc;
         double xs = sn->x[s], ys = sn->y[s], zs = sn->z[s];
         sn_compute_scalars(p, U, xs, ys, zs, sn->vx[s], sn->vy[s], sn->vz[s], sn->e_sn[s], sn->m_ej[s], &sc);
@@ -506,13 +522,29 @@ int orc_deposit(const orc_params *p, const orc_state *U, orc_sinks *sk, orc_sne 
                     sn_cell_deposit(p, &sc, xs, ys, zs, sn->e_sn[s], sn->m_ej[s], i, j, k, cnt,
                                     rho, U->mx[c] / rho, U->my[c] / rho, U->mz[c] / rho, d, da, dc);
                     for (int f = 0; f < 5; ++f) {
+                        #pragma omp atomic
                         mo->S[f][c] += d[f];
-                        if (mo->Sabs[f]) mo->Sabs[f][c] += da[f];
-                        if (mo->Scond[f]) mo->Scond[f][c] += dc[f];
+                        if (mo->Sabs[f]) {
+                            #pragma omp atomic
+                            mo->Sabs[f][c] += da[f];
+                        }
+                        if (mo->Scond[f]) {
+                            #pragma omp atomic
+                            mo->Scond[f][c] += dc[f];
+                        }
                     }
-                    if (mo->Tp) mo->Tp[c] += (fabs(d[1]) + fabs(d[2])) + fabs(d[3]);
-                    if (mo->Te) mo->Te[c] += fabs(d[4]);
-                    if (mo->sn_count) mo->sn_count[c] += 1;
+                    if (mo->Tp) {
+                        #pragma omp atomic
+                        mo->Tp[c] += (fabs(d[1]) + fabs(d[2])) + fabs(d[3]);
+                    }
+                    if (mo->Te) {
+                        #pragma omp atomic
+                        mo->Te[c] += fabs(d[4]);
+                    }
+                    if (mo->sn_count) {
+                        #pragma omp atomic
+                        mo->sn_count[c] += 1;
+                    }
                 }
     }
     return 0;
@@ -583,6 +615,7 @@ int orc_repro_buffers(const orc_params *p, const orc_state *U, orc_mesh_out *mo,
 /* Steps 3+5 (O7) on every cell, in place; sn_touched[c] != 0 marks cells with an SN contribution. */
 int orc_apply(const orc_params *p, orc_state *U, const orc_mesh_out *mo, const int32_t *sn_touched) {
     const int64_t N = (int64_t)p->nx * p->ny * p->nz;
+    #pragma omp parallel for schedule(static)
     for (int64_t c = 0; c < N; ++c) {
         double u[6] = { U->rho[c], U->mx[c], U->my[c], U->mz[c], U->etot[c], U->eint[c] };
         double A[6], S[5];
@@ -600,6 +633,7 @@ int orc_apply(const orc_params *p, orc_state *U, const orc_mesh_out *mo, const i
 /* Step 4 (O8, Eq. 5) with the deposition function re-evaluated from the PRE-step state U_old (L79; R15). */
 int orc_return(const orc_params *p, const orc_state *U_old, const double *eta, orc_sinks *sk, double dt) {
     const double V = p->dx * p->dx * p->dx;
+    #pragma omp parallel for schedule(dynamic, 16)
     for (int64_t s = 0; s < sk->n; ++s) {
         sink_scalars sc;
         double xs = sk->x[s], ys = sk->y[s], zs = sk->z[s];
@@ -834,3 +868,11 @@ int64_t orc_create_sinks(const orc_params *p, orc_state *U, const double *a0, in
 }
 
 int32_t orc_sizeof_params(void) { return (int32_t)sizeof(orc_params); }
+
+/* threads the timed all-cores build uses (1 in the plain build) */
+#ifdef _OPENMP
+#include <omp.h>
+int32_t orc_threads(void) { return (int32_t)omp_get_max_threads(); }
+#else
+int32_t orc_threads(void) { return 1; }
+#endif

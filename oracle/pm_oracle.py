@@ -16,8 +16,10 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "pm_oracle.c")
 _LIB = os.path.join(_HERE, "liboracle_pm.so")
+_LIB_OMP = os.path.join(_HERE, "liboracle_pm_omp.so")     # the same source with -fopenmp: bench.py's all-cores timing leg only
 _lock = threading.Lock()
 _lib = None
+_lib_omp = None
 
 c_dp = C.POINTER(C.c_double)
 c_ip = C.POINTER(C.c_int32)
@@ -73,6 +75,32 @@ def build(force: bool = False) -> str:
             cmd = ["gcc", "-O2", "-ffp-contract=off", "-fPIC", "-shared", "-o", _LIB, _SRC, "-lm"]
             subprocess.check_call(cmd)
     return _LIB
+
+
+def build_omp(force: bool = False) -> str:
+    """The same file compiled with -fopenmp: timed by bench.py on all host cores, never compared
+    against -- its sums depend on the order of the atomic additions."""
+    with _lock:
+        stale = (not os.path.exists(_LIB_OMP)) or os.path.getmtime(_LIB_OMP) < os.path.getmtime(_SRC)
+        if force or stale:
+            subprocess.check_call(["gcc", "-O2", "-ffp-contract=off", "-fopenmp", "-fPIC", "-shared", "-o", _LIB_OMP, _SRC, "-lm"])
+    return _LIB_OMP
+
+
+def lib_omp():
+    """The OpenMP build; only orc_step and orc_threads are called on it."""
+    global _lib_omp
+    if _lib_omp is None:
+        build_omp()
+        L = C.CDLL(_LIB_OMP)
+        L.orc_sizeof_params.restype = C.c_int32
+        assert L.orc_sizeof_params() == C.sizeof(OrcParams), "orc_params layout mismatch"
+        L.orc_threads.restype = C.c_int32
+        L.orc_step.restype = C.c_int
+        L.orc_step.argtypes = [C.POINTER(OrcParams), C.POINTER(OrcState), C.POINTER(OrcSinks), C.POINTER(OrcSNe),
+                               C.c_double, C.POINTER(OrcMeshOut), c_dp]
+        _lib_omp = L
+    return _lib_omp
 
 
 def lib():
@@ -159,10 +187,12 @@ SN_DIAG = ("m_snr", "v_snr", "vcx", "vcy", "vcz", "n_h", "r_m", "p_rad")
 class Oracle:
     """Holds one problem (params, state, particles; all numpy, modified in place by step())."""
 
-    def __init__(self, params: dict, state, sinks, sne, keep_abs: bool = True, mesh: bool = True, abs_channels=None):
+    def __init__(self, params: dict, state, sinks, sne, keep_abs: bool = True, mesh: bool = True, abs_channels=None,
+                 omp: bool = False):
         """abs_channels = (accretion channels, SN channels) whose error-scale meshes (Aabs, Sabs) are kept; None: all of them
-        (with keep_abs) -- a 512^3 run keeps only the ones its comparisons read."""
-        self.L = lib()
+        (with keep_abs) -- a 512^3 run keeps only the ones its comparisons read.  omp=True: the OpenMP build (step() only;
+        for timing, not for comparisons)."""
+        self.L = lib_omp() if omp else lib()
         self.pd = dict(params)
         self.p = make_params(params)
         self.state, self.sinks, self.sne = state, sinks, sne

@@ -61,3 +61,34 @@ def test_algorithmic_bytes_dense_limits():
     assert b0["apply"] == 0.0 and b0["sne"] == 0.0 and b0["sinks"] == 0.0 and b0["zero"] == 0.0
     # SN deposit at config 5's probed cell fraction (T_SN ~ 0.48): ~2.1 GB, not the 6.4 GB of round 1's line
     assert 2.0e9 < bench.algorithmic_bytes(N, Nb, 10 ** 5, 9 * 10 ** 5, 0.55, 0.12, 0.48)["sne"] < 2.2e9
+
+
+def test_openmp_build_of_the_oracle_is_the_same_program():
+    """bench.py's all-cores leg times oracle/pm_oracle.c compiled with -fopenmp.  The pragmas must
+    not change what is computed: on a small mixed workload the two builds agree to the reorder tolerance (the OpenMP build's
+    sums depend on the order of its atomic additions), conserve the same totals, and the plain build -- the parity reference --
+    stays deterministic."""
+    import hashlib
+
+    import numpy as np
+
+    from oracle import pm_oracle as po
+    from paper_2509_18261_b200 import inputs
+
+    def run(omp):
+        w = inputs.scaled_mixed(40, 800, seed_index=5)
+        o = po.Oracle(w.params, w.state, w.sinks, w.sne, keep_abs=False, omp=omp)
+        for _ in range(2):
+            o.step(w.dt)
+        return w
+
+    a, b, c = run(False), run(False), run(True)
+    digest = lambda w: hashlib.sha256(b"".join(getattr(w.state, f).tobytes() for f in w.state.FIELDS)).hexdigest()
+    assert digest(a) == digest(b), "the plain build must not depend on anything but its inputs"
+    assert po.lib_omp().orc_threads() >= 1 and po.lib().orc_threads() == 1
+    for f in a.state.FIELDS:
+        x, y = getattr(a.state, f), getattr(c.state, f)
+        scale = np.abs(x).max()
+        assert np.all(np.abs(x - y) <= 1e-9 * np.abs(x) + 1e-12 * scale), f
+    assert abs(a.state.rho.sum() - c.state.rho.sum()) <= 1e-12 * a.state.rho.sum()
+    assert np.allclose(a.sinks.m, c.sinks.m, rtol=1e-11, atol=0)
