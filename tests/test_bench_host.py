@@ -63,32 +63,51 @@ def test_algorithmic_bytes_dense_limits():
     assert 2.0e9 < bench.algorithmic_bytes(N, Nb, 10 ** 5, 9 * 10 ** 5, 0.55, 0.12, 0.48)["sne"] < 2.2e9
 
 
-def test_openmp_build_of_the_oracle_is_the_same_program():
+_OMP_SCRIPT = """
+import sys
+import numpy as np
+sys.path.insert(0, {root!r})
+from oracle import pm_oracle as po
+from paper_2509_18261_b200 import inputs
+w = inputs.scaled_mixed(40, 800, seed_index=5)
+o = po.Oracle(w.params, w.state, w.sinks, w.sne, keep_abs=False, omp=True)
+for _ in range(2):
+    o.step(w.dt)
+np.savez({out!r}, threads=po.lib_omp().orc_threads(), m=w.sinks.m, **{{f: getattr(w.state, f) for f in w.state.FIELDS}})
+"""
+
+
+def test_openmp_build_of_the_oracle_is_the_same_program(tmp_path):
     """bench.py's all-cores leg times oracle/pm_oracle.c compiled with -fopenmp.  The pragmas must
     not change what is computed: on a small mixed workload the two builds agree to the reorder tolerance (the OpenMP build's
     sums depend on the order of its atomic additions), conserve the same totals, and the plain build -- the parity reference --
-    stays deterministic."""
+    stays deterministic.  The OpenMP build runs in a process of its own, so that this one stays single-threaded for the
+    tests that fork."""
     import hashlib
+    import subprocess
 
     import numpy as np
 
     from oracle import pm_oracle as po
     from paper_2509_18261_b200 import inputs
 
-    def run(omp):
+    def run():
         w = inputs.scaled_mixed(40, 800, seed_index=5)
-        o = po.Oracle(w.params, w.state, w.sinks, w.sne, keep_abs=False, omp=omp)
+        o = po.Oracle(w.params, w.state, w.sinks, w.sne, keep_abs=False)
         for _ in range(2):
             o.step(w.dt)
         return w
 
-    a, b, c = run(False), run(False), run(True)
+    a, b = run(), run()
     digest = lambda w: hashlib.sha256(b"".join(getattr(w.state, f).tobytes() for f in w.state.FIELDS)).hexdigest()
     assert digest(a) == digest(b), "the plain build must not depend on anything but its inputs"
-    assert po.lib_omp().orc_threads() >= 1 and po.lib().orc_threads() == 1
+    assert po.lib().orc_threads() == 1
+    out = str(tmp_path / "omp.npz")
+    subprocess.check_call([sys.executable, "-c", _OMP_SCRIPT.format(root=ROOT, out=out)])
+    c = np.load(out)
+    assert int(c["threads"]) >= 1
     for f in a.state.FIELDS:
-        x, y = getattr(a.state, f), getattr(c.state, f)
-        scale = np.abs(x).max()
-        assert np.all(np.abs(x - y) <= 1e-9 * np.abs(x) + 1e-12 * scale), f
-    assert abs(a.state.rho.sum() - c.state.rho.sum()) <= 1e-12 * a.state.rho.sum()
-    assert np.allclose(a.sinks.m, c.sinks.m, rtol=1e-11, atol=0)
+        x, y = getattr(a.state, f), c[f]
+        assert np.all(np.abs(x - y) <= 1e-9 * np.abs(x) + 1e-12 * np.abs(x).max()), f
+    assert abs(a.state.rho.sum() - c["rho"].sum()) <= 1e-12 * a.state.rho.sum()
+    assert np.allclose(a.sinks.m, c["m"], rtol=1e-11, atol=0)
