@@ -199,7 +199,7 @@ def algorithmic_bytes(N, Nb, nk, nn, t, ts, tn, fk=1.0, fn=1.0, nch=6):
 def run_sharded(args, rank, world, local_rank):
     """--sharded: the z-slab decomposition of SURVEY.md 8(f)4.  Rank r holds the planes [n r, n (r + 1)) of a periodic
     n x n x (n world) domain with its own config-5-shaped particle set (weak scaling); a step is the state halo exchange,
-    pm_deposit, pm_slab_pack, the exchange of the buffer's z ghost planes (Eq. 3), pm_fold_ghosts, pm_apply_limited, the
+    pm_deposit, pm_slab_put (or pm_slab_pack + messages), i.e. the exchange of the buffer's z ghost planes (Eq. 3), pm_fold_ghosts, pm_apply_limited, the
     owner -> ghost copy of the return mesh (R16) and pm_return_to_particles.  With one rank the exchanges are copies onto the
     rank itself and the result is the periodic single-domain step.  Same timing rules as the default arm."""
     import numpy as np
@@ -228,7 +228,7 @@ def run_sharded(args, rank, world, local_rank):
 
     def make_ctx(flags):
         c = pm.Context(params, device=str(dev), flags=flags)
-        return c, sharded.SlabStep(c, rank, world)
+        return c, sharded.SlabStep(c, rank, world, peer_put=not args.sharded_messages)
 
     ctx, stepper = make_ctx(0)
     g = ctx.ghost_width()
@@ -303,7 +303,7 @@ def run_sharded(args, rank, world, local_rank):
                 "steps": args.steps, "warmup": warm, "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": None, "dtype": "f64", "data": "synthetic",
                 "config": {"workload": f"config5-shaped {n}^3 slab per rank, z-slab decomposition over {world} rank(s) (--sharded)",
-                           "cells_per_rank": N, "particles_per_rank": npart, "multi_gpu": "z slabs, nearest-neighbour exchange of ghost planes",
+                           "cells_per_rank": N, "particles_per_rank": npart, "multi_gpu": "z slabs, nearest-neighbour exchange of ghost planes: " + ("NCCL point-to-point messages" if args.sharded_messages else "the pack kernel stores into the neighbours' receive slabs through peer memory (CUDA IPC; one host barrier per step)"),
                            "exchange_bytes_per_rank_per_step": xbytes, "l2_policy": "inputs larger than L2"},
                 "particles_per_s": world * npart * args.steps / (total_ms * 1e-3), "kernel_ms": kernel_ms, "clocks": clocks,
                 "e2e": {"value": world * N / e2e_s / 1e6, "unit": UNIT, "h2d_bytes_per_step": 6 * N * 8 + (7 * w.sinks.n + 8 * w.sne.n) * 8,
@@ -634,6 +634,10 @@ def main():
     ap.add_argument("--sharded", action="store_true",
                     help="z-slab decomposition (SURVEY 8(f)4): every rank holds one n^3 slab of an n x n x (n world) domain and "
                          "exchanges ghost planes with its z neighbours; default (without the flag): independent replicas")
+    ap.add_argument("--sharded-messages", action="store_true",
+                    help="with --sharded: send the buffer's ghost planes as NCCL point-to-point messages (pm_slab_pack + send/recv) "
+                         "instead of the default, the pack kernel storing them into the neighbours' receive slabs through peer memory "
+                         "(pm_slab_put)")
     ap.add_argument("--reproducible", action="store_true",
                     help="Appendix A mode (PM_FLAG_REPRODUCIBLE): 4 more buffer channels + rounding pass; a separate workload variant")
     args = ap.parse_args()

@@ -173,6 +173,29 @@ int pm_slab_describe(pm_ctx *ctx, pm_slab_desc *out);
 /* After pm_deposit: fill buf_send_lo / buf_send_hi from the buffer mesh's z ghost planes (stale tiles as zeros). */
 int pm_slab_pack(pm_ctx *ctx);
 
+/* Peer-memory form of the Step 2 exchange: compute step and transfer in ONE kernel.  pm_slab_put replaces "pm_slab_pack, then
+ * send / receive": the pack kernel stores this rank's low z ghost planes straight into the LOWER neighbour's receive slab and
+ * its high ones into the UPPER neighbour's, through peer-mapped device memory (NVLink / NVSwitch between GPUs of a node; plain
+ * device memory when both ranks share a GPU or a rank is its own neighbour).  No staging copy, no library collective.
+ *   set-up, once:  every rank calls pm_slab_ipc_export (a 64-byte CUDA IPC handle of its slab memory), the handles travel by any
+ *                  host channel (torch.distributed.all_gather_object in sharded.py), and every rank calls pm_slab_connect_ipc with
+ *                  its two neighbours' handles (NULL = this ctx is its own neighbour on that side; with two ranks both handles are
+ *                  the same peer's and it is opened once).  Neighbours that live in the SAME process (several ctxs, one process)
+ *                  are connected with pm_slab_connect_local instead (CUDA IPC handles cannot be opened by their own process).
+ *   every step:    pm_deposit -> pm_slab_put -> [all ranks: synchronise the ctx's stream, then a host barrier: every put has
+ *                  landed] -> pm_fold_ghosts -> ... as above.
+ * The receive slabs exist twice and pm_slab_put alternates between the two sets, so a put of step n + 1 never lands in memory
+ * the neighbour's fold of step n may still be reading, and ONE barrier per step suffices: a rank leaves the barrier of step n + 1
+ * only after its stream, and with it its fold of step n, has drained.  All ranks must call pm_slab_put in every step of a run
+ * (the sets alternate in lock step); pm_slab_pack steps (which use set 0) may not be mixed in between.
+ * Errors: PM_EORDER (not connected; not directly after pm_deposit), PM_EINVAL (not a slab ctx; neighbour of another shape),
+ * PM_ECUDA (IPC: the peer's GPU is not peer-accessible from this one). */
+#define PM_IPC_HANDLE_BYTES 64
+int pm_slab_ipc_export(pm_ctx *ctx, void *handle /* HOST, PM_IPC_HANDLE_BYTES */, int64_t *slab_bytes /* HOST, optional: bytes of one slab */);
+int pm_slab_connect_ipc(pm_ctx *ctx, const void *handle_lower, const void *handle_upper);
+int pm_slab_connect_local(pm_ctx *ctx, pm_ctx *lower, pm_ctx *upper);      /* NULL = ctx itself */
+int pm_slab_put(pm_ctx *ctx);
+
 /* Margin M of Appendix A (N_bit = log2 r + 52 + M; default 28, the paper's example, L612).  Needs PM_FLAG_REPRODUCIBLE. */
 int pm_set_repro_margin(pm_ctx *ctx, int32_t M);
 

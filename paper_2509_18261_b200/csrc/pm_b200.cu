@@ -34,6 +34,9 @@ constexpr size_t kSnDenseSmem = (size_t)5 * kAccCells * sizeof(double) + (size_t
 // ---------------------------------------------------------------------------------------------------------------
 // context
 // ---------------------------------------------------------------------------------------------------------------
+// slab memory of a z-slab ctx: send_lo | send_hi | recv_lo | recv_hi | recv_lo' | recv_hi' (the primed pair: odd pm_slab_put steps)
+constexpr int kSlabParts = 6;
+
 enum Stage { ST_IDLE = 0, ST_DEPOSITED = 1, ST_FOLDED = 2, ST_APPLIED = 3 };
 
 struct pm_ctx {
@@ -81,7 +84,15 @@ struct pm_ctx {
     bool ever_deposited;
     double *slab_mem;   // z-slab mode: send_lo | send_hi | recv_lo | recv_hi, each nch * g * pk doubles (pm_slab.cuh)
     long long slab_elems;   // doubles per slab
-    bool slab_packed;   // pm_slab_pack has run since the last pm_deposit
+    bool slab_packed;   // pm_slab_pack / pm_slab_put has run since the last pm_deposit
+    // peer-memory form of the exchange (pm_slab_put): where this rank's two slabs go -- the lower neighbour's recv_hi and the
+    // upper neighbour's recv_lo, one pair per step parity (two receive-slab sets, so that a put of step n + 1 never lands in
+    // memory the neighbour's fold of step n still reads)
+    double *put_lo[2], *put_hi[2];
+    void *ipc_base[2];  // bases opened with cudaIpcOpenMemHandle (closed by pm_destroy); NULL when the neighbour is in-process
+    bool peers_set;
+    bool put_step;      // this step's slabs travelled by pm_slab_put: the fold reads the receive set of put_parity
+    int put_parity;
     bool dense_smem_ok; // the device grants the dense SN kernel its shared memory (tile accumulator, 150 KB)
     bool grav_in_ch1;   // buffer channel 1 holds the last pm_gravity_deposit (until the next pm_deposit): the debug view must not
                         // "fill in" its stale tiles
@@ -789,8 +800,8 @@ extern "C" int pm_create(const pm_params *prm, int device, void *cuda_stream, pm
     if (e == cudaSuccess && gs > 0 && P.tl_num > 0.0) e = cudaMalloc(&c->ret_tr, (size_t)Nst * sizeof(double));
     if (e == cudaSuccess && P.zopen) {
         c->slab_elems = (long long)c->nch * g * P.pk;
-        e = cudaMalloc(&c->slab_mem, (size_t)4 * c->slab_elems * sizeof(double));
-        if (e == cudaSuccess) e = cudaMemsetAsync(c->slab_mem, 0, (size_t)4 * c->slab_elems * sizeof(double), c->stream);
+        e = cudaMalloc(&c->slab_mem, (size_t)kSlabParts * c->slab_elems * sizeof(double));
+        if (e == cudaSuccess) e = cudaMemsetAsync(c->slab_mem, 0, (size_t)kSlabParts * c->slab_elems * sizeof(double), c->stream);
     }
     if (e == cudaSuccess && (prm->flags & PM_FLAG_DEBUG_LAMBDA)) e = cudaMalloc(&c->lam, (size_t)N * sizeof(double));
     if (e == cudaSuccess) e = cudaMalloc(&c->err_flag, sizeof(int));
@@ -843,6 +854,7 @@ extern "C" int pm_destroy(pm_ctx *c) {
     if (c->bin_mem) cudaFree(c->bin_mem);
     if (c->grav_mem) cudaFree(c->grav_mem);
     if (c->tile_live) cudaFree(c->tile_live);
+    for (int k = 0; k < 2; ++k) if (c->ipc_base[k] && !(k == 1 && c->ipc_base[1] == c->ipc_base[0])) cudaIpcCloseMemHandle(c->ipc_base[k]);
     if (c->slab_mem) cudaFree(c->slab_mem);
     if (c->create_mem) cudaFree(c->create_mem);
     if (c->err_flag) cudaFree(c->err_flag);
@@ -982,6 +994,7 @@ extern "C" int pm_deposit(pm_ctx *c, const pm_state *st, const pm_sinks *sk, con
     c->ever_deposited = true;
     c->grav_in_ch1 = false;
     c->slab_packed = false;
+    c->put_step = false;
     c->stage = ST_DEPOSITED;
     c->buffer_valid = false;              // unfolded until pm_fold_ghosts
     return PM_OK;
@@ -1002,7 +1015,8 @@ extern "C" int pm_fold_ghosts(pm_ctx *c) {
     tick(c, PM_K_FOLD, 0);
     const Tiles T = tiles_of(c);
     if (P.zopen && !c->slab_packed) PM_FAIL(c, PM_EORDER, "pm_fold_ghosts (z slab): pm_slab_pack and the exchange of the slabs come first");
-    const double *rlo = P.zopen ? c->slab_mem + 2 * c->slab_elems : nullptr, *rhi = P.zopen ? c->slab_mem + 3 * c->slab_elems : nullptr;
+    const int rset = (P.zopen && c->put_step) ? 2 * c->put_parity : 0;
+    const double *rlo = P.zopen ? c->slab_mem + (2 + rset) * c->slab_elems : nullptr, *rhi = P.zopen ? c->slab_mem + (3 + rset) * c->slab_elems : nullptr;
     if (c->repro) {
         if (W == 2) k_fold_ghosts<2, kReproChannels, true><<<blocks, 256, 0, c->stream>>>(P, c->buf, T, n_edge, n_z, n_y, rlo, rhi);
         else k_fold_ghosts<1, kReproChannels, true><<<blocks, 256, 0, c->stream>>>(P, c->buf, T, n_edge, n_z, n_y, rlo, rhi);
@@ -1120,6 +1134,97 @@ extern "C" int pm_slab_pack(pm_ctx *c) {
     int rc = check_launch(c, "k_slab_pack");
     if (rc != PM_OK) return rc;
     c->slab_packed = true;
+    return PM_OK;
+}
+
+// ---- peer-memory form of the Step 2 exchange: pack + put in one kernel -----------------------------------------------------
+static void slab_set_peers(pm_ctx *c, double *base_lower, double *base_upper) {
+    for (int p = 0; p < 2; ++p) {
+        c->put_lo[p] = base_lower + (3 + 2 * p) * c->slab_elems;      // my low ghost planes -> the lower neighbour's recv_hi
+        c->put_hi[p] = base_upper + (2 + 2 * p) * c->slab_elems;      // my high ghost planes -> the upper neighbour's recv_lo
+    }
+    c->peers_set = true;
+    c->put_parity = 1;                                                 // the first put toggles it to 0
+}
+
+static int slab_close_ipc(pm_ctx *c) {
+    for (int k = 0; k < 2; ++k)
+        if (c->ipc_base[k]) {
+            if (k == 1 && c->ipc_base[1] == c->ipc_base[0]) { c->ipc_base[1] = nullptr; continue; }
+            PM_CUDA(c, cudaIpcCloseMemHandle(c->ipc_base[k]));
+            c->ipc_base[k] = nullptr;
+        }
+    return PM_OK;
+}
+
+extern "C" int pm_slab_connect_local(pm_ctx *c, pm_ctx *lower, pm_ctx *upper) {
+    if (!c) return PM_EINVAL;
+    if (!c->P.zopen) PM_FAIL(c, PM_EINVAL, "pm_slab_connect_local: the ctx was not created with z_slab = 1");
+    if (!lower) lower = c;
+    if (!upper) upper = c;
+    for (pm_ctx *o : { lower, upper })
+        if (!o->P.zopen || o->slab_elems != c->slab_elems)
+            PM_FAIL(c, PM_EINVAL, "pm_slab_connect_local: the neighbour's slabs have another shape (nx, ny, ghost width and channel count must agree)");
+    int rc = slab_close_ipc(c);
+    if (rc != PM_OK) return rc;
+    slab_set_peers(c, lower->slab_mem, upper->slab_mem);
+    return PM_OK;
+}
+
+extern "C" int pm_slab_ipc_export(pm_ctx *c, void *handle, int64_t *slab_bytes) {
+    if (!c) return PM_EINVAL;
+    if (!handle) PM_FAIL(c, PM_EINVAL, "pm_slab_ipc_export: null handle buffer");
+    if (!c->P.zopen) PM_FAIL(c, PM_EINVAL, "pm_slab_ipc_export: the ctx was not created with z_slab = 1");
+    static_assert(sizeof(cudaIpcMemHandle_t) == PM_IPC_HANDLE_BYTES, "pm.h states the size of an IPC handle");
+    PM_CUDA(c, cudaSetDevice(c->device));
+    cudaIpcMemHandle_t h;
+    PM_CUDA(c, cudaIpcGetMemHandle(&h, c->slab_mem));
+    std::memcpy(handle, &h, sizeof(h));
+    if (slab_bytes) *slab_bytes = c->slab_elems * (int64_t)sizeof(double);
+    return PM_OK;
+}
+
+extern "C" int pm_slab_connect_ipc(pm_ctx *c, const void *handle_lower, const void *handle_upper) {
+    if (!c) return PM_EINVAL;
+    if (!c->P.zopen) PM_FAIL(c, PM_EINVAL, "pm_slab_connect_ipc: the ctx was not created with z_slab = 1");
+    PM_CUDA(c, cudaSetDevice(c->device));
+    int rc = slab_close_ipc(c);
+    if (rc != PM_OK) return rc;
+    double *base[2] = { c->slab_mem, c->slab_mem };                   // NULL handle: this ctx is its own neighbour on that side
+    const void *hs[2] = { handle_lower, handle_upper };
+    for (int k = 0; k < 2; ++k) {
+        if (!hs[k]) continue;
+        if (k == 1 && hs[0] && std::memcmp(hs[0], hs[1], PM_IPC_HANDLE_BYTES) == 0) {     // two ranks: both neighbours are the same peer
+            c->ipc_base[1] = c->ipc_base[0]; base[1] = base[0];
+            continue;
+        }
+        cudaIpcMemHandle_t h;
+        std::memcpy(&h, hs[k], sizeof(h));
+        void *ptr = nullptr;
+        PM_CUDA(c, cudaIpcOpenMemHandle(&ptr, h, cudaIpcMemLazyEnablePeerAccess));
+        c->ipc_base[k] = ptr; base[k] = static_cast<double *>(ptr);
+    }
+    slab_set_peers(c, base[0], base[1]);
+    return PM_OK;
+}
+
+extern "C" int pm_slab_put(pm_ctx *c) {
+    if (!c) return PM_EINVAL;
+    if (!c->P.zopen) PM_FAIL(c, PM_EINVAL, "pm_slab_put: the ctx was not created with z_slab = 1");
+    if (!c->peers_set) PM_FAIL(c, PM_EORDER, "pm_slab_put: connect the neighbours first (pm_slab_connect_ipc / pm_slab_connect_local)");
+    if (c->stage != ST_DEPOSITED || c->slab_packed) PM_FAIL(c, PM_EORDER, "pm_slab_put must follow pm_deposit (once)");
+    PM_CUDA(c, cudaSetDevice(c->device));
+    const DevP &P = c->P;
+    const long long n = 2ll * P.g * P.pk;
+    const unsigned blocks = (unsigned)((n + 255) / 256);
+    c->put_parity ^= 1;
+    double *lo = c->put_lo[c->put_parity], *hi = c->put_hi[c->put_parity];
+    if (c->repro) k_slab_pack<kReproChannels><<<blocks, 256, 0, c->stream>>>(P, c->buf, tiles_of(c), lo, hi);
+    else k_slab_pack<kBufChannels><<<blocks, 256, 0, c->stream>>>(P, c->buf, tiles_of(c), lo, hi);
+    int rc = check_launch(c, "k_slab_pack (put)");
+    if (rc != PM_OK) return rc;
+    c->slab_packed = true;
+    c->put_step = true;
     return PM_OK;
 }
 

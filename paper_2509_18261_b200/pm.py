@@ -27,7 +27,7 @@ STATUS_NAMES = {0: "PM_OK", -1: "PM_EINVAL", -2: "PM_ENOMEM", -3: "PM_ECUDA", -4
 EXPORTS = ["pm_create", "pm_deposit", "pm_fold_ghosts", "pm_apply_limited", "pm_return_to_particles", "pm_check",
            "pm_step_host", "pm_step_host_begin", "pm_step_host_end", "pm_destroy", "pm_last_error", "pm_launch_count", "pm_kernel_times", "pm_probe_red_f64", "pm_set_repro_margin", "pm_create_sinks", "pm_gravity_deposit", "pm_gravity_kick", "pm_drift", "pm_slab_describe", "pm_slab_pack", "pm_debug_round_buffers", "pm_debug_buffer", "pm_debug_tile_counts",
            "pm_debug_return_mesh", "pm_debug_lambda", "pm_debug_sink_scalars", "pm_debug_sn_scalars",
-           "pm_debug_stencil", "pm_noalloc_setup", "pm_gravity_deposit_noalloc", "pm_noalloc_last_error"]
+           "pm_debug_stencil", "pm_slab_ipc_export", "pm_slab_connect_ipc", "pm_slab_connect_local", "pm_slab_put", "pm_noalloc_setup", "pm_gravity_deposit_noalloc", "pm_noalloc_last_error"]
 
 c_dp = C.POINTER(C.c_double)
 PM_NOALLOC_MAX_GHOSTED_CELLS = 327680      # include/pm.h
@@ -126,6 +126,10 @@ def lib():
         L.pm_debug_tile_counts.argtypes = [vp, i64p, i64p, i64p]
         L.pm_slab_describe.argtypes = [vp, C.POINTER(PmSlabDesc)]
         L.pm_slab_pack.argtypes = [vp]
+        L.pm_slab_put.argtypes = [vp]
+        L.pm_slab_ipc_export.argtypes = [vp, C.c_char_p, i64p]
+        L.pm_slab_connect_ipc.argtypes = [vp, C.c_char_p, C.c_char_p]
+        L.pm_slab_connect_local.argtypes = [vp, vp, vp]
         L.pm_debug_return_mesh.argtypes = [vp, C.c_int, C.POINTER(vp)]
         L.pm_debug_lambda.argtypes = [vp, C.POINTER(vp)]
         L.pm_debug_sink_scalars.argtypes = [vp, C.POINTER(vp), i64p]
@@ -291,6 +295,25 @@ class Context:
     # ---- z-slab decomposition -------------------------------------------------------
     def pm_slab_pack(self):
         self._chk(self.L.pm_slab_pack(self.h), "pm_slab_pack")
+
+    def pm_slab_put(self):
+        """Pack + put: this rank's z ghost planes go straight into the neighbours' receive slabs (peer memory)."""
+        self._chk(self.L.pm_slab_put(self.h), "pm_slab_put")
+
+    def pm_slab_ipc_export(self) -> bytes:
+        """The 64-byte CUDA IPC handle of this ctx's slab memory, to be handed to the two neighbours."""
+        buf = C.create_string_buffer(64)
+        self._chk(self.L.pm_slab_ipc_export(self.h, buf, None), "pm_slab_ipc_export")
+        return buf.raw
+
+    def pm_slab_connect_ipc(self, handle_lower, handle_upper):
+        """Neighbours in other processes (handles from their pm_slab_ipc_export); None = this ctx is its own neighbour there."""
+        self._chk(self.L.pm_slab_connect_ipc(self.h, handle_lower, handle_upper), "pm_slab_connect_ipc")
+
+    def pm_slab_connect_local(self, lower=None, upper=None):
+        """Neighbours in this process (other Context objects); None = this ctx itself."""
+        self._chk(self.L.pm_slab_connect_local(self.h, lower.h if lower is not None else None, upper.h if upper is not None else None),
+                  "pm_slab_connect_local")
 
     def pm_slab_describe(self) -> dict:
         """Device tensors (views of ctx-owned memory) of the slab messages: buf / ret / rtr x send_lo, send_hi, recv_lo, recv_hi."""

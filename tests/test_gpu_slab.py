@@ -43,8 +43,9 @@ def pick(prt, sel, cls, names, shift_z=0.0):
 class Pair:
     """Two slab contexts on one GPU and the copies between them (rank 0: planes [0, h), rank 1: planes [h, n))."""
 
-    def __init__(self, w, flags=pm.PM_FLAG_DEBUG_SCALARS | pm.PM_FLAG_DEBUG_LAMBDA):
+    def __init__(self, w, flags=pm.PM_FLAG_DEBUG_SCALARS | pm.PM_FLAG_DEBUG_LAMBDA, put=False):
         self.w = w
+        self.put = put
         n = w.params["nz"]
         self.h = h = n // 2
         self.n = n
@@ -65,6 +66,9 @@ class Pair:
             self.sinks.append(pm.DeviceSinks.from_host(sk, DEV) if sk.n else None)
             self.sne.append(pm.DeviceSNe.from_host(sn, DEV) if sn.n else None)
         self.desc = [c.pm_slab_describe() for c in self.ctx]
+        if put:                                     # peer-memory exchange: each ctx stores into the other's receive slabs
+            self.ctx[0].pm_slab_connect_local(self.ctx[1], self.ctx[1])
+            self.ctx[1].pm_slab_connect_local(self.ctx[0], self.ctx[0])
 
     def xchg(self, grp):
         d0, d1 = self.desc
@@ -88,8 +92,9 @@ class Pair:
         self.halo()
         for r in range(2):
             self.ctx[r].pm_deposit(self.state[r], self.sinks[r], self.sne[r], dt)
-            self.ctx[r].pm_slab_pack()
-        self.xchg("buf")
+            self.ctx[r].pm_slab_put() if self.put else self.ctx[r].pm_slab_pack()
+        if not self.put:
+            self.xchg("buf")
         for r in range(2):
             self.ctx[r].pm_fold_ghosts()
         if stop_after == "fold":
@@ -259,3 +264,79 @@ def test_second_step_and_truelove_fill_back():
         parity.close_strict(g.sink_field("dm"), o.sink_diag["dm"], "sink dm")
         for c in g.ctx:
             c.close()
+
+
+def test_put_to_itself_is_the_periodic_fold_bit_for_bit():
+    """pm_slab_put with the ctx as its own neighbour (the pack kernel stores into the ctx's own receive slabs) over three
+    consecutive steps -- both receive sets -- against the periodic fold of the same arbitrary buffer contents."""
+    n = 24
+    p = inputs.default_params(n)
+    rng = np.random.default_rng(11)
+    plain = pm.Context(dict(p, z_slab=0), device="cuda:0")
+    slab = pm.Context(dict(p, z_slab=1), device="cuda:0")
+    slab.pm_slab_connect_ipc(None, None)
+    g = slab.ghost_width()
+    st_plain = pm.DeviceState(*(torch.ones(n ** 3, dtype=torch.float64, device=DEV) for _ in range(6)))
+    st_slab = pm.DeviceState(*(torch.ones((n + 2 * g) * n * n, dtype=torch.float64, device=DEV) for _ in range(6)))
+    for step in range(3):
+        outs = []
+        filled = None
+        for c, st in ((plain, st_plain), (slab, st_slab)):
+            c.pm_deposit(st, None, None, 0.1)
+            views = [c.debug_buffer(ch)[0] for ch in range(6)]
+            if filled is None:
+                filled = [torch.from_numpy(rng.standard_normal(tuple(v.shape))).to(DEV) for v in views]
+            for v, f in zip(views, filled):
+                v.copy_(f)
+            if c is slab:
+                c.pm_slab_put()
+            c.pm_fold_ghosts()
+            outs.append([c.debug_buffer(ch)[1].clone() for ch in range(6)])
+            c.pm_check()                                             # (the next pm_deposit abandons the step)
+        for a, b in zip(*outs):
+            assert torch.equal(a, b), f"step {step}"
+    slab.pm_deposit(st_slab, None, None, 0.1)
+    slab.pm_slab_put()
+    with pytest.raises(pm.PmError) as e:                             # a second put in one step
+        slab.pm_slab_put()
+    assert e.value.status == pm.PM_EORDER
+    fresh = pm.Context(dict(p, z_slab=1), device="cuda:0")
+    fresh.pm_deposit(st_slab, None, None, 0.1)
+    with pytest.raises(pm.PmError) as e:                             # a put without neighbours
+        fresh.pm_slab_put()
+    assert e.value.status == pm.PM_EORDER
+    for c in (plain, slab, fresh):
+        c.close()
+
+
+def test_two_half_domains_with_peer_puts_follow_the_oracle_for_three_steps():
+    """The two slab contexts store their ghost planes straight into each other's receive slabs (pm_slab_connect_local +
+    pm_slab_put), three steps in a row on the same contexts, so that both receive sets and their alternation are used; the
+    oracle runs alongside.  Step 1 to the strict tolerances, the free-running trajectory to 1e-9 (as in tests/parity.py)."""
+    n = 40
+    w = inputs.scaled_mixed(n, 900, seed_index=8)
+    h = n // 2
+    rng = np.random.default_rng(8)
+    for prt in (w.sinks, w.sne):
+        k = max(prt.n // 5, 2)
+        prt.z[:k] = np.mod(rng.choice([0.0, float(h)], size=k) + rng.uniform(-3.0, 3.0, size=k), float(n))
+    o = parity.make_oracle(w)
+    g = Pair(w, put=True)
+    for step in range(3):
+        o.step(w.dt)
+        g.step()
+        rho, m = g.state_np()[0], g.sink_field("m")
+        if step == 0:
+            parity.close_strict(rho, o.state.rho, "rho")
+            parity.close_strict(m, o.sinks.m, "sink m")
+            parity.close_strict(g.sink_field("dm"), o.sink_diag["dm"], "sink dm")
+        assert np.all(np.abs(rho - o.state.rho) <= 1e-9 * np.abs(o.state.rho)), f"rho, step {step}"
+        assert np.all(np.abs(m - o.sinks.m) <= 1e-9 * np.abs(o.sinks.m)), f"sink m, step {step}"
+        E = g.state_np()[4]
+        assert np.all(np.abs(E - o.state.etot) <= 1e-9 * np.abs(o.state.etot)), f"E, step {step}"
+    V = float(w.params["dx"]) ** 3
+    mass = V * rho.sum() + m.sum()
+    mass0 = V * w.state.rho.sum() + w.sinks.m.sum()
+    assert abs((mass - mass0) - 3 * w.sne.m_ej.sum()) <= 1e-12 * mass
+    for c in g.ctx:
+        c.close()
