@@ -188,6 +188,7 @@ int pm_slab_pack(pm_ctx *ctx);
  * the neighbour's fold of step n may still be reading, and ONE barrier per step suffices: a rank leaves the barrier of step n + 1
  * only after its stream, and with it its fold of step n, has drained.  All ranks must call pm_slab_put in every step of a run
  * (the sets alternate in lock step); pm_slab_pack steps (which use set 0) may not be mixed in between.
+ * The neighbours' slab memory must stay alive while this ctx can still put: destroy the ctxs of a run together, after a barrier.
  * Errors: PM_EORDER (not connected; not directly after pm_deposit), PM_EINVAL (not a slab ctx; neighbour of another shape),
  * PM_ECUDA (IPC: the peer's GPU is not peer-accessible from this one). */
 #define PM_IPC_HANDLE_BYTES 64

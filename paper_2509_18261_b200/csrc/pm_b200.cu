@@ -1,7 +1,8 @@
 // pm_b200.cu -- kernels and C ABI of libpm_b200 (see include/pm.h).  sm_100a only; built with -fmad=false.
 //
 // Kernels:
-//   (a0, the buffer reset, has no kernel of its own: tiles are zeroed on their first touch inside the deposit kernels, pm_tiles.cuh)
+//   k_tiles_mark / k_tiles_zero / k_zero_sweep   a0  buffer reset by 8^3 tiles: live tiles from the particle bins, zeroed tile by tile
+//                      or, when most of the mesh is live, by a linear sweep (pm_tiles.cuh)
 //   k_deposit_sinks    a1-a3  one warp per sink: kernel means -> Bondi-Hoyle rate -> Gaussian weights -> fp64 RED
 //   k_deposit_sne      a1,a4,a5  one warp per SN: omega counts -> stencil sums -> Eq. 17 -> fp64 RED (5 channels)
 //   k_fold_ghosts      a6  gather fold: every owned cell within g of a face sums its <= 7 ghost images, fixed order
@@ -126,7 +127,7 @@ static void tick(pm_ctx *c, int k, int which) {
 }
 
 // ---------------------------------------------------------------------------------------------------------------
-// a0: buffer reset.  No sweep: see pm_tiles.cuh.  The kernel below is for the test-only views (pm_debug_buffer,
+// a0: buffer reset: see pm_tiles.cuh.  The kernel below is for the test-only views (pm_debug_buffer,
 // pm_debug_round_buffers): it stores the zeros that stale tiles stand for and marks them live, so that the raw buffer can be read.
 // ---------------------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(128) k_tiles_materialize(const DevP P, double *__restrict__ buf, const Tiles T, const bool repro,
