@@ -174,7 +174,7 @@ def whole_job_value(cells_per_rank: int, steps: int, world: int, total_ms: float
     return world * cells_per_rank * steps / (total_ms * 1e-3) / 1e6
 
 
-def algorithmic_bytes(N, Nb, nk, nn, t, ts, tn, fk=1.0, fn=1.0, nch=6):
+def algorithmic_bytes(N, Nb, nk, nn, t, ts, tn, fk=1.0, fn=1.0, nch=6, Ng=None):
     """Bytes each kernel group must move per step: SURVEY.md 8(d)'s per-cell figures, each touched CELL counted once.
     t, ts, tn = fraction of the owned cells touched by any particle / by a sink / by a supernova; fk, fn = fraction of the
     buffer-mesh tiles that are live in channel group K (accretion) / N (supernovae) -- stale tiles are neither reset nor
@@ -190,7 +190,9 @@ def algorithmic_bytes(N, Nb, nk, nn, t, ts, tn, fk=1.0, fn=1.0, nch=6):
         "zero": 8.0 * buf_live * Nb,                                   # a0 + the write-back of a3/a5: each live buffer word written once
         "sinks": 8.0 * 5 * ts * N + 8.0 * 10 * nk,                    # a2: gather 5 fields; particle records
         "sne": 8.0 * 4 * tn * N + 8.0 * 8 * nn,                       # a4: gather 4 fields; particle records
-        "fold": 3 * 8.0 * buf_live * (Nb - N),                         # read ghosts, read-modify-write their owned images
+        "fold": 3 * 8.0 * buf_live * (Nb - N if Ng is None else Ng),   # read ghosts, read-modify-write their owned images (Ng: the
+                                                                       # ghost cells that can hold anything -- the kernels wrap x at
+                                                                       # the source, so only the y and z ghost zones; default: 8(d)'s all)
         "apply": N * (8.0 * buf_live + 96.0 * t + 32.0 * ts),          # live buffer words; 6 + 6 state words and 4 return words where touched
         "return": 8.0 * 4 * ts * N + 8.0 * 12 * nk,
     }
@@ -536,8 +538,9 @@ def run_ours(args, rank, world, local_rank):
 
     if rank == 0:
         peak, peak_src = measured_peak()
-        abytes = algorithmic_bytes(N, Nb, w.sinks.n, w.sne.n, t_frac, ts_frac, tn_frac, fk, fn, nch)
-        sbytes = algorithmic_bytes(N, Nb, w.sinks.n, w.sne.n, t4, ts4, tn4, fk, fn, nch)
+        Ng = n * ((n + 8) ** 2 - n * n)                               # y and z ghost zones of the x-wrapped buffer
+        abytes = algorithmic_bytes(N, Nb, w.sinks.n, w.sne.n, t_frac, ts_frac, tn_frac, fk, fn, nch, Ng)
+        sbytes = algorithmic_bytes(N, Nb, w.sinks.n, w.sne.n, t4, ts4, tn4, fk, fn, nch, Ng)
         dbytes = algorithmic_bytes(N, Nb, w.sinks.n, w.sne.n, 1.0, 1.0, 1.0, 1.0, 1.0, nch)
         kernels = {}
         for k in pm.KERNEL_GROUPS:

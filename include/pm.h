@@ -8,7 +8,8 @@
  *                          and the supernova recipe of Sec. 3.2.1 (Eqs. 17-20; L203-230): every particle adds its
  *                          deposition function dU^s_ijk into a ghost-zoned buffer mesh with fp64 atomic additions.
  *   pm_fold_ghosts         Step 2, Eq. 3 (L67-71): ghost-zone contents are added to the owning real zones.  On one
- *                          GPU the "other rank" is the periodic image, so this is an in-device periodic fold.
+ *                          GPU the "other rank" is the periodic image, so this is an in-device periodic fold.  (y and z ghost
+ *                          zones; along x, the fastest axis, particles add to the periodic image directly.)
  *   pm_apply_limited       Steps 3 + 5, Eqs. 4 and 6 (L73-77, L89-93) fused: the cell-wise limiters (Eqs. 15-16,
  *                          L161-171, with BASELINE's max-removable-fraction and density floor; Eq. 21) and
  *                          U := U + eta dU^sum, in place on the caller's conserved state.
@@ -323,7 +324,9 @@ int pm_probe_red_f64(pm_ctx *ctx, int64_t footprint_bytes, int32_t channels, dou
  * The channel is a contiguous (dims[0], dims[1], dims[2]) = (nz+2g, ny+2g, row pitch) array, x fastest; the row pitch
  * is nx + 2*gx with gx = g rounded up to even (keeps 128-bit accesses aligned).  *origin = element offset of owned
  * cell (0,0,0); owned cell (i,j,k) sits at origin + (k*dims[1] + j)*dims[2] + i, ghost cells at i,j,k in [-g, n+g).
- * *ghost = g.  Stale tiles (no particle touched them in this step) are filled with the zeros they stand for first. */
+ * *ghost = g.  Stale tiles (no particle touched them in this step) are filled with the zeros they stand for first.
+ * The x ghost columns (i < 0, i >= nx) exist for alignment only and stay empty: particles wrap x where they add; the y and z
+ * ghost zones hold the deposits that pm_fold_ghosts (or the slab exchange) adds to their owners. */
 int pm_debug_buffer(pm_ctx *ctx, int channel, const double **dev_ptr, int64_t dims[3], int64_t *origin, int32_t *ghost);
 
 /* Tiles of the buffer mesh (8^3 cells, ghost tiles included) and how many of them the last pm_deposit marked live per channel

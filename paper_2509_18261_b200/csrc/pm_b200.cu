@@ -290,7 +290,7 @@ __global__ void __launch_bounds__(128) k_deposit_sinks(const DevP P, const DevSt
                 amt = fmax(amt, truelove_excess(P, U.rho[q], U.eint[q]));
                 ret_tr[q] = -CUDART_INF;                              // invalidate last step's entry (rewritten by the apply pass)
             }
-            double *dst = buf0 + ghost_index(P, i, j, k);
+            double *dst = buf0 + deposit_index(P, i, j, k);
             red_add(dst, -amt);                                     // R1: signed change
             if (REPRO) red_add(dst + kChK * P.Nb, kSinkUnit);         // Appendix A: contribution count
         }
@@ -359,7 +359,7 @@ __global__ void __launch_bounds__(kSnWarps * 32) k_deposit_sne(const DevP P, con
         const double rho = U.rho[q];
         double d[5];
         sn_cell_deposit(P, sc, xs, ys, zs, e_sn, m_ej, i, j, k, cnt, rho, U.mx[q] / rho, U.my[q] / rho, U.mz[q] / rho, d);
-        double *dst = buf + P.Nb + ghost_index(P, i, j, k);
+        double *dst = buf + P.Nb + deposit_index(P, i, j, k);
 #pragma unroll
         for (int f = 0; f < 5; ++f) red_add(dst + (long long)f * P.Nb, d[f]);
         if (REPRO) {                                 // Appendix A: error scales and the contribution count (dst is channel 1)
@@ -402,8 +402,9 @@ __global__ void k_debug_stencil(const DevP P, int kind, double xs, double ys, do
 }
 
 // ---------------------------------------------------------------------------------------------------------------
-// a6: ghost fold (gather form).  One thread per owned cell that lies within g of a face; it adds, in the fixed
-// order (z image, y image, x image), the ghost copies of itself to the owned value, for all six channels.
+// a6: ghost fold (gather form).  One thread per owned cell that lies within g of a y or z face; it adds, in the fixed
+// order (z image, y image, zy image), the ghost copies of itself to the owned value, for all six channels.  There are no x
+// images: the particles wrap x where they add (deposit_index, pm_device.cuh).
 // ---------------------------------------------------------------------------------------------------------------
 template <int VEC> struct Vec;
 template <> struct Vec<1> { typedef double type; };
@@ -420,8 +421,8 @@ __device__ __forceinline__ void stv(double *p, const double v[VEC]) {
     else *p = v[0];
 }
 
-// W = 2: one thread folds two x-adjacent cells with 128-bit accesses (needs g and nx even, so that a pair never straddles
-// the g-wide face strip and every pair is 16-byte aligned); W = 1 otherwise.  Counts are in units of W cells.
+// W = 2: one thread folds two x-adjacent cells with 128-bit accesses (needs nx even: every pair is then 16-byte aligned, the
+// ghosted row pitch and the x origin gx being even); W = 1 otherwise.  Counts are in units of W cells.
 // STAMPS: a stale tile stands for zeros (pm_tiles.cuh) and is not read; an owned cell whose own tile is stale has no live image
 // either (a deposit that reaches a ghost cell also claims the tile of its image), so there is nothing to do for it.  Channel 0
 // belongs to group K, channels 1..7 to group N, the Appendix A count channel (8) is live where either group is.
@@ -446,7 +447,7 @@ __global__ void __launch_bounds__(256) k_fold_ghosts(const DevP P, double *__res
         long long r = t - (long long)kk * plane;
         j = (int)(r / nxw); i = W * (int)(r - (long long)j * nxw);
         k = kk < g ? kk : nz - 2 * g + kk;
-    } else if (t < n_zslab + n_yslab) {      // interior k, j in [0,g) U [ny-g,ny)
+    } else {                                 // interior k, j in [0,g) U [ny-g,ny)   (no x faces: the deposits wrap x themselves)
         long long r = t - n_zslab;
         const long long slab = (long long)nxw * 2 * g;
         int kk = (int)(r / slab);
@@ -454,18 +455,9 @@ __global__ void __launch_bounds__(256) k_fold_ghosts(const DevP P, double *__res
         int jj = (int)(r / nxw); i = W * (int)(r - (long long)jj * nxw);
         k = g + kk;
         j = jj < g ? jj : ny - 2 * g + jj;
-    } else {                                 // interior k and j, i in [0,g) U [nx-g,nx)
-        long long r = t - n_zslab - n_yslab;
-        const int w = 2 * g / W;
-        const long long slab = (long long)(ny - 2 * g) * w;
-        int kk = (int)(r / slab);
-        r -= (long long)kk * slab;
-        int jj = (int)(r / w); int ii = W * (int)(r - (long long)jj * w);
-        k = g + kk; j = g + jj;
-        i = ii < g ? ii : nx - 2 * g + ii;
     }
     // image offsets per axis: 0 plus (+n if within g of the low face) or (-n if within g of the high face)
-    const int ox = i < g ? nx : (i >= nx - g ? -nx : 0);
+    const int ox = 0;                         // the deposits wrap x themselves (deposit_index): the x ghost columns are empty
     const int oy = j < g ? ny : (j >= ny - g ? -ny : 0);
     const int oz = k < g ? nz : (k >= nz - g ? -nz : 0);
     const long long base = ghost_index(P, i, j, k);
@@ -1007,11 +999,10 @@ extern "C" int pm_fold_ghosts(pm_ctx *c) {
     PM_CUDA(c, cudaSetDevice(c->device));
     const DevP &P = c->P;
     const long long g2 = 2 * P.g;
-    const int W = (P.g % 2 == 0 && P.nx % 2 == 0) ? 2 : 1;
+    const int W = P.nx % 2 == 0 ? 2 : 1;
     const long long n_z = g2 * P.ny * P.nx / W;
     const long long n_y = (long long)(P.nz - g2) * g2 * P.nx / W;
-    const long long n_x = (long long)(P.nz - g2) * (P.ny - g2) * g2 / W;
-    const long long n_edge = n_z + n_y + n_x;
+    const long long n_edge = n_z + n_y;                     // no x faces: deposit_index wraps x at the source
     const unsigned blocks = (unsigned)((n_edge + 255) / 256);
     tick(c, PM_K_FOLD, 0);
     const Tiles T = tiles_of(c);
@@ -1285,11 +1276,10 @@ extern "C" int pm_create_sinks(pm_ctx *c, pm_state *st, int64_t max_new, double 
 static int fold_gravity_channel(pm_ctx *c, double *gbuf) {
     const DevP &P = c->P;
     const long long g2 = 2 * P.g;
-    const int W = (P.g % 2 == 0 && P.nx % 2 == 0) ? 2 : 1;
+    const int W = P.nx % 2 == 0 ? 2 : 1;
     const long long n_z = g2 * P.ny * P.nx / W;
     const long long n_y = (long long)(P.nz - g2) * g2 * P.nx / W;
-    const long long n_x = (long long)(P.nz - g2) * (P.ny - g2) * g2 / W;
-    const long long n_edge = n_z + n_y + n_x;
+    const long long n_edge = n_z + n_y;
     const unsigned blocks = (unsigned)((n_edge + 255) / 256);
     if (W == 2) k_fold_ghosts<2, 1, false><<<blocks, 256, 0, c->stream>>>(P, gbuf, tiles_of(c), n_edge, n_z, n_y, nullptr, nullptr);
     else k_fold_ghosts<1, 1, false><<<blocks, 256, 0, c->stream>>>(P, gbuf, tiles_of(c), n_edge, n_z, n_y, nullptr, nullptr);
@@ -1745,8 +1735,7 @@ extern "C" int pm_gravity_deposit_noalloc(int device, void *cuda_stream, int32_t
         const long long g2 = 2 * P.g;
         const long long n_z = g2 * P.ny * P.nx;
         const long long n_y = (long long)(P.nz - g2) * g2 * P.nx;
-        const long long n_x = (long long)(P.nz - g2) * (P.ny - g2) * g2;
-        const long long n_edge = n_z + n_y + n_x;
+        const long long n_edge = n_z + n_y;
         k_fold_ghosts<1, 1, false><<<(unsigned)((n_edge + 255) / 256), 256, 0, stream>>>(P, mesh, Tiles{nullptr, nullptr}, n_edge, n_z, n_y, nullptr, nullptr);
         NOALLOC_CUDA(cudaGetLastError());
     }

@@ -89,6 +89,12 @@ __device__ __forceinline__ long long owned_index(const DevP &P, int i, int j, in
 __device__ __forceinline__ long long ghost_index(const DevP &P, int i, int j, int k) {
     return (long long)(k + P.g) * P.pk + (long long)(j + P.g) * P.pj + (i + P.gx);
 }
+// Where a particle ADDS: x is wrapped into [0, nx) on the spot (the mesh is periodic in x inside every ctx, also on a z slab), so
+// the x ghost columns of the buffer mesh never receive anything and the fold has no x images to gather (its x faces were 32-byte
+// strips at a 4 KB stride: a third of its bytes and more than half of its time).  y and z keep their ghost zones (Eq. 3).
+__device__ __forceinline__ long long deposit_index(const DevP &P, int i, int j, int k) {
+    return ghost_index(P, wrap1(i, P.nx), j, k);
+}
 
 // Bin key of a host cell: super-blocks in raster order, the 4x4x4 tiles inside one in Morton order.  Particles are
 // processed bin by bin (a counting sort by this key, filled by atomic append -- no global comparison sort), so that

@@ -42,7 +42,8 @@ __global__ void __launch_bounds__(256) k_grav_deposit(const DevP P, const double
         atomicOr(err_flag, 1);
         return;
     }
-    const long long base = ghost_index(P, i0, j0, k0);
+    const long long base = ghost_index(P, 0, j0, k0);
+    const int ix[2] = { wrap1(i0, P.nx), wrap1(i0 + 1, P.nx) };       // x wrapped on the spot (deposit_index); y, z through the ghost layer
 #pragma unroll
     for (int dk = 0; dk < 2; ++dk)
 #pragma unroll
@@ -50,7 +51,7 @@ __global__ void __launch_bounds__(256) k_grav_deposit(const DevP P, const double
             const double wzy = wz[dk] * wy[dj];
             double *row = buf + base + dk * P.pk + dj * P.pj;
 #pragma unroll
-            for (int di = 0; di < 2; ++di) atomicAdd(row + di, m * (wzy * wx[di]) / P.V);
+            for (int di = 0; di < 2; ++di) atomicAdd(row + ix[di], m * (wzy * wx[di]) / P.V);
         }
 }
 

@@ -97,7 +97,7 @@ __device__ __forceinline__ int sink_owned(const SinkWarpSmem &sm, int code) {
     return sm.off[2][code >> 8] + sm.off[1][(code >> 4) & 15] + sm.off[0][code & 15];
 }
 __device__ __forceinline__ int sink_ghosted(const SinkWarpSmem &sm, int code) {
-    return sm.goff[1][code >> 8] + sm.goff[0][(code >> 4) & 15] + (code & 15);
+    return sm.goff[1][code >> 8] + sm.goff[0][(code >> 4) & 15] + sm.off[0][code & 15];     // x wrapped into [0, nx) (deposit_index)
 }
 
 __device__ __forceinline__ double sink_weight(const SinkWarpSmem &sm, int code) {
@@ -146,7 +146,7 @@ __global__ void __launch_bounds__(kFastSinkWarps * 32, kFastSinkMinBlocks) k_dep
     for (int i = lane; i < nm; i += 32) wsum += sink_weight(sm, sm.code[i]);
     wsum = warp_sum(wsum);
     const double k = sc.mdot * dt / (wsum * P.V);         // a = mdot (w / sum w) dt / V
-    double *const sbuf = buf0 + (ih - 4 + P.gx);
+    double *const sbuf = buf0 + P.gx;
     for (int i = lane; i < nm; i += 32) {
         const int code = sm.code[i];
         double *dst = sbuf + sink_ghosted(sm, code);

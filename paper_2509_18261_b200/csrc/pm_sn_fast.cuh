@@ -257,6 +257,7 @@ __device__ __forceinline__ void sn_deposit_one(const DevP &P, const DevState &U,
     const double k_p = sc.p_rad * inv_vsnr;
     double *const sbuf = buf + P.Nb + ((long long)(kh - 3 + P.g) * P.pk + (long long)(jh - 3 + P.g) * P.pj + (ih - 3 + P.gx));
     const int pj = (int)P.pj, pk = (int)P.pk;
+    const bool xin = ih >= 3 && ih + 3 < P.nx;            // warp-uniform: the box does not cross the periodic x seam
     if (DENSE) {
         // the same values, added into the CTA's tile accumulator: all 32 lanes stay in the loop (the lock is taken per warp)
         volatile double *const acc = tile->acc;
@@ -308,7 +309,7 @@ __device__ __forceinline__ void sn_deposit_one(const DevP &P, const DevState &U,
         const double drho = omega * k_rho;
         const double pscale = (k_p * omega) * ir;
         const double prx = pscale * ddx, pry = pscale * ddy, prz = pscale * ddz;
-        double *dst = sbuf + (cc * pk + b * pj + a);              // ghosted layout: no wrap, plain strides
+        double *dst = sbuf + (cc * pk + b * pj + (xin ? a : sm.off[0][a] - (ih - 3)));   // y, z: ghosted, plain strides; x wrapped (deposit_index)
         // omega rho (v_COM - v) = omega (rho v_COM - m): no division by rho
         const double dpx = fma(omega, fma(rho, sc.vcx, -mx), fma(drho, sc.vcx, prx));
         const double dpy = fma(omega, fma(rho, sc.vcy, -my), fma(drho, sc.vcy, pry));
@@ -423,7 +424,7 @@ __global__ void __launch_bounds__(kSnDenseWarps * 32, 1) k_deposit_sne_dense(con
             const int lx = e % kAccSide, r = e / kAccSide, ly = r % kAccSide, lz = r / kAccSide;
             const int i = tile.ox + lx, j = tile.oy + ly, k = tile.oz + lz;
             if (i >= P.nx + P.g || j >= P.ny + P.g || k >= P.nz + P.g) continue;      // beyond the ghost zone (ragged last tile): never touched
-            double *dst = buf + P.Nb + ghost_index(P, i, j, k);
+            double *dst = buf + P.Nb + deposit_index(P, i, j, k);
 #pragma unroll
             for (int f = 0; f < 5; ++f) {
                 const double v = acc[f * kAccCells + e];

@@ -17,6 +17,18 @@ def dev(a):
     return torch.from_numpy(np.ascontiguousarray(a)).to(DEV)
 
 
+def fold_x_only(buf, g):
+    """The oracle's ghost-zoned buffer (nz + 2g, ny + 2g, nx + 2g) with its x ghost columns added to the owned columns they
+    image and then emptied: the kernels wrap x where they add (csrc/pm_device.cuh: deposit_index), so on the GPU only the y
+    and z ghost zones ever hold anything before the fold."""
+    out = buf.copy()
+    out[:, :, g:2 * g] += buf[:, :, -g:]
+    out[:, :, -2 * g:-g] += buf[:, :, :g]
+    out[:, :, :g] = 0.0
+    out[:, :, -g:] = 0.0
+    return out
+
+
 def run_deposit(w, with_gas=True):
     ctx = pm.Context(w.params, device=DEV)
     out = torch.empty(w.rho_gas.shape, dtype=torch.float64, device=DEV)
@@ -30,7 +42,7 @@ def check_deposit(w, with_gas=True):
     p = w.params
     ghosted, owned, g, ox = ctx.debug_buffer(1)
     # Step 1 alone: the ghost cells keep what was deposited into them (the fold leaves them in place)
-    ref_buf = go.gravity_deposit_buffer(p, w.x, w.y, w.z, w.m, g=g)
+    ref_buf = fold_x_only(go.gravity_deposit_buffer(p, w.x, w.y, w.z, w.m, g=g), g)
     gb = ghosted[:, :, ox - g:ox - g + p["nx"] + 2 * g].cpu().numpy()
     ghost_mask = np.ones(ref_buf.shape, dtype=bool)
     ghost_mask[g:-g, g:-g, g:-g] = False

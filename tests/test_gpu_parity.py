@@ -114,6 +114,9 @@ def test_seam_particles():
     ghosted, owned, gz, ox = g.ctx.debug_buffer(1)
     ghost_sum = float(ghosted.abs().sum() - owned.abs().sum())
     assert ghost_sum > 0.0, "seam particles must have deposited into ghost zones"
+    # x is wrapped where the particles add (deposit_index): the x ghost columns stay empty, y and z ghost zones are used
+    xg = torch.cat([ghosted[:, :, :ox], ghosted[:, :, ox + 32:]], dim=2)
+    assert float(xg.abs().sum()) == 0.0
 
 
 def test_stacked_particles_contention():
