@@ -17,6 +17,9 @@
  *                          (supernova particles skip this step, L201).
  *   pm_gravity_deposit / pm_gravity_kick / pm_drift   PM gravity for the particles' own motion (L95, L107): Steps 1, 2, 5
  *                          with the cloud-in-cell kernel, interpolation back with the same kernel, kick-drift-kick.
+ *   z_slab = 1, pm_slab_pack / pm_slab_put   Step 2 across ranks (L97): a domain cut along z; the z ghost planes travel to the
+ *                          two neighbours as messages, or are stored straight into their receive slabs by the pack kernel.
+ *   pm_gravity_deposit_noalloc   the gravity deposit without a ctx and without any allocation (static device scratch).
  *
  * All pointers inside pm_state / pm_sinks / pm_sne are DEVICE pointers (cudaMalloc'ed by the caller, e.g. torch
  * allocations) unless a function says "host".  Every array is fp64, contiguous.  Mesh fields hold nx*ny*nz values,
