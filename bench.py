@@ -442,6 +442,34 @@ def run_ours(args, rank, world, local_rank):
                      "hbm_footprint_5GB_5ch": ctx.pm_probe_red_f64(5 << 30, 5), "unit": "1e9 fp64 RED lanes/s",
                      "pattern": "rows of 7 consecutive doubles, 5 planes (pm_probe_red_f64)"}
 
+    # ---- the same step through pm_step_graph (one call, replayed from a CUDA graph): what the launch overhead is worth ---------
+    graph_leg = None
+    if rank == 0 and world == 1:
+        torch.cuda.synchronize(dev)                   # the side stream below does not wait for the default stream by itself
+        gstream = torch.cuda.Stream(dev)              # a default stream cannot be captured
+        with torch.cuda.stream(gstream):
+            gctx = pm.Context(w.params, device=str(dev), stream=gstream, flags=mode)
+            gst = pm.DeviceState(*(f.clone() for f in st.fields()))
+            for i in range(max(warm, 3)):
+                gctx.pm_step_graph(gst, sk, sn, w.dt, reuse_args=i > 0)
+            gctx.pm_check()
+            gsteps = max(args.steps, 10)
+            g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            t0 = time.perf_counter()
+            g0.record()
+            for _ in range(gsteps):
+                gctx.pm_step_graph(gst, sk, sn, w.dt, reuse_args=True)
+            g1.record()
+            host_s = time.perf_counter() - t0          # until the last call returns: what the host spends enqueuing
+            g1.synchronize()
+            graph_leg = {"ms_per_step": g0.elapsed_time(g1) / gsteps, "host_us_per_call": host_s / gsteps * 1e6, "steps": gsteps,
+                         "state": gctx.debug_graph_state(),
+                         "api": "pm_step_graph: deposit + fold + apply + return captured once, then one cudaGraphLaunch per step; "
+                                "CUDA events on the launching stream"}
+            gctx.close()
+            del gst
+        torch.cuda.synchronize(dev)
+
     # ---- row (f)3, not part of the step: PM gravity (Steps 1, 2, 5; L95, L107) for the same number of particles --------
     gravity = None
     if rank == 0 and world == 1 and not args.reproducible and args.config is None:
@@ -602,6 +630,8 @@ def run_ours(args, rank, world, local_rank):
         }
         if creation:
             line["sink_creation"] = creation
+        if graph_leg:
+            line["graph_step"] = graph_leg
         if gravity:
             line["gravity"] = gravity
         if red_probe:

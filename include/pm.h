@@ -286,6 +286,17 @@ const char *pm_noalloc_last_error(void);
 /* Synchronise the ctx's stream and report PM_ECUDA / PM_EDOMAIN raised by earlier asynchronous work. */
 int pm_check(pm_ctx *ctx);
 
+/* One whole step with DEVICE buffers as ONE call: pm_deposit, pm_fold_ghosts, pm_apply_limited and (when there are sinks)
+ * pm_return_to_particles, replayed from a CUDA graph.  A step is twelve kernel launches and a memset; on small meshes the
+ * host's launch calls take longer than the kernels run.  The first call with a given set of arguments (all pointers in state,
+ * sinks and sne, the particle counts, dt) makes the plain calls; the second captures the same calls from the ctx's stream into
+ * a graph and launches it; from the third on the call is one cudaGraphLaunch.  The kernels read particle data and state from
+ * memory, so moving particles and evolving gas replay the same graph; any change of a pointer, a count or dt starts over with
+ * plain calls.  Same results as the four calls (same kernels, same order).  Falls back to the plain calls, every time, when
+ * the ctx's stream is a default stream (those cannot be captured) or the ctx has PM_FLAG_TIMING.  Not on a z slab (PM_EINVAL).
+ * Asynchronous; errors as for the four calls. */
+int pm_step_graph(pm_ctx *ctx, pm_state *state, pm_sinks *sinks, const pm_sne *sne, double dt);
+
 /* One whole step with HOST buffers (the end-to-end path): copies state and particles host -> device into
  * ctx-owned staging (allocated on first use), runs deposit, fold, apply, return, copies the state and the sink
  * fields (vx, vy, vz, m and the optional dm, dp*) back, and synchronises.  All pointers in the three structs are
@@ -331,6 +342,10 @@ int pm_probe_red_f64(pm_ctx *ctx, int64_t footprint_bytes, int32_t channels, dou
  * The x ghost columns (i < 0, i >= nx) exist for alignment only and stay empty: particles wrap x where they add; the y and z
  * ghost zones hold the deposits that pm_fold_ghosts (or the slab exchange) adds to their owners. */
 int pm_debug_buffer(pm_ctx *ctx, int channel, const double **dev_ptr, int64_t dims[3], int64_t *origin, int32_t *ghost);
+
+/* Where pm_step_graph stands: 0 = the next call makes plain calls, 1 = the next call with the same arguments captures,
+ * 2 = calls with the same arguments replay the graph.  HOST output. */
+int pm_debug_graph_state(pm_ctx *ctx, int32_t *state);
 
 /* Tiles of the buffer mesh (8^3 cells, ghost tiles included) and how many of them the last pm_deposit marked live per channel
  * group (K: accretion channel, N: supernova channels); stale tiles are neither reset nor read.  HOST outputs.  Synchronises. */

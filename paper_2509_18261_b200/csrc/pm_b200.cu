@@ -97,6 +97,11 @@ struct pm_ctx {
     bool dense_smem_ok; // the device grants the dense SN kernel its shared memory (tile accumulator, 150 KB)
     bool grav_in_ch1;   // buffer channel 1 holds the last pm_gravity_deposit (until the next pm_deposit): the debug view must not
                         // "fill in" its stale tiles
+    // pm_step_graph: the four calls of a step captured once into a CUDA graph and replayed while the arguments stay the same
+    struct GraphKey { pm_state st; pm_sinks sk; pm_sne sn; double dt; } gkey;
+    cudaGraphExec_t gexec;
+    int gstate;         // 0: nothing; 1: gkey has run once eagerly (scratch memory is in place); 2: gexec replays gkey
+    long long glaunches;   // kernels in the graph (pm_launch_count advances by this per replay)
     bool timing;        // PM_FLAG_TIMING
     cudaEvent_t ev[PM_NUM_KERNELS][2];
     bool ev_used[PM_NUM_KERNELS];
@@ -711,6 +716,7 @@ static bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 
 
 static int grow(pm_ctx *c, double **p, long long *cap, long long need) {
     if (need <= *cap) return PM_OK;
+    c->gstate = 0;                          // a captured step (pm_step_graph) holds the old address
     if (*p) { PM_CUDA(c, cudaFree(*p)); *p = nullptr; *cap = 0; }
     long long n = need + need / 4 + 64;
     cudaError_t e = cudaMalloc(p, (size_t)n * sizeof(double));
@@ -839,6 +845,7 @@ extern "C" int pm_destroy(pm_ctx *c) {
     for (double *p : ptrs) if (p) cudaFree(p);
     if (c->timing)
         for (int k = 0; k < PM_NUM_KERNELS; ++k) { cudaEventDestroy(c->ev[k][0]); cudaEventDestroy(c->ev[k][1]); }
+    if (c->gexec) cudaGraphExecDestroy(c->gexec);
     if (c->up_stream) {
         cudaStreamSynchronize(c->up_stream); cudaStreamSynchronize(c->down_stream);
         cudaStreamDestroy(c->up_stream); cudaStreamDestroy(c->down_stream);
@@ -861,6 +868,7 @@ extern "C" int pm_set_repro_margin(pm_ctx *c, int32_t M) {
     if (!c->repro) PM_FAIL(c, PM_EINVAL, "pm_set_repro_margin needs PM_FLAG_REPRODUCIBLE");
     if (M < 0 || M > 52) PM_FAIL(c, PM_EINVAL, "pm_set_repro_margin: M must be in [0, 52]");
     c->repro_M = M;
+    c->gstate = 0;       // the margin is an argument of the captured apply kernel
     return PM_OK;
 }
 
@@ -901,6 +909,7 @@ extern "C" int pm_deposit(pm_ctx *c, const pm_state *st, const pm_sinks *sk, con
         // dense-bin counters (front, back, queue head) | dense-bin list
         const long long need = 2 * np + nkeys + nscan + nkeys + nocc + 2 + 3 + P.ntile;
         if (need > c->bin_cap) {
+            c->gstate = 0;                  // a captured step (pm_step_graph) holds the old address
             if (c->bin_mem) { PM_CUDA(c, cudaFree(c->bin_mem)); c->bin_mem = nullptr; c->bin_cap = 0; }
             const long long cap = need + need / 4;
             cudaError_t e = cudaMalloc(&c->bin_mem, (size_t)cap * sizeof(int));
@@ -1494,6 +1503,80 @@ extern "C" int pm_step_host(pm_ctx *c, pm_state *hs, pm_sinks *hk, const pm_sne 
     int rc = pm_step_host_begin(c, 0, hs, hk, hn, dt);
     if (rc != PM_OK) return rc;
     return pm_step_host_end(c, 0);
+}
+
+// ---- pm_step_graph ---------------------------------------------------------------------------------------------
+// One step = twelve launches and a memset; on small meshes (BASELINE configs 1-3) the host's launch calls take longer than the
+// kernels run.  The four calls are therefore captured once into a CUDA graph and replayed while the argument pointers, the
+// particle counts and dt stay what they were: first call with a set of arguments -> plain calls (they put the scratch memory in
+// place: no allocation may happen under capture); second call -> the same calls under stream capture, instantiate, launch; from
+// the third on -> one cudaGraphLaunch.  The kernels read positions, masses and the state from memory, so a run whose particles
+// move and whose gas evolves replays the same graph.
+static int step_calls(pm_ctx *c, pm_state *st, pm_sinks *sk, const pm_sne *sn, double dt) {
+    int rc = pm_deposit(c, st, sk, sn, dt);
+    if (rc == PM_OK) rc = pm_fold_ghosts(c);
+    if (rc == PM_OK) rc = pm_apply_limited(c, st);
+    if (rc == PM_OK && sk && sk->n > 0) rc = pm_return_to_particles(c, sk);
+    return rc;
+}
+
+extern "C" int pm_step_graph(pm_ctx *c, pm_state *st, pm_sinks *sk, const pm_sne *sn, double dt) {
+    if (!c) return PM_EINVAL;
+    if (!state_ok(st)) PM_FAIL(c, PM_EINVAL, "pm_step_graph: null state pointer");
+    if (c->P.zopen) PM_FAIL(c, PM_EINVAL, "pm_step_graph: not available on a z slab (the exchange sits between the calls)");
+    pm_ctx::GraphKey key;
+    std::memset(&key, 0, sizeof(key));
+    key.st = *st; key.dt = dt;
+    if (sk) key.sk = *sk;
+    if (sn) key.sn = *sn;
+    // the legacy default stream cannot be captured, and the events of PM_FLAG_TIMING must not end up inside a graph
+    const bool capturable = c->stream != nullptr && c->stream != cudaStreamLegacy && c->stream != cudaStreamPerThread && !c->timing;
+    const bool same = c->gstate > 0 && std::memcmp(&key, &c->gkey, sizeof(key)) == 0;
+    if (capturable && same && c->gstate == 2) {
+        PM_CUDA(c, cudaSetDevice(c->device));
+        PM_CUDA(c, cudaGraphLaunch(c->gexec, c->stream));
+        // what the four calls leave behind on the host side
+        c->launches += c->glaunches;
+        c->n_sinks_dep = sk ? sk->n : 0; c->n_sne_dep = sn ? sn->n : 0; c->dt = dt;
+        c->ever_deposited = true; c->grav_in_ch1 = false; c->buffer_valid = true;
+        c->stage = (sk && sk->n > 0) ? ST_IDLE : ST_APPLIED;
+        return PM_OK;
+    }
+    if (capturable && same && c->gstate == 1) {
+        PM_CUDA(c, cudaSetDevice(c->device));
+        const long long l0 = c->launches;
+        cudaGraph_t graph = nullptr;
+        cudaError_t e = cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal);
+        if (e == cudaSuccess) {
+            const int rc = step_calls(c, st, sk, sn, dt);
+            e = cudaStreamEndCapture(c->stream, &graph);
+            if (rc == PM_OK && e == cudaSuccess && graph) {
+                if (c->gexec) { cudaGraphExecDestroy(c->gexec); c->gexec = nullptr; }
+                e = cudaGraphInstantiate(&c->gexec, graph, 0);
+                cudaGraphDestroy(graph);
+                if (e == cudaSuccess) {
+                    c->glaunches = c->launches - l0;
+                    c->gstate = 2;
+                    PM_CUDA(c, cudaGraphLaunch(c->gexec, c->stream));
+                    return PM_OK;
+                }
+            } else if (graph) cudaGraphDestroy(graph);
+        }
+        cudaGetLastError();                    // capture refused or broken: forget it and do the step the plain way
+        c->launches = l0;
+        c->gstate = 0;
+        c->stage = ST_IDLE;
+    }
+    const int rc = step_calls(c, st, sk, sn, dt);
+    if (rc == PM_OK && capturable) { c->gkey = key; c->gstate = 1; }
+    else c->gstate = 0;
+    return rc;
+}
+
+extern "C" int pm_debug_graph_state(pm_ctx *c, int32_t *state) {
+    if (!c || !state) return PM_EINVAL;
+    *state = c->gstate;
+    return PM_OK;
 }
 
 // ---- test-only views ---------------------------------------------------------------------------------------------

@@ -25,7 +25,7 @@ KERNEL_GROUPS = ("bin", "zero", "sinks", "sne", "fold", "apply", "return")
 STATUS_NAMES = {0: "PM_OK", -1: "PM_EINVAL", -2: "PM_ENOMEM", -3: "PM_ECUDA", -4: "PM_EORDER", -5: "PM_EDOMAIN"}
 
 EXPORTS = ["pm_create", "pm_deposit", "pm_fold_ghosts", "pm_apply_limited", "pm_return_to_particles", "pm_check",
-           "pm_step_host", "pm_step_host_begin", "pm_step_host_end", "pm_destroy", "pm_last_error", "pm_launch_count", "pm_kernel_times", "pm_probe_red_f64", "pm_set_repro_margin", "pm_create_sinks", "pm_gravity_deposit", "pm_gravity_kick", "pm_drift", "pm_slab_describe", "pm_slab_pack", "pm_debug_round_buffers", "pm_debug_buffer", "pm_debug_tile_counts",
+           "pm_step_host", "pm_step_host_begin", "pm_step_host_end", "pm_step_graph", "pm_destroy", "pm_last_error", "pm_launch_count", "pm_kernel_times", "pm_probe_red_f64", "pm_set_repro_margin", "pm_create_sinks", "pm_gravity_deposit", "pm_gravity_kick", "pm_drift", "pm_slab_describe", "pm_slab_pack", "pm_debug_round_buffers", "pm_debug_buffer", "pm_debug_tile_counts", "pm_debug_graph_state",
            "pm_debug_return_mesh", "pm_debug_lambda", "pm_debug_sink_scalars", "pm_debug_sn_scalars",
            "pm_debug_stencil", "pm_slab_ipc_export", "pm_slab_connect_ipc", "pm_slab_connect_local", "pm_slab_put", "pm_noalloc_setup", "pm_gravity_deposit_noalloc", "pm_noalloc_last_error"]
 
@@ -109,6 +109,7 @@ def lib():
         L.pm_step_host.argtypes = [vp, C.POINTER(PmState), C.POINTER(PmSinks), C.POINTER(PmSNe), C.c_double]
         L.pm_step_host_begin.argtypes = [vp, C.c_int, C.POINTER(PmState), C.POINTER(PmSinks), C.POINTER(PmSNe), C.c_double]
         L.pm_step_host_end.argtypes = [vp, C.c_int]
+        L.pm_step_graph.argtypes = [vp, C.POINTER(PmState), C.POINTER(PmSinks), C.POINTER(PmSNe), C.c_double]
         L.pm_destroy.argtypes = [vp]
         L.pm_last_error.argtypes = [vp]
         L.pm_last_error.restype = C.c_char_p
@@ -124,6 +125,7 @@ def lib():
         L.pm_debug_round_buffers.argtypes = [vp]
         L.pm_debug_buffer.argtypes = [vp, C.c_int, C.POINTER(vp), i64p, i64p, i32p]
         L.pm_debug_tile_counts.argtypes = [vp, i64p, i64p, i64p]
+        L.pm_debug_graph_state.argtypes = [vp, i32p]
         L.pm_slab_describe.argtypes = [vp, C.POINTER(PmSlabDesc)]
         L.pm_slab_pack.argtypes = [vp]
         L.pm_slab_put.argtypes = [vp]
@@ -343,6 +345,21 @@ class Context:
         self._chk(self.L.pm_deposit(self.h, C.byref(cs), C.byref(ck) if ck else None, C.byref(cn) if cn else None, dt),
                   "pm_deposit")
 
+    def pm_step_graph(self, state: DeviceState, sinks, sne, dt: float, reuse_args: bool = False):
+        """The four calls of a step as one call, replayed from a CUDA graph while the arguments stay the same.
+        reuse_args=True keeps the marshalled structs of the previous call (the caller promises that state, sinks and sne still
+        hold the same tensors): a replay then costs one ctypes call."""
+        hit = getattr(self, "_graph_args", None) if reuse_args else None
+        if hit is None:
+            self._on_device(state, sinks, sne)
+            cs = state.c(self._cells())
+            ck = sinks.c() if sinks is not None else None
+            cn = sne.c() if sne is not None else None
+            hit = self._graph_args = (cs, ck, cn, (state, sinks, sne))       # the owners are kept alive with the pointers
+        cs, ck, cn, _ = hit
+        self._chk(self.L.pm_step_graph(self.h, C.byref(cs), C.byref(ck) if ck else None, C.byref(cn) if cn else None, dt),
+                  "pm_step_graph")
+
     def pm_fold_ghosts(self):
         self._chk(self.L.pm_fold_ghosts(self.h), "pm_fold_ghosts")
 
@@ -443,6 +460,11 @@ class Context:
         g = C.c_double(0.0)
         self._chk(self.L.pm_probe_red_f64(self.h, int(footprint_bytes), int(channels), C.byref(g)), "pm_probe_red_f64")
         return g.value
+
+    def debug_graph_state(self) -> int:
+        v = C.c_int32()
+        self._chk(self.L.pm_debug_graph_state(self.h, C.byref(v)), "pm_debug_graph_state")
+        return int(v.value)
 
     def pm_launch_count(self) -> int:
         return int(self.L.pm_launch_count(self.h))
