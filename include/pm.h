@@ -292,8 +292,9 @@ int pm_check(pm_ctx *ctx);
  * sinks and sne, the particle counts, dt) makes the plain calls; the second captures the same calls from the ctx's stream into
  * a graph and launches it; from the third on the call is one cudaGraphLaunch.  The kernels read particle data and state from
  * memory, so moving particles and evolving gas replay the same graph; any change of a pointer, a count or dt starts over with
- * plain calls.  Same results as the four calls (same kernels, same order).  Falls back to the plain calls, every time, when
- * the ctx's stream is a default stream (those cannot be captured) or the ctx has PM_FLAG_TIMING.  Not on a z slab (PM_EINVAL).
+ * plain calls.  Same results as the four calls (same kernels, same order).  The graph runs on a stream of the ctx's own, ordered
+ * after the work already in the ctx's stream and before what is enqueued there next (two events per call), so the ctx's stream
+ * may be a default stream.  With PM_FLAG_TIMING the plain calls are made every time.  Not on a z slab (PM_EINVAL).
  * Asynchronous; errors as for the four calls. */
 int pm_step_graph(pm_ctx *ctx, pm_state *state, pm_sinks *sinks, const pm_sne *sne, double dt);
 

@@ -100,6 +100,8 @@ struct pm_ctx {
     // pm_step_graph: the four calls of a step captured once into a CUDA graph and replayed while the arguments stay the same
     struct GraphKey { pm_state st; pm_sinks sk; pm_sne sn; double dt; } gkey;
     cudaGraphExec_t gexec;
+    cudaStream_t gstream; cudaEvent_t gev_in, gev_out;   // the graph runs on a stream of the ctx's own, ordered against the caller's
+                                                        // stream by two events: a default stream cannot be captured
     int gstate;         // 0: nothing; 1: gkey has run once eagerly (scratch memory is in place); 2: gexec replays gkey
     long long glaunches;   // kernels in the graph (pm_launch_count advances by this per replay)
     bool timing;        // PM_FLAG_TIMING
@@ -846,6 +848,7 @@ extern "C" int pm_destroy(pm_ctx *c) {
     if (c->timing)
         for (int k = 0; k < PM_NUM_KERNELS; ++k) { cudaEventDestroy(c->ev[k][0]); cudaEventDestroy(c->ev[k][1]); }
     if (c->gexec) cudaGraphExecDestroy(c->gexec);
+    if (c->gstream) { cudaStreamSynchronize(c->gstream); cudaStreamDestroy(c->gstream); cudaEventDestroy(c->gev_in); cudaEventDestroy(c->gev_out); }
     if (c->up_stream) {
         cudaStreamSynchronize(c->up_stream); cudaStreamSynchronize(c->down_stream);
         cudaStreamDestroy(c->up_stream); cudaStreamDestroy(c->down_stream);
@@ -1520,6 +1523,17 @@ static int step_calls(pm_ctx *c, pm_state *st, pm_sinks *sk, const pm_sne *sn, d
     return rc;
 }
 
+// The graph is captured from, and replayed on, a stream of the ctx's own (the caller's may be a default stream, which cannot be
+// captured); two events order it after what the caller's stream holds and the caller's stream after it.
+static int graph_launch(pm_ctx *c) {
+    PM_CUDA(c, cudaEventRecord(c->gev_in, c->stream));
+    PM_CUDA(c, cudaStreamWaitEvent(c->gstream, c->gev_in, 0));
+    PM_CUDA(c, cudaGraphLaunch(c->gexec, c->gstream));
+    PM_CUDA(c, cudaEventRecord(c->gev_out, c->gstream));
+    PM_CUDA(c, cudaStreamWaitEvent(c->stream, c->gev_out, 0));
+    return PM_OK;
+}
+
 extern "C" int pm_step_graph(pm_ctx *c, pm_state *st, pm_sinks *sk, const pm_sne *sn, double dt) {
     if (!c) return PM_EINVAL;
     if (!state_ok(st)) PM_FAIL(c, PM_EINVAL, "pm_step_graph: null state pointer");
@@ -1529,12 +1543,12 @@ extern "C" int pm_step_graph(pm_ctx *c, pm_state *st, pm_sinks *sk, const pm_sne
     key.st = *st; key.dt = dt;
     if (sk) key.sk = *sk;
     if (sn) key.sn = *sn;
-    // the legacy default stream cannot be captured, and the events of PM_FLAG_TIMING must not end up inside a graph
-    const bool capturable = c->stream != nullptr && c->stream != cudaStreamLegacy && c->stream != cudaStreamPerThread && !c->timing;
+    const bool capturable = !c->timing;      // the events of PM_FLAG_TIMING must not end up inside a graph
     const bool same = c->gstate > 0 && std::memcmp(&key, &c->gkey, sizeof(key)) == 0;
     if (capturable && same && c->gstate == 2) {
         PM_CUDA(c, cudaSetDevice(c->device));
-        PM_CUDA(c, cudaGraphLaunch(c->gexec, c->stream));
+        const int rc = graph_launch(c);
+        if (rc != PM_OK) return rc;
         // what the four calls leave behind on the host side
         c->launches += c->glaunches;
         c->n_sinks_dep = sk ? sk->n : 0; c->n_sne_dep = sn ? sn->n : 0; c->dt = dt;
@@ -1544,12 +1558,20 @@ extern "C" int pm_step_graph(pm_ctx *c, pm_state *st, pm_sinks *sk, const pm_sne
     }
     if (capturable && same && c->gstate == 1) {
         PM_CUDA(c, cudaSetDevice(c->device));
+        if (!c->gstream) {
+            PM_CUDA(c, cudaStreamCreateWithFlags(&c->gstream, cudaStreamNonBlocking));
+            PM_CUDA(c, cudaEventCreateWithFlags(&c->gev_in, cudaEventDisableTiming));
+            PM_CUDA(c, cudaEventCreateWithFlags(&c->gev_out, cudaEventDisableTiming));
+        }
         const long long l0 = c->launches;
+        cudaStream_t const user = c->stream;
         cudaGraph_t graph = nullptr;
-        cudaError_t e = cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal);
+        cudaError_t e = cudaStreamBeginCapture(c->gstream, cudaStreamCaptureModeThreadLocal);
         if (e == cudaSuccess) {
+            c->stream = c->gstream;                          // every launch of the four calls goes to c->stream
             const int rc = step_calls(c, st, sk, sn, dt);
-            e = cudaStreamEndCapture(c->stream, &graph);
+            c->stream = user;
+            e = cudaStreamEndCapture(c->gstream, &graph);
             if (rc == PM_OK && e == cudaSuccess && graph) {
                 if (c->gexec) { cudaGraphExecDestroy(c->gexec); c->gexec = nullptr; }
                 e = cudaGraphInstantiate(&c->gexec, graph, 0);
@@ -1557,8 +1579,7 @@ extern "C" int pm_step_graph(pm_ctx *c, pm_state *st, pm_sinks *sk, const pm_sne
                 if (e == cudaSuccess) {
                     c->glaunches = c->launches - l0;
                     c->gstate = 2;
-                    PM_CUDA(c, cudaGraphLaunch(c->gexec, c->stream));
-                    return PM_OK;
+                    return graph_launch(c);
                 }
             } else if (graph) cudaGraphDestroy(graph);
         }

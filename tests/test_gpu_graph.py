@@ -84,17 +84,27 @@ def test_graph_step_follows_the_oracle():
 
 def test_fallbacks_and_refusals():
     w = inputs.scaled_mixed(32, 200, seed_index=5)
-    # the default stream of torch is the legacy default stream: no capture, plain calls every time, same results
+    # the default stream of torch is the legacy default stream, which cannot be captured: the graph lives on a stream of the
+    # ctx's own, ordered against the default stream by events -- interleaved with torch work on the default stream
     c = pm.Context(w.params, device="cuda:0", flags=pm.PM_FLAG_REPRODUCIBLE)
     d = pm.Context(w.params, device="cuda:0", flags=pm.PM_FLAG_REPRODUCIBLE)
     sc, kc, nc = device_copy(w)
     sd, kd, nd = device_copy(w)
-    for _ in range(3):
+    for step in range(5):
+        sc.rho.mul_(1.0 + 1e-3 * step)                    # torch kernels on the default stream between the steps
+        sd.rho.mul_(1.0 + 1e-3 * step)
         c.pm_step_graph(sc, kc, nc, w.dt)
-        assert c.debug_graph_state() == 0                     # nothing to capture on a default stream
+        assert c.debug_graph_state() == min(step + 1, 2)
         plain_step(d, sd, kd, nd, w.dt)
-    for fa, fb in zip(sc.fields(), sd.fields()):
-        assert torch.equal(fa, fb)
+        for fa, fb in zip(sc.fields(), sd.fields()):
+            assert torch.equal(fa, fb), step
+    # PM_FLAG_TIMING: plain calls every time
+    t = pm.Context(w.params, device="cuda:0", flags=pm.PM_FLAG_TIMING)
+    for _ in range(3):
+        t.pm_step_graph(sc, kc, nc, w.dt)
+        assert t.debug_graph_state() == 0
+    assert t.pm_kernel_times()["sne"] > 0.0
+    t.close()
     # only SNe: no return pass, the ctx is left where pm_apply_limited leaves it
     e = pm.Context(w.params, device="cuda:0")
     e.pm_step_graph(sc, None, nc, w.dt)
