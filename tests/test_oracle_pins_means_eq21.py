@@ -183,3 +183,63 @@ def test_eq21_fallback_branch_R25():
     assert res[0][1][5] == pytest.approx(3.2 - 4.0 / 6.0, rel=1e-14) and res[0][1][5] < 3.0       # below e_min: the inequality cannot be met
     assert res[1][1][5] == pytest.approx(3.2 - 4.0 / 6.0, rel=1e-14)
     assert res[2][1][5] == 0.0
+
+
+def test_eq21_lambda_against_a_root_finder_that_shares_nothing_with_the_oracle():
+    """Eq. 21 (L238-241) on 500 random cells: lambda must be the LARGEST value in [0, 1] at which the inequality
+    |p_1 + lambda S_p|^2 / (2 rho_2) <= E_2 - e_min holds, found here by scanning the inequality itself on a fine grid from 1
+    downwards and bisecting the crossing -- no quadratic formula, no discriminant, no branch logic in common with the oracle.
+    The cells cover every case: not binding (lambda = 1), the inequality holding on [0, lambda], holding only on an interval
+    inside (0, 1) (momentum that first has to cancel p_1: two roots in [0, 1], the larger one counts), and holding nowhere (the
+    R25 fall-back, lambda = 0)."""
+    rng = np.random.default_rng(21)
+    cells = []
+    for q in range(500):
+        rho = float(rng.uniform(0.5, 2.0))
+        eint = float(rng.uniform(0.2, 2.0))
+        s_rho = float(rng.uniform(0.0, 1.0))
+        s_p = rng.normal(0.0, 3.0, size=3)
+        if q % 4 == 0:                                         # p_1 against S_p and a small energy budget: interval cases
+            p1 = -rng.uniform(0.2, 0.8) * s_p + rng.normal(0.0, 0.1, size=3)
+            s_e = float(rng.uniform(-0.9, 0.3) * eint)
+        else:
+            p1 = rng.normal(0.0, 1.5, size=3)
+            s_e = float(rng.uniform(-0.5, 6.0))
+        cells.append(dict(consistent(rho, tuple(float(x) for x in p1), eint), S=(s_rho, tuple(float(x) for x in s_p), s_e)))
+    res = apply_cells(cells)
+    kinds = {"from_zero": 0, "not_binding": 0, "fallback": 0, "interval": 0}
+    grid = np.linspace(1.0, 0.0, 20001)
+    for (lam, u), c in zip(res, cells):
+        rho2 = c["rho"] + c["S"][0]
+        e2 = c["E"] + c["S"][2]
+        emin = rho2 * c["eint"] / c["rho"]                     # theta = 1 (R25)
+        p1, sp = np.array(c["p"]), np.array(c["S"][1])
+
+        def slack(x):                                          # >= 0: the inequality holds at lambda = x (x: scalar or array)
+            v = p1[None, :] + np.atleast_1d(x)[:, None] * sp[None, :]
+            return (e2 - emin) - np.einsum("ij,ij->i", v, v) / (2.0 * rho2)
+
+        if slack(1.0)[0] >= 0.0:
+            want = 1.0
+            kinds["not_binding"] += 1
+        else:
+            ok = slack(grid) >= 0.0
+            if not ok.any():
+                want = 0.0
+                kinds["fallback"] += 1
+            else:
+                i = int(np.argmax(ok))                          # first grid point from the top where it holds
+                lo, hi = grid[i], grid[i - 1]                   # holds at lo, fails at hi
+                for _ in range(80):
+                    mid = 0.5 * (lo + hi)
+                    if slack(mid)[0] >= 0.0:
+                        lo = mid
+                    else:
+                        hi = mid
+                want = lo
+                kinds["from_zero" if slack(0.0)[0] >= 0.0 else "interval"] += 1
+        # the crossing is a root of a quadratic: its position moves by ~eps |terms| / |slope|; 2e-9 covers every case drawn
+        assert lam == pytest.approx(want, abs=2e-9), (lam, want, c)
+        if want == 0.0 and slack(0.0)[0] < 0.0:                 # fall-back: no momentum added, e_int clipped at >= 0 (R25)
+            assert u[5] >= 0.0
+    assert min(kinds.values()) >= 10, kinds
