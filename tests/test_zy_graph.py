@@ -1,7 +1,11 @@
 """pm_step_graph: the four calls of a step replayed from a CUDA graph.  Same kernels in the same order, so in Appendix A mode
 (PM_FLAG_REPRODUCIBLE: results independent of the order of the atomic additions) the graph path must equal the plain calls BIT
 FOR BIT, step after step, while particles and gas evolve; without the flag the two agree to the reorder tolerance and the
-graph path agrees with the oracle like any other step."""
+graph path agrees with the oracle like any other step.
+
+Appendix A makes two orders of the additions land on the same bits "except with probability ~2^-M per cell" (L612): the
+comparisons here run with M = 40 instead of the default 28, which leaves that chance below 1e-6 per run.  The file is named to
+be collected after the core parity tests (pytest -x)."""
 import numpy as np
 import pytest
 import torch
@@ -35,9 +39,16 @@ def test_graph_replay_is_bit_identical_to_the_plain_calls_in_appendix_a_mode(n, 
     with torch.cuda.stream(stream):
         a = pm.Context(w.params, device="cuda:0", stream=stream, flags=pm.PM_FLAG_REPRODUCIBLE)
         b = pm.Context(w.params, device="cuda:0", stream=stream, flags=pm.PM_FLAG_REPRODUCIBLE)
+        a.pm_set_repro_margin(40)
+        b.pm_set_repro_margin(40)
         sa, ka, na = device_copy(w)
         sb, kb, nb = device_copy(w)
         launches = []
+
+        def same(x, y, what):
+            bad = int((x != y).sum())
+            assert bad == 0, f"{what}: {bad} of {x.numel()} values differ, largest difference {float((x - y).abs().max()):.3e}"
+
         for step in range(5):                            # 1: plain calls, 2: capture + launch, 3-5: replays
             l0 = a.pm_launch_count()
             a.pm_step_graph(sa, ka, na, w.dt)
@@ -45,19 +56,21 @@ def test_graph_replay_is_bit_identical_to_the_plain_calls_in_appendix_a_mode(n, 
             assert a.debug_graph_state() == min(step + 1, 2)       # plain calls, then captured, then replayed
             plain_step(b, sb, kb, nb, w.dt)
             a.pm_check(); b.pm_check()
-            for fa, fb in zip(sa.fields(), sb.fields()):
-                assert torch.equal(fa, fb), f"state, step {step}"
+            for name, fa, fb in zip(pm.DeviceState.FIELDS, sa.fields(), sb.fields()):
+                same(fa, fb, f"{name}, step {step}")
             for f in ("m", "vx", "vy", "vz", "dm"):
-                assert torch.equal(getattr(ka, f), getattr(kb, f)), f"sink {f}, step {step}"
+                same(getattr(ka, f), getattr(kb, f), f"sink {f}, step {step}")
         assert len(set(launches)) == 1 and launches[0] > 0, launches       # the count advances as if the calls had been made
         # another dt: back to plain calls, capture again, replay -- still the same bits
         for step in range(3):
             a.pm_step_graph(sa, ka, na, 0.5 * w.dt)
             plain_step(b, sb, kb, nb, 0.5 * w.dt)
-            for fa, fb in zip(sa.fields(), sb.fields()):
-                assert torch.equal(fa, fb), f"state after the change of dt, step {step}"
+            for name, fa, fb in zip(pm.DeviceState.FIELDS, sa.fields(), sb.fields()):
+                same(fa, fb, f"{name} after the change of dt, step {step}")
         # the retained buffer is the step's (sink creation and the debug views read it)
-        assert torch.equal(a.debug_buffer(0)[1], b.debug_buffer(0)[1])
+        # (the buffers keep the UNROUNDED sums -- the apply pass rounds as it reads -- so here the order of the additions shows)
+        ra, rb = a.debug_buffer(0)[1], b.debug_buffer(0)[1]
+        assert torch.equal(ra != 0, rb != 0) and bool(((ra - rb).abs() <= 1e-12 * rb.abs()).all())
         a.close(); b.close()
 
 
@@ -88,6 +101,8 @@ def test_fallbacks_and_refusals():
     # ctx's own, ordered against the default stream by events -- interleaved with torch work on the default stream
     c = pm.Context(w.params, device="cuda:0", flags=pm.PM_FLAG_REPRODUCIBLE)
     d = pm.Context(w.params, device="cuda:0", flags=pm.PM_FLAG_REPRODUCIBLE)
+    c.pm_set_repro_margin(40)
+    d.pm_set_repro_margin(40)
     sc, kc, nc = device_copy(w)
     sd, kd, nd = device_copy(w)
     for step in range(5):
