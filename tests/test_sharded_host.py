@@ -113,3 +113,69 @@ def test_neighbours_and_self_exchange():
     rl, rh = torch.zeros(6), torch.zeros(6)
     sharded.exchange_slabs(a, b, rl, rh)                 # one rank: its low ghosts fold onto its own top planes and vice versa
     assert torch.equal(rh, a) and torch.equal(rl, b)
+
+
+class _FakeSlabCtx:
+    """Stands in for pm.Context in SlabStep's set-up and call sequence (no GPU): records what it is asked to do."""
+
+    def __init__(self, rank):
+        self.rank = rank
+        self.params = {"z_slab": 1, "nx": 8, "ny": 8, "nz": 8}
+        self.calls = []
+        self.connected = None
+
+        class _S:
+            def synchronize(self_inner):
+                self.calls.append("sync")
+        self.stream = _S()
+
+    def pm_slab_describe(self):
+        keys = [g + "_" + s for g in ("buf", "ret", "rtr") for s in ("send_lo", "send_hi", "recv_lo", "recv_hi")]
+        return dict({k: None for k in keys}, state_ghost_planes=4)
+
+    def pm_slab_ipc_export(self):
+        return ("handle-of-rank-%d" % self.rank).encode().ljust(64, b".")
+
+    def pm_slab_connect_ipc(self, lower, upper):
+        self.connected = (lower, upper)
+
+    def __getattr__(self, name):                     # pm_deposit, pm_slab_put, pm_fold_ghosts, ... : just note the order
+        if name.startswith("pm_"):
+            return lambda *a, **k: self.calls.append(name)
+        raise AttributeError(name)
+
+
+def _peer_worker(rank, world, port, out):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        ctx = _FakeSlabCtx(rank)
+        step = sharded.SlabStep(ctx, rank, world, peer_put=True)
+
+        class _NoFields:
+            def fields(self):
+                return []
+        step.step(_NoFields(), None, None, 0.1)
+        out[rank] = (ctx.connected, list(ctx.calls))
+    finally:
+        dist.destroy_process_group()
+
+
+def test_peer_put_setup_hands_every_rank_its_two_neighbours_handles_world3():
+    """SlabStep(peer_put=True): all ranks publish the IPC handle of their slab memory, every rank connects to the handle of
+    rank - 1 (its low ghost planes go there) and of rank + 1, periodic in the rank index; a step then puts, drains its stream
+    and meets the others BEFORE it folds.  Three ranks, so that lower and upper neighbour differ."""
+    world, port = 3, _free_port()
+    with mp.Manager() as m:
+        out = m.dict()
+        mp.spawn(_peer_worker, args=(world, port, out), nprocs=world, join=True)
+        res = dict(out)
+    h = lambda r: ("handle-of-rank-%d" % r).encode().ljust(64, b".")
+    for r in range(3):
+        connected, calls = res[r]
+        assert connected == (h((r - 1) % 3), h((r + 1) % 3))
+        assert calls == ["pm_deposit", "pm_slab_put", "sync", "pm_fold_ghosts", "pm_apply_limited", "pm_return_to_particles"]
+    # one rank: its own neighbour on both sides, no handle travels
+    ctx = _FakeSlabCtx(0)
+    sharded.SlabStep(ctx, 0, 1, peer_put=True)
+    assert ctx.connected == (None, None)
