@@ -1,7 +1,7 @@
 """z-slab decomposition with TWO PROCESSES, peer-memory form of Step 2: each rank's pack kernel stores its
 ghost planes straight into the other rank's receive slabs (pm_slab_put), the slab memory being mapped into the neighbour
 process through a CUDA IPC handle -- the mechanism that carries the transfer over NVLink when the ranks sit on different GPUs
-of a node.  This box has one GPU, so both ranks use cuda:0; no kernel of one rank ever waits for a kernel of the other (the only
+of a node.  This box has one GPU, so all ranks use cuda:0 (two ranks: both neighbours are the same peer; three: they differ); no kernel of one rank ever waits for a kernel of the other (the only
 synchronisation is "drain the stream, then a host barrier", sharded.SlabStep._landed).  The control plane is gloo; the state
 halo and the return-mesh fill-back travel through sharded.exchange_slabs (staged through host memory on this backend).
 
@@ -23,7 +23,7 @@ if ROOT not in sys.path:
 from paper_2509_18261_b200 import inputs  # noqa: E402
 
 pytestmark = pytest.mark.gpu
-N, NPART, SEED, STEPS = 40, 900, 12, 3
+N, NPART, SEED, STEPS = 48, 1400, 12, 3
 
 
 def _free_port():
@@ -32,14 +32,14 @@ def _free_port():
         return s.getsockname()[1]
 
 
-def workload():
+def workload(world):
     """The same on every rank and in the parent: seeded, a fifth of the particles within 3 cells of a cut."""
     w = inputs.scaled_mixed(N, NPART, seed_index=SEED)
-    h = N // 2
+    h = N // world
     rng = np.random.default_rng(SEED)
     for prt in (w.sinks, w.sne):
         k = max(prt.n // 5, 2)
-        prt.z[:k] = np.mod(rng.choice([0.0, float(h)], size=k) + rng.uniform(-3.0, 3.0, size=k), float(N))
+        prt.z[:k] = np.mod(rng.choice([float(h * r) for r in range(world)], size=k) + rng.uniform(-3.0, 3.0, size=k), float(N))
     return w
 
 
@@ -52,7 +52,7 @@ def _worker(rank, world, port, outdir):
     try:
         dev = torch.device("cuda:0")
         torch.cuda.set_device(dev)
-        w = workload()
+        w = workload(world)
         h = N // world
         z0 = rank * h
         p = dict(w.params, nz=h, z_slab=1)
@@ -90,7 +90,8 @@ def _worker(rank, world, port, outdir):
         dist.destroy_process_group()
 
 
-def test_two_processes_put_their_ghost_planes_into_each_other(tmp_path):
+@pytest.mark.parametrize("world", [2, 3])
+def test_processes_put_their_ghost_planes_into_each_other(tmp_path, world):
     mode = subprocess.run(["nvidia-smi", "--query-gpu=compute_mode", "--format=csv,noheader", "--id=0"],
                           capture_output=True, text=True).stdout.strip()
     if mode and mode != "Default":
@@ -98,12 +99,12 @@ def test_two_processes_put_their_ghost_planes_into_each_other(tmp_path):
     import torch.multiprocessing as mp
 
     from tests import parity
-    world, port = 2, _free_port()
+    port = _free_port()
     mp.spawn(_worker, args=(world, port, str(tmp_path)), nprocs=world, join=True)
     r = [np.load(os.path.join(str(tmp_path), f"rank{k}.npz")) for k in range(world)]
-    w = workload()
+    w = workload(world)
     o = parity.make_oracle(w)
-    parity.CONTEXT["test"] = "two_processes_peer_put"
+    parity.CONTEXT["test"] = f"{world}_processes_peer_put"
     for s in range(STEPS):
         o.step(w.dt)
         got = {f: np.concatenate([r[k][f"{f}{s}"] for k in range(world)], axis=0) for f in ("rho", "mx", "my", "mz", "etot", "eint")}
@@ -122,8 +123,8 @@ def test_two_processes_put_their_ghost_planes_into_each_other(tmp_path):
             assert np.all(np.abs(got[f] - ref) <= 1e-9 * (np.abs(ref) + np.abs(o.state.rho))), f"{f}, step {s}"
         assert np.all(np.abs(m - o.sinks.m) <= 1e-9 * np.abs(o.sinks.m)), f"sink m, step {s}"
     # sinks at the cuts really used the other rank's cells
-    h = N // 2
-    near = np.minimum(np.abs(w.sinks.z - h), np.minimum(w.sinks.z, N - w.sinks.z)) < 3.0
+    h = N // world
+    near = np.min(np.abs(w.sinks.z[:, None] - np.array([float(h * r) for r in range(world + 1)])[None, :]), axis=1) < 3.0
     assert near.sum() >= 2 and np.all(o.sink_diag["dm"][near] > 0)
     V = float(w.params["dx"]) ** 3
     mass = V * got["rho"].sum() + m.sum()
